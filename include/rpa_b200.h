@@ -1,0 +1,128 @@
+/* rpa_b200.h -- C-ABI of the B200-native static-subspace RPA correlation-energy hot path.
+ *
+ * Method: Weinberg et al., "Static Subspace Approximation for Random Phase Approximation
+ * Correlation Energies: Implementation and Performance" (arxiv 2405.20258); citations below are
+ * line numbers of /root/reference/PAPER.md.  Readings of ambiguous passages (R1..R18) are listed
+ * in DESIGN.md.
+ *
+ * Conventions that hold for every entry point
+ *   - complex128 = interleaved (re, im) doubles (cuDoubleComplex, torch.complex128).
+ *   - "dev" pointers are device pointers on the context's device, "host" pointers are host memory.
+ *     The caller owns every array it passes; the library never frees caller memory and keeps no
+ *     pointer past the call, except the workspace given to rpa_set_workspace.
+ *   - All device work is enqueued on the CUDA stream given to rpa_create (a cudaStream_t, e.g.
+ *     torch.cuda.current_stream().cuda_stream).  Calls return after enqueueing unless stated.
+ *   - Return value: 0 = RPA_OK, negative = error (outputs undefined); text via rpa_last_error.
+ *     The library never exits the process and never throws across this boundary.
+ *   - There is no CPU fallback: without a CUDA device every call fails with RPA_ERR_CUDA.
+ */
+#ifndef RPA_B200_H
+#define RPA_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rpa_ctx rpa_ctx; /* opaque, library-owned */
+
+enum {
+  RPA_OK = 0,
+  RPA_ERR_INVALID = -1,     /* null pointer, non-positive size, Miller index outside the grid,
+                               grid axis with a prime factor other than 2/3/5, n_eig > n_g, v < 0 */
+  RPA_ERR_WORKSPACE = -2,   /* workspace missing or too small (see rpa_workspace_bytes) */
+  RPA_ERR_CUDA = -3,        /* CUDA runtime error (message has the CUDA error string) */
+  RPA_ERR_NOT_POSDEF = -4,  /* Cholesky of 1 - chi_s broke down: chi_s not negative-semidefinite */
+  RPA_ERR_NO_CONVERGENCE = -5 /* subspace iteration / Jacobi hit its iteration cap */
+};
+
+/* Statement of the problem: cell, FFT grid, the epsilon G-sphere with v(q+G), and
+ * the wavefunction G-sphere.
+ *   cell   host [9]   row-major lattice vectors a1,a2,a3 in bohr (kept for reference only)
+ *   fft    host [3]   FFT grid (N1,N2,N3); every axis must factor into 2,3,5 and be <= 4096
+ *   g_eps  host [n_g][3]  Miller indices of the epsilon sphere, any order (order defines M's G order)
+ *   vcoul  host [n_g]     v(q+G) >= 0 (bare Coulomb 4 pi/(Omega |q+G|^2) in the configs)
+ *   g_wfn  host [n_pw][3] Miller indices of the wavefunction sphere, any order
+ *   |Miller index| must be < N/2 on each axis.  The pair product is alias-free (exact G-space
+ *   convolution) when 2 max|n_wfn| + max|n_eps| < N; the library does not require it.
+ *   device / cuda_stream: CUDA device ordinal and the caller's stream.
+ * Synchronises once (uploads plans: twiddles, index maps, v^1/2).                              */
+int rpa_create(rpa_ctx** out, const double cell[9], const int fft[3], int n_g, const int32_t* g_eps,
+               const double* vcoul, int n_pw, const int32_t* g_wfn, int device, void* cuda_stream);
+int rpa_destroy(rpa_ctx* ctx);
+const char* rpa_last_error(const rpa_ctx* ctx); /* valid until the next call on ctx; ctx may be NULL */
+
+/* Scratch memory: the caller allocates (e.g. a torch uint8 tensor) and lends it to the context.
+ * rpa_workspace_bytes = what the five stage calls below need for blocks of (nvb, nc) bands,
+ * n_eig basis vectors and n_w frequencies; rpa_energy_workspace_bytes = what rpa_energy_* needs. */
+size_t rpa_workspace_bytes(const rpa_ctx* ctx, int nvb, int nc, int n_eig, int n_w);
+size_t rpa_energy_workspace_bytes(const rpa_ctx* ctx, int nv, int nc, int nvb, int n_eig, int n_w);
+int rpa_set_workspace(rpa_ctx* ctx, void* dev_ptr, size_t bytes);
+
+/* (a1) MTXEL, PAPER.md:52 eq. 3, :96, :104-110; reading R7/R8.
+ *   u_n(r) = sum_G c_n(G) e^{+iG.r};  M[v][c][G] = (1/N_r) sum_r conj(u_v(r)) u_c(r) e^{-iG.r}, G on the
+ *   epsilon sphere.  psi_v dev [nvb][n_pw], psi_c dev [nc][n_pw] (rows = bands, sum_G |c|^2 = 1),
+ *   M dev out [nvb][nc][n_g], G fastest.  One valence block (eq. 14) per call.     */
+int rpa_mtxel(rpa_ctx* ctx, const void* psi_v, int nvb, const void* psi_c, int nc, void* M);
+
+/* (a2) CHI_SUM at omega = 0, eq. 6 with :71 eq. 5 and :152 eq. 15; readings R5/R6.
+ *   chi0[G][G'] (+)= - sum_{v,c} v^1/2(G) M[v][c][G] (2/Delta_vc) conj(M[v][c][G']) v^1/2(G'),
+ *   Delta_vc = e_c[c] - e_v[v] > 0.  e_v dev [nvb], e_c dev [nc].  accumulate: 0 overwrite, 1 add (the
+ *   sum over valence blocks).  chi0 dev in/out [n_g][n_g], both triangles written.              */
+int rpa_chi0_static(rpa_ctx* ctx, const void* M, int nvb, int nc, const double* e_v, const double* e_c,
+                    int accumulate, void* chi0);
+
+/* (a3) Static subspace basis; reading R9.  The n_eig eigenpairs of Hermitian chi0 with
+ *   the greatest |lambda| (chi0 is negative-semidefinite: the most negative ones).
+ *   C dev out [n_eig][n_g], row i = eigenvector i (unit 2-norm); lambda dev out [n_eig] ascending.
+ *   tol: relative residual target ||chi0 c_i - lambda_i c_i|| <= tol |lambda_1| (<= 0 selects 1e-11).
+ *   iters_out host, optional: subspace iterations used (0 = direct Jacobi of the whole matrix).
+ *   Synchronises (convergence is checked on the host).                                           */
+int rpa_subspace_basis(rpa_ctx* ctx, const void* chi0, int n_eig, double tol, void* C, double* lambda,
+                       int* iters_out);
+
+/* (a4) Projected chi_s(i omega_k), PAPER.md:84 eq. 7, :88 eq. 8, :158.
+ *   B_vc = C^H v^1/2 M_vc;  chi_s[k] (+)= - sum_vc B_vc D_vc(omega_k) B_vc^H,
+ *   D = 2 Delta/(Delta^2 + omega^2).  omega dev [n_w].  chi_s dev in/out [n_w][n_eig][n_eig].
+ *   C == NULL means the identity (n_eig must equal n_g): the full-basis chi~0(i omega_k).         */
+int rpa_chi_subspace_freq(rpa_ctx* ctx, const void* M, int nvb, int nc, const double* e_v,
+                          const double* e_c, const void* C, int n_eig, const double* omega, int n_w,
+                          int accumulate, void* chi_s);
+
+/* (a5) E_c, PAPER.md:35 eq. 1, :160, :174; reading R10.
+ *   per k: L L^H = 1 - chi_s[k];  t_k = 2 sum_i ln L_ii + Re Tr chi_s[k];  E_c = (1/2 pi) sum_k W_k t_k.
+ *   weight dev [n_w] (quadrature weight incl. Jacobian).  e_c host out; per_freq host out [n_w],
+ *   optional.  chi_s is not modified.  Synchronises.                                             */
+int rpa_correlation_energy(rpa_ctx* ctx, const void* chi_s, int n_eig, const double* weight, int n_w,
+                           double* e_c, double* per_freq);
+
+/* Whole path (PAPER.md:139-158 NV-block two-pass loop): for each valence block of nvb bands
+ * {a1, a2}; a3; for each block {a1, a4}; a5.  All inputs dev (rpa_energy_device) or host
+ * (rpa_energy_host: inputs are copied to the device and the scalar copied back inside the call).
+ *   psi_v [nv][n_pw], psi_c [nc][n_pw], e_v [nv], e_c [nc], omega/weight [n_w].
+ *   keep_m != 0: keep all M blocks resident and skip the second MTXEL pass when they fit in the
+ *   workspace (the single-block case of PAPER.md:158); otherwise recompute.
+ *   stage_ms host out [5], optional: device time of a1 (both passes), a2, a3, a4, a5 in ms.
+ *   lambda_out host [n_eig], per_freq host [n_w]: optional.  Synchronises.                       */
+int rpa_energy_device(rpa_ctx* ctx, const void* psi_v, int nv, const void* psi_c, int nc, const double* e_v,
+                      const double* e_c, int nvb, int n_eig, double tol, const double* omega,
+                      const double* weight, int n_w, int keep_m, double* e_c_out, double* lambda_out,
+                      double* per_freq, double* stage_ms);
+int rpa_energy_host(rpa_ctx* ctx, const void* psi_v, int nv, const void* psi_c, int nc, const double* e_v,
+                    const double* e_c, int nvb, int n_eig, double tol, const double* omega,
+                    const double* weight, int n_w, int keep_m, double* e_c_out, double* lambda_out,
+                    double* per_freq, double* stage_ms);
+
+/* Measurement helpers (bench.py / profiles): register-only FP64 peaks on the context's device.
+ *   kind 0: mma.sync m8n8k4 f64 (DMMA), kind 1: DFMA.  Returns TFLOP/s in *tflops; runs `iters`
+ *   launches of a fixed-size kernel on the context stream and synchronises.                      */
+int rpa_fp64_peak(rpa_ctx* ctx, int kind, int iters, double* tflops);
+/* Number of kernels launched by this context since creation (for bench.py's gpu_launches). */
+long long rpa_launch_count(const rpa_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RPA_B200_H */

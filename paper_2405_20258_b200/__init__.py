@@ -1,0 +1,12 @@
+"""B200-native static-subspace RPA correlation energy (arxiv 2405.20258) -- thin Python binding over the C-ABI
+library `librpa_b200.so` (include/rpa_b200.h).  Argument marshalling only: every step of the hot path runs in
+the library's CUDA kernels.  PyTorch supplies device memory and the CUDA stream, nothing else."""
+from .binding import (RpaContext, RpaError, load_library, library_path, EXPORTED_SYMBOLS,
+                      rpa_create, rpa_destroy, rpa_workspace_bytes, rpa_energy_workspace_bytes, rpa_set_workspace,
+                      rpa_mtxel, rpa_chi0_static, rpa_subspace_basis, rpa_chi_subspace_freq,
+                      rpa_correlation_energy, rpa_energy_device, rpa_energy_host, rpa_fp64_peak, rpa_launch_count)
+
+__all__ = ["RpaContext", "RpaError", "load_library", "library_path", "EXPORTED_SYMBOLS",
+           "rpa_create", "rpa_destroy", "rpa_workspace_bytes", "rpa_energy_workspace_bytes", "rpa_set_workspace",
+           "rpa_mtxel", "rpa_chi0_static", "rpa_subspace_basis", "rpa_chi_subspace_freq",
+           "rpa_correlation_energy", "rpa_energy_device", "rpa_energy_host", "rpa_fp64_peak", "rpa_launch_count"]

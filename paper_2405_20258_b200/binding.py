@@ -1,0 +1,249 @@
+"""ctypes binding with the same names as the C-ABI entry points of include/rpa_b200.h.
+
+Tensors are torch CUDA tensors (complex128 / float64, contiguous); the binding passes their data pointers and the
+current torch CUDA stream.  There is no fallback: if the shared library is missing or no CUDA device is present the
+calls raise."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB = None
+
+EXPORTED_SYMBOLS = [
+    "rpa_create", "rpa_destroy", "rpa_last_error", "rpa_workspace_bytes", "rpa_energy_workspace_bytes",
+    "rpa_set_workspace", "rpa_mtxel", "rpa_chi0_static", "rpa_subspace_basis", "rpa_chi_subspace_freq",
+    "rpa_correlation_energy", "rpa_energy_device", "rpa_energy_host", "rpa_fp64_peak", "rpa_launch_count",
+]
+
+
+class RpaError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"rpa error {code}: {msg}")
+        self.code = code
+
+
+def library_path() -> str:
+    return os.path.join(_HERE, "librpa_b200.so")
+
+
+def load_library(build_if_missing: bool = True):
+    """dlopen librpa_b200.so (building it in-tree with nvcc first if it is missing or stale)."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    path = library_path()
+    if build_if_missing:
+        from . import _build
+        try:
+            _build.build()
+        except Exception:
+            if not os.path.exists(path):
+                raise
+    if not os.path.exists(path):
+        raise RpaError(-3, f"{path} is missing: build it with `python -m paper_2405_20258_b200._build` (no CPU fallback)")
+    lib = C.CDLL(path)
+    vp, ci, cd, pd, pi = C.c_void_p, C.c_int, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_int)
+    lib.rpa_create.argtypes = [C.POINTER(vp), pd, pi, ci, C.POINTER(C.c_int32), pd, ci, C.POINTER(C.c_int32), ci, vp]
+    lib.rpa_create.restype = ci
+    lib.rpa_destroy.argtypes = [vp]
+    lib.rpa_destroy.restype = ci
+    lib.rpa_last_error.argtypes = [vp]
+    lib.rpa_last_error.restype = C.c_char_p
+    lib.rpa_workspace_bytes.argtypes = [vp, ci, ci, ci, ci]
+    lib.rpa_workspace_bytes.restype = C.c_size_t
+    lib.rpa_energy_workspace_bytes.argtypes = [vp, ci, ci, ci, ci, ci]
+    lib.rpa_energy_workspace_bytes.restype = C.c_size_t
+    lib.rpa_set_workspace.argtypes = [vp, vp, C.c_size_t]
+    lib.rpa_set_workspace.restype = ci
+    lib.rpa_mtxel.argtypes = [vp, vp, ci, vp, ci, vp]
+    lib.rpa_mtxel.restype = ci
+    lib.rpa_chi0_static.argtypes = [vp, vp, ci, ci, vp, vp, ci, vp]
+    lib.rpa_chi0_static.restype = ci
+    lib.rpa_subspace_basis.argtypes = [vp, vp, ci, cd, vp, vp, pi]
+    lib.rpa_subspace_basis.restype = ci
+    lib.rpa_chi_subspace_freq.argtypes = [vp, vp, ci, ci, vp, vp, vp, ci, vp, ci, ci, vp]
+    lib.rpa_chi_subspace_freq.restype = ci
+    lib.rpa_correlation_energy.argtypes = [vp, vp, ci, vp, ci, pd, pd]
+    lib.rpa_correlation_energy.restype = ci
+    energy_args = [vp, vp, ci, vp, ci, vp, vp, ci, ci, cd, vp, vp, ci, ci, pd, pd, pd, pd]
+    lib.rpa_energy_device.argtypes = energy_args
+    lib.rpa_energy_device.restype = ci
+    lib.rpa_energy_host.argtypes = energy_args
+    lib.rpa_energy_host.restype = ci
+    lib.rpa_fp64_peak.argtypes = [vp, ci, ci, pd]
+    lib.rpa_fp64_peak.restype = ci
+    lib.rpa_launch_count.argtypes = [vp]
+    lib.rpa_launch_count.restype = C.c_longlong
+    _LIB = lib
+    return lib
+
+
+def _check(ctx, rc):
+    if rc != 0:
+        msg = load_library().rpa_last_error(ctx)
+        raise RpaError(rc, msg.decode() if msg else "?")
+
+
+def _dev(t, dtype=None):
+    """device pointer of a contiguous CUDA tensor"""
+    import torch
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or not t.is_contiguous():
+        raise TypeError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"expected dtype {dtype}, got {t.dtype}")
+    return C.c_void_p(t.data_ptr())
+
+
+class RpaContext:
+    """Owns an rpa_ctx* and the workspace tensor lent to it."""
+
+    def __init__(self, handle, device):
+        self.handle = handle
+        self.device = device
+        self.workspace = None
+
+    def close(self):
+        if self.handle:
+            load_library().rpa_destroy(self.handle)
+            self.handle = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def rpa_create(cell, fft, g_eps, vcoul, g_wfn, device: int = 0, stream=None) -> RpaContext:
+    import torch
+    lib = load_library()
+    if not torch.cuda.is_available():
+        raise RpaError(-3, "no CUDA device: the RPA hot path has no CPU fallback")
+    cell = np.ascontiguousarray(cell, dtype=np.float64).reshape(9)
+    fft = np.ascontiguousarray(fft, dtype=np.int32).reshape(3)
+    g_eps = np.ascontiguousarray(g_eps, dtype=np.int32)
+    g_wfn = np.ascontiguousarray(g_wfn, dtype=np.int32)
+    vcoul = np.ascontiguousarray(vcoul, dtype=np.float64)
+    if stream is None:
+        stream = torch.cuda.current_stream(device).cuda_stream
+    h = C.c_void_p()
+    rc = lib.rpa_create(C.byref(h), cell.ctypes.data_as(C.POINTER(C.c_double)), fft.ctypes.data_as(C.POINTER(C.c_int)),
+                        g_eps.shape[0], g_eps.ctypes.data_as(C.POINTER(C.c_int32)),
+                        vcoul.ctypes.data_as(C.POINTER(C.c_double)), g_wfn.shape[0],
+                        g_wfn.ctypes.data_as(C.POINTER(C.c_int32)), device, C.c_void_p(stream))
+    _check(None, rc)
+    return RpaContext(h, device)
+
+
+def rpa_destroy(ctx: RpaContext):
+    ctx.close()
+
+
+def rpa_workspace_bytes(ctx, nvb, nc, n_eig, n_w) -> int:
+    return int(load_library().rpa_workspace_bytes(ctx.handle, nvb, nc, n_eig, n_w))
+
+
+def rpa_energy_workspace_bytes(ctx, nv, nc, nvb, n_eig, n_w) -> int:
+    return int(load_library().rpa_energy_workspace_bytes(ctx.handle, nv, nc, nvb, n_eig, n_w))
+
+
+def rpa_set_workspace(ctx, tensor):
+    """Lend a torch uint8 CUDA tensor as scratch memory (kept alive by the context)."""
+    ptr = _dev(tensor)
+    _check(ctx.handle, load_library().rpa_set_workspace(ctx.handle, ptr, tensor.numel() * tensor.element_size()))
+    ctx.workspace = tensor
+
+
+def rpa_mtxel(ctx, psi_v, psi_c, M):
+    import torch
+    nvb, nc = psi_v.shape[0], psi_c.shape[0]
+    _check(ctx.handle, load_library().rpa_mtxel(ctx.handle, _dev(psi_v, torch.complex128), nvb,
+                                                _dev(psi_c, torch.complex128), nc, _dev(M, torch.complex128)))
+    return M
+
+
+def rpa_chi0_static(ctx, M, e_v, e_c, accumulate, chi0):
+    import torch
+    _check(ctx.handle, load_library().rpa_chi0_static(ctx.handle, _dev(M, torch.complex128), e_v.shape[0], e_c.shape[0],
+                                                      _dev(e_v, torch.float64), _dev(e_c, torch.float64),
+                                                      int(bool(accumulate)), _dev(chi0, torch.complex128)))
+    return chi0
+
+
+def rpa_subspace_basis(ctx, chi0, n_eig, tol, Cmat, lam):
+    import torch
+    iters = C.c_int(0)
+    _check(ctx.handle, load_library().rpa_subspace_basis(ctx.handle, _dev(chi0, torch.complex128), n_eig, float(tol),
+                                                         _dev(Cmat, torch.complex128), _dev(lam, torch.float64),
+                                                         C.byref(iters)))
+    return iters.value
+
+
+def rpa_chi_subspace_freq(ctx, M, e_v, e_c, Cmat, n_eig, omega, accumulate, chi_s):
+    import torch
+    _check(ctx.handle, load_library().rpa_chi_subspace_freq(
+        ctx.handle, _dev(M, torch.complex128), e_v.shape[0], e_c.shape[0], _dev(e_v, torch.float64),
+        _dev(e_c, torch.float64), _dev(Cmat, torch.complex128) if Cmat is not None else None, n_eig,
+        _dev(omega, torch.float64), omega.shape[0], int(bool(accumulate)), _dev(chi_s, torch.complex128)))
+    return chi_s
+
+
+def rpa_correlation_energy(ctx, chi_s, n_eig, weight):
+    import torch
+    n_w = weight.shape[0]
+    e = C.c_double(0.0)
+    per = (C.c_double * n_w)()
+    _check(ctx.handle, load_library().rpa_correlation_energy(ctx.handle, _dev(chi_s, torch.complex128), n_eig,
+                                                             _dev(weight, torch.float64), n_w, C.byref(e), per))
+    return e.value, np.array(per[:])
+
+
+def _energy(fn_name, ctx, psi_v, psi_c, e_v, e_c, nvb, n_eig, tol, omega, weight, keep_m, ptr):
+    nv, nc, n_w = psi_v.shape[0], psi_c.shape[0], omega.shape[0]
+    e = C.c_double(0.0)
+    lam = (C.c_double * n_eig)()
+    per = (C.c_double * n_w)()
+    ms = (C.c_double * 5)()
+    fn = getattr(load_library(), fn_name)
+    _check(ctx.handle, fn(ctx.handle, ptr(psi_v), nv, ptr(psi_c), nc, ptr(e_v), ptr(e_c), int(nvb), int(n_eig), float(tol),
+                          ptr(omega), ptr(weight), n_w, int(bool(keep_m)), C.byref(e), lam, per, ms))
+    return dict(E_c=e.value, lam=np.array(lam[:]), t=np.array(per[:]),
+                stage_ms=dict(zip(("mtxel", "chi0_static", "basis", "chi_freq", "energy"), ms[:])))
+
+
+def rpa_energy_device(ctx, psi_v, psi_c, e_v, e_c, nvb, n_eig, tol, omega, weight, keep_m=False):
+    """All inputs are CUDA tensors."""
+    return _energy("rpa_energy_device", ctx, psi_v, psi_c, e_v, e_c, nvb, n_eig, tol, omega, weight, keep_m, _dev)
+
+
+def rpa_energy_host(ctx, psi_v, psi_c, e_v, e_c, nvb, n_eig, tol, omega, weight, keep_m=False):
+    """All inputs are HOST arrays (numpy, or CPU torch tensors, ideally pinned); copies happen inside the call."""
+    import torch
+
+    def hptr(a):
+        if isinstance(a, torch.Tensor):
+            if a.is_cuda or not a.is_contiguous():
+                raise TypeError("expected a contiguous CPU tensor")
+            return C.c_void_p(a.data_ptr())
+        if not isinstance(a, np.ndarray) or not a.flags["C_CONTIGUOUS"]:
+            raise TypeError("expected a C-contiguous numpy array")
+        return C.c_void_p(a.ctypes.data)
+
+    return _energy("rpa_energy_host", ctx, psi_v, psi_c, e_v, e_c, nvb, n_eig, tol, omega, weight, keep_m, hptr)
+
+
+def rpa_fp64_peak(ctx, kind: int, iters: int = 20) -> float:
+    t = C.c_double(0.0)
+    _check(ctx.handle, load_library().rpa_fp64_peak(ctx.handle, kind, iters, C.byref(t)))
+    return t.value
+
+
+def rpa_launch_count(ctx) -> int:
+    return int(load_library().rpa_launch_count(ctx.handle))

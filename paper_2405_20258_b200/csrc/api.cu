@@ -1,0 +1,363 @@
+// C-ABI of librpa_b200.so (include/rpa_b200.h): argument checking, workspace carving and the NV-block two-pass driver
+// (PAPER.md:139-158).  All arithmetic of the hot path runs in the CUDA kernels of the other translation units.
+#include <algorithm>
+#include <cmath>
+
+#include "rpa_internal.h"
+
+static thread_local std::string g_null_err;
+
+int rpa_fail(rpa_ctx* ctx, int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof(buf), fmt, ap);
+  va_end(ap);
+  if (ctx) ctx->err = buf; else g_null_err = buf;
+  return code;
+}
+
+namespace {
+
+__global__ void sqrt_kernel(const double* __restrict__ v, int n, double* __restrict__ out) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = sqrt(v[i]);
+}
+
+size_t chi_freq_vchunk(const rpa_ctx* ctx, int nvb, int nc, int n_eig) {
+  (void)ctx;
+  const size_t per_v = (size_t)nc * n_eig * sizeof(cplx);
+  size_t budget = (size_t)4 << 30;
+  size_t vc = std::max<size_t>(1, budget / std::max<size_t>(per_v, 1));
+  return std::min<size_t>(vc, (size_t)nvb);
+}
+size_t chi_freq_workspace(const rpa_ctx* ctx, int nvb, int nc, int n_eig) {
+  return ws_round(chi_freq_vchunk(ctx, nvb, nc, n_eig) * nc * n_eig * sizeof(cplx));
+}
+
+int do_chi0_static(rpa_ctx* ctx, const cplx* M, int nvb, int nc, const double* e_v, const double* e_c, int accumulate,
+                   cplx* chi0) {
+  ZgemmParams g;
+  g.A = M; g.lda = ctx->n_g; g.a_km = true; g.B = M; g.ldb = ctx->n_g; g.b_kn = true;
+  g.C = chi0; g.ldc = ctx->n_g; g.M = ctx->n_g; g.N = ctx->n_g; g.K = nvb * nc;
+  g.conj_b = true; g.herm = true; g.accumulate = accumulate != 0; g.alpha = -1.0;
+  g.rs = ctx->d_vsqrt; g.cs = ctx->d_vsqrt;
+  g.wmode = 1; g.e_v = e_v; g.e_c = e_c; g.nc = nc; g.omega = nullptr;
+  return zgemm_dmma(ctx, g);
+}
+
+int do_chi_freq(rpa_ctx* ctx, WsAlloc& ws, const cplx* M, int nvb, int nc, const double* e_v, const double* e_c, const cplx* C,
+                int n_eig, const double* omega, int n_w, int accumulate, cplx* chi_s) {
+  const int n_g = ctx->n_g;
+  if (!C) {  // full basis: chi~0(i w_k) directly from M
+    ZgemmParams g;
+    g.A = M; g.lda = n_g; g.a_km = true; g.B = M; g.ldb = n_g; g.b_kn = true;
+    g.C = chi_s; g.ldc = n_g; g.M = n_g; g.N = n_g; g.K = nvb * nc;
+    g.conj_b = true; g.herm = true; g.accumulate = accumulate != 0; g.alpha = -1.0;
+    g.rs = ctx->d_vsqrt; g.cs = ctx->d_vsqrt;
+    g.wmode = 1; g.e_v = e_v; g.e_c = e_c; g.nc = nc; g.omega = omega;
+    g.batch = n_w; g.strideC = (long long)n_g * n_g;
+    return zgemm_dmma(ctx, g);
+  }
+  const int vchunk = (int)chi_freq_vchunk(ctx, nvb, nc, n_eig);
+  cplx* Bp = ws.get<cplx>((size_t)vchunk * nc * n_eig);
+  if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_chi_subspace_freq: workspace too small (need %zu bytes)", ws.off);
+  for (int v0 = 0; v0 < nvb; v0 += vchunk) {
+    const int nv = std::min(vchunk, nvb - v0);
+    const int P = nv * nc;
+    // projection  Bp[p][i] = sum_G M[p][G] v^1/2(G) conj(C[i][G])        (eq. 7)
+    ZgemmParams g;
+    g.A = M + (long long)v0 * nc * n_g; g.lda = n_g; g.a_km = false;
+    g.B = C; g.ldb = n_g; g.b_kn = false;
+    g.C = Bp; g.ldc = n_eig; g.M = P; g.N = n_eig; g.K = n_g; g.conj_b = true;
+    g.wmode = 2; g.wk = ctx->d_vsqrt;
+    int rc = zgemm_dmma(ctx, g);
+    if (rc) return rc;
+    // chi_s[k] (+)= - sum_p Bp[p][:] D_p(w_k) Bp[p][:]^H                   (eq. 8)
+    ZgemmParams h;
+    h.A = Bp; h.lda = n_eig; h.a_km = true; h.B = Bp; h.ldb = n_eig; h.b_kn = true;
+    h.C = chi_s; h.ldc = n_eig; h.M = n_eig; h.N = n_eig; h.K = P;
+    h.conj_b = true; h.herm = true; h.accumulate = (accumulate != 0) || v0 > 0; h.alpha = -1.0;
+    h.wmode = 1; h.e_v = e_v + v0; h.e_c = e_c; h.nc = nc; h.omega = omega;
+    h.batch = n_w; h.strideC = (long long)n_eig * n_eig;
+    rc = zgemm_dmma(ctx, h);
+    if (rc) return rc;
+  }
+  return RPA_OK;
+}
+
+bool bad_ctx(rpa_ctx* ctx) { return ctx == nullptr; }
+
+}  // namespace
+
+extern "C" {
+
+int rpa_create(rpa_ctx** out, const double cell[9], const int fft[3], int n_g, const int32_t* g_eps, const double* vcoul,
+               int n_pw, const int32_t* g_wfn, int device, void* cuda_stream) {
+  if (!out) return rpa_fail(nullptr, RPA_ERR_INVALID, "rpa_create: out is null");
+  *out = nullptr;
+  if (!cell || !fft || !g_eps || !vcoul || !g_wfn) return rpa_fail(nullptr, RPA_ERR_INVALID, "rpa_create: null argument");
+  if (n_g <= 0 || n_pw <= 0) return rpa_fail(nullptr, RPA_ERR_INVALID, "rpa_create: n_g and n_pw must be positive");
+  for (int i = 0; i < n_g; i++)
+    if (!(vcoul[i] >= 0.0) || !std::isfinite(vcoul[i]))
+      return rpa_fail(nullptr, RPA_ERR_INVALID, "rpa_create: vcoul[%d] is negative or not finite", i);
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev <= 0)
+    return rpa_fail(nullptr, RPA_ERR_CUDA, "rpa_create: no CUDA device (%s); there is no CPU fallback",
+                    e == cudaSuccess ? "device count 0" : cudaGetErrorString(e));
+  if (device < 0 || device >= ndev) return rpa_fail(nullptr, RPA_ERR_INVALID, "rpa_create: device %d out of range", device);
+  rpa_ctx* ctx = new rpa_ctx();
+  ctx->device = device;
+  ctx->stream = (cudaStream_t)cuda_stream;
+  memcpy(ctx->cell, cell, sizeof(ctx->cell));
+  for (int a = 0; a < 3; a++) ctx->fft[a] = fft[a];
+  ctx->n_g = n_g; ctx->n_pw = n_pw;
+  auto fail = [&](int rc) { g_null_err = ctx->err; rpa_destroy(ctx); return rc; };
+  if ((e = cudaSetDevice(device)) != cudaSuccess) return fail(rpa_fail(ctx, RPA_ERR_CUDA, "cudaSetDevice: %s", cudaGetErrorString(e)));
+  cudaDeviceProp prop;
+  if ((e = cudaGetDeviceProperties(&prop, device)) != cudaSuccess)
+    return fail(rpa_fail(ctx, RPA_ERR_CUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e)));
+  ctx->sm_count = prop.multiProcessorCount;
+  if (prop.major < 10) return fail(rpa_fail(ctx, RPA_ERR_CUDA, "device %d is sm_%d%d; this library is built for sm_100a only", device, prop.major, prop.minor));
+  long long nr = 1;
+  for (int a = 0; a < 3; a++) {
+    if (fft[a] < 1) return fail(rpa_fail(ctx, RPA_ERR_INVALID, "rpa_create: fft[%d] = %d", a, fft[a]));
+    nr *= fft[a];
+  }
+  if (nr > 2147483647LL) return fail(rpa_fail(ctx, RPA_ERR_INVALID, "rpa_create: fft grid too large"));
+  ctx->n_r = (int)nr;
+  int rc = mtxel_plan_create(ctx, g_eps, g_wfn);
+  if (rc) return fail(rc);
+  double* d_v = nullptr;
+  if (cudaMalloc(&d_v, n_g * sizeof(double)) != cudaSuccess || cudaMalloc(&ctx->d_vsqrt, n_g * sizeof(double)) != cudaSuccess)
+    return fail(rpa_fail(ctx, RPA_ERR_CUDA, "rpa_create: cudaMalloc failed"));
+  cudaMemcpy(d_v, vcoul, n_g * sizeof(double), cudaMemcpyHostToDevice);
+  sqrt_kernel<<<(n_g + 255) / 256, 256, 0, ctx->stream>>>(d_v, n_g, ctx->d_vsqrt);
+  ctx->launches++;
+  e = cudaStreamSynchronize(ctx->stream);
+  cudaFree(d_v);
+  if (e != cudaSuccess) return fail(rpa_fail(ctx, RPA_ERR_CUDA, "rpa_create: %s", cudaGetErrorString(e)));
+  *out = ctx;
+  return RPA_OK;
+}
+
+int rpa_destroy(rpa_ctx* ctx) {
+  if (!ctx) return RPA_OK;
+  cudaSetDevice(ctx->device);
+  mtxel_plan_destroy(ctx);
+  cudaFree(ctx->d_vsqrt);
+  delete ctx;
+  return RPA_OK;
+}
+
+const char* rpa_last_error(const rpa_ctx* ctx) { return ctx ? ctx->err.c_str() : g_null_err.c_str(); }
+
+long long rpa_launch_count(const rpa_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+size_t rpa_workspace_bytes(const rpa_ctx* ctx, int nvb, int nc, int n_eig, int n_w) {
+  if (!ctx || nvb < 1 || nc < 1 || n_eig < 1 || n_w < 1) return 0;
+  size_t need = mtxel_workspace_bytes(ctx, nvb, nc);
+  need = std::max(need, basis_workspace_bytes(ctx, ctx->n_g, n_eig));
+  need = std::max(need, chi_freq_workspace(ctx, nvb, nc, n_eig));
+  need = std::max(need, energy_workspace_bytes(ctx, n_eig, n_w));
+  return need + 4096;
+}
+
+int rpa_set_workspace(rpa_ctx* ctx, void* dev_ptr, size_t bytes) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  if (dev_ptr && ((uintptr_t)dev_ptr & 255)) return rpa_fail(ctx, RPA_ERR_INVALID, "workspace must be 256-byte aligned");
+  ctx->ws = (char*)dev_ptr;
+  ctx->ws_bytes = dev_ptr ? bytes : 0;
+  return RPA_OK;
+}
+
+int rpa_mtxel(rpa_ctx* ctx, const void* psi_v, int nvb, const void* psi_c, int nc, void* M) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  if (!psi_v || !psi_c || !M || nvb < 1 || nc < 1) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_mtxel: invalid argument");
+  if ((long long)nvb * nc > 2147483647LL) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_mtxel: too many pairs in one block");
+  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
+  WsAlloc ws(ctx->ws, ctx->ws_bytes);
+  return mtxel_run(ctx, ws, (const cplx*)psi_v, nvb, (const cplx*)psi_c, nc, (cplx*)M);
+}
+
+int rpa_chi0_static(rpa_ctx* ctx, const void* M, int nvb, int nc, const double* e_v, const double* e_c, int accumulate,
+                    void* chi0) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  if (!M || !e_v || !e_c || !chi0 || nvb < 1 || nc < 1) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_chi0_static: invalid argument");
+  if ((long long)nvb * nc > 2147483647LL) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_chi0_static: too many pairs");
+  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
+  return do_chi0_static(ctx, (const cplx*)M, nvb, nc, e_v, e_c, accumulate, (cplx*)chi0);
+}
+
+int rpa_subspace_basis(rpa_ctx* ctx, const void* chi0, int n_eig, double tol, void* C, double* lambda, int* iters_out) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  if (!chi0 || !C || !lambda) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_subspace_basis: null argument");
+  if (n_eig < 1 || n_eig > ctx->n_g) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_subspace_basis: n_eig = %d not in 1..n_g = %d", n_eig, ctx->n_g);
+  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
+  WsAlloc ws(ctx->ws, ctx->ws_bytes);
+  return basis_run(ctx, ws, (const cplx*)chi0, ctx->n_g, n_eig, tol, (cplx*)C, lambda, iters_out);
+}
+
+int rpa_chi_subspace_freq(rpa_ctx* ctx, const void* M, int nvb, int nc, const double* e_v, const double* e_c, const void* C,
+                          int n_eig, const double* omega, int n_w, int accumulate, void* chi_s) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  if (!M || !e_v || !e_c || !omega || !chi_s || nvb < 1 || nc < 1 || n_w < 1)
+    return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_chi_subspace_freq: invalid argument");
+  if (n_eig < 1 || n_eig > ctx->n_g || (!C && n_eig != ctx->n_g))
+    return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_chi_subspace_freq: n_eig = %d invalid (n_g = %d, C %s)", n_eig, ctx->n_g, C ? "given" : "null");
+  if ((long long)nvb * nc > 2147483647LL) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_chi_subspace_freq: too many pairs");
+  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
+  WsAlloc ws(ctx->ws, ctx->ws_bytes);
+  return do_chi_freq(ctx, ws, (const cplx*)M, nvb, nc, e_v, e_c, (const cplx*)C, n_eig, omega, n_w, accumulate, (cplx*)chi_s);
+}
+
+int rpa_correlation_energy(rpa_ctx* ctx, const void* chi_s, int n_eig, const double* weight, int n_w, double* e_c,
+                           double* per_freq) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  if (!chi_s || !weight || !e_c || n_eig < 1 || n_w < 1) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_correlation_energy: invalid argument");
+  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
+  WsAlloc ws(ctx->ws, ctx->ws_bytes);
+  return energy_run(ctx, ws, (const cplx*)chi_s, n_eig, weight, n_w, e_c, per_freq);
+}
+
+int rpa_fp64_peak(rpa_ctx* ctx, int kind, int iters, double* tflops) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  if (!tflops || kind < 0 || kind > 1) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_fp64_peak: invalid argument");
+  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
+  return fp64_peak_kernel(ctx, kind, iters, tflops);
+}
+
+// ------------------------------------------------------------------------------------------------
+// whole path
+static size_t energy_persistent_bytes(const rpa_ctx* ctx, int nv, int nc, int nvb, int n_eig, int n_w, bool keep_all) {
+  const size_t n_g = ctx->n_g;
+  size_t b = ws_round(n_g * n_g * sizeof(cplx)) + ws_round((size_t)n_eig * n_g * sizeof(cplx)) + ws_round(n_eig * sizeof(double)) +
+             ws_round((size_t)n_w * n_eig * n_eig * sizeof(cplx));
+  b += ws_round((size_t)(keep_all ? nv : nvb) * nc * n_g * sizeof(cplx));
+  return b;
+}
+
+size_t rpa_energy_workspace_bytes(const rpa_ctx* ctx, int nv, int nc, int nvb, int n_eig, int n_w) {
+  if (!ctx || nv < 1 || nc < 1 || n_eig < 1 || n_w < 1) return 0;
+  if (nvb < 1 || nvb > nv) nvb = nv;
+  const size_t inputs = ws_round((size_t)nv * ctx->n_pw * sizeof(cplx)) + ws_round((size_t)nc * ctx->n_pw * sizeof(cplx)) +
+                        ws_round(nv * sizeof(double)) + ws_round(nc * sizeof(double)) + 2 * ws_round(n_w * sizeof(double));
+  return inputs + energy_persistent_bytes(ctx, nv, nc, nvb, n_eig, n_w, false) + rpa_workspace_bytes(ctx, nvb, nc, n_eig, n_w);
+}
+
+int rpa_energy_device(rpa_ctx* ctx, const void* psi_v_, int nv, const void* psi_c_, int nc, const double* e_v, const double* e_c,
+                      int nvb, int n_eig, double tol, const double* omega, const double* weight, int n_w, int keep_m,
+                      double* e_c_out, double* lambda_out, double* per_freq, double* stage_ms) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  if (!psi_v_ || !psi_c_ || !e_v || !e_c || !omega || !weight || !e_c_out || nv < 1 || nc < 1 || n_w < 1)
+    return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_energy: invalid argument");
+  if (n_eig < 1 || n_eig > ctx->n_g) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_energy: n_eig = %d not in 1..%d", n_eig, ctx->n_g);
+  if (nvb < 1 || nvb > nv) nvb = nv;
+  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
+  const cplx* psi_v = (const cplx*)psi_v_;
+  const cplx* psi_c = (const cplx*)psi_c_;
+  const int n_g = ctx->n_g, n_pw = ctx->n_pw;
+  const int nblocks = (nv + nvb - 1) / nvb;
+  const size_t stage_need = rpa_workspace_bytes(ctx, nvb, nc, n_eig, n_w);
+  bool keep_all = keep_m && nblocks > 0 &&
+                  energy_persistent_bytes(ctx, nv, nc, nvb, n_eig, n_w, true) + stage_need <= ctx->ws_bytes;
+  if (nblocks == 1) keep_all = true;
+  WsAlloc ws(ctx->ws, ctx->ws_bytes);
+  cplx* chi0 = ws.get<cplx>((size_t)n_g * n_g);
+  cplx* C = ws.get<cplx>((size_t)n_eig * n_g);
+  double* lam = ws.get<double>(n_eig);
+  cplx* chi_s = ws.get<cplx>((size_t)n_w * n_eig * n_eig);
+  cplx* Mbuf = ws.get<cplx>((size_t)(keep_all ? nv : nvb) * nc * n_g);
+  if (!ws.ok || ws.off + stage_need > ctx->ws_bytes)
+    return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_energy: workspace too small (need %zu bytes, have %zu)", ws.off + stage_need,
+                    ctx->ws_bytes);
+  char* scratch = ctx->ws + ws.off;
+  const size_t scratch_bytes = ctx->ws_bytes - ws.off;
+
+  // stage timers: events are recorded around every stage call and summed after the final synchronisation
+  std::vector<cudaEvent_t> evs;
+  std::vector<int> ev_stage;
+  auto tic = [&](int stage) {
+    if (!stage_ms) return;
+    cudaEvent_t a; cudaEventCreate(&a); cudaEventRecord(a, ctx->stream); evs.push_back(a); ev_stage.push_back(stage);
+  };
+  auto toc = [&]() {
+    if (!stage_ms) return;
+    cudaEvent_t b; cudaEventCreate(&b); cudaEventRecord(b, ctx->stream); evs.push_back(b); ev_stage.push_back(-1);
+  };
+  auto cleanup = [&]() { for (auto e : evs) cudaEventDestroy(e); };
+  int rc = RPA_OK;
+  for (int b = 0; b < nblocks && !rc; b++) {  // pass 1: MTXEL + static CHI_SUM (eq. 15)
+    const int v0 = b * nvb, nb = std::min(nvb, nv - v0);
+    cplx* M = keep_all ? Mbuf + (size_t)v0 * nc * n_g : Mbuf;
+    WsAlloc s1(scratch, scratch_bytes);
+    tic(0); rc = mtxel_run(ctx, s1, psi_v + (size_t)v0 * n_pw, nb, psi_c, nc, M); toc();
+    if (rc) break;
+    tic(1); rc = do_chi0_static(ctx, M, nb, nc, e_v + v0, e_c, b > 0, chi0); toc();
+  }
+  if (!rc) {
+    WsAlloc s2(scratch, scratch_bytes);
+    tic(2); rc = basis_run(ctx, s2, chi0, n_g, n_eig, tol, C, lam, nullptr); toc();
+  }
+  for (int b = 0; b < nblocks && !rc; b++) {  // pass 2: (MTXEL again) + projected chi_s(i w)
+    const int v0 = b * nvb, nb = std::min(nvb, nv - v0);
+    cplx* M = keep_all ? Mbuf + (size_t)v0 * nc * n_g : Mbuf;
+    if (!keep_all) {
+      WsAlloc s1(scratch, scratch_bytes);
+      tic(0); rc = mtxel_run(ctx, s1, psi_v + (size_t)v0 * n_pw, nb, psi_c, nc, M); toc();
+      if (rc) break;
+    }
+    WsAlloc s3(scratch, scratch_bytes);
+    tic(3); rc = do_chi_freq(ctx, s3, M, nb, nc, e_v + v0, e_c, C, n_eig, omega, n_w, b > 0, chi_s); toc();
+  }
+  if (!rc) {
+    WsAlloc s4(scratch, scratch_bytes);
+    tic(4); rc = energy_run(ctx, s4, chi_s, n_eig, weight, n_w, e_c_out, per_freq); toc();
+  }
+  if (rc) { cleanup(); return rc; }
+  if (lambda_out) RPA_CUDA(ctx, cudaMemcpyAsync(lambda_out, lam, n_eig * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+  RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  if (stage_ms) {
+    for (int s = 0; s < 5; s++) stage_ms[s] = 0.0;
+    for (size_t i = 0; i + 1 < evs.size(); i += 2) {
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, evs[i], evs[i + 1]);
+      stage_ms[ev_stage[i]] += ms;
+    }
+  }
+  cleanup();
+  return RPA_OK;
+}
+
+int rpa_energy_host(rpa_ctx* ctx, const void* psi_v, int nv, const void* psi_c, int nc, const double* e_v, const double* e_c,
+                    int nvb, int n_eig, double tol, const double* omega, const double* weight, int n_w, int keep_m,
+                    double* e_c_out, double* lambda_out, double* per_freq, double* stage_ms) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  if (!psi_v || !psi_c || !e_v || !e_c || !omega || !weight || !e_c_out || nv < 1 || nc < 1 || n_w < 1)
+    return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_energy_host: invalid argument");
+  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
+  WsAlloc ws(ctx->ws, ctx->ws_bytes);
+  cplx* d_pv = ws.get<cplx>((size_t)nv * ctx->n_pw);
+  cplx* d_pc = ws.get<cplx>((size_t)nc * ctx->n_pw);
+  double* d_ev = ws.get<double>(nv);
+  double* d_ec = ws.get<double>(nc);
+  double* d_om = ws.get<double>(n_w);
+  double* d_wt = ws.get<double>(n_w);
+  if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_energy_host: workspace too small for the inputs (%zu bytes)", ws.off);
+  RPA_CUDA(ctx, cudaMemcpyAsync(d_pv, psi_v, (size_t)nv * ctx->n_pw * sizeof(cplx), cudaMemcpyHostToDevice, ctx->stream));
+  RPA_CUDA(ctx, cudaMemcpyAsync(d_pc, psi_c, (size_t)nc * ctx->n_pw * sizeof(cplx), cudaMemcpyHostToDevice, ctx->stream));
+  RPA_CUDA(ctx, cudaMemcpyAsync(d_ev, e_v, nv * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+  RPA_CUDA(ctx, cudaMemcpyAsync(d_ec, e_c, nc * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+  RPA_CUDA(ctx, cudaMemcpyAsync(d_om, omega, n_w * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+  RPA_CUDA(ctx, cudaMemcpyAsync(d_wt, weight, n_w * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+  // run on the remainder of the workspace
+  char* save_ws = ctx->ws; size_t save_bytes = ctx->ws_bytes;
+  ctx->ws = save_ws + ws.off; ctx->ws_bytes = save_bytes - ws.off;
+  int rc = rpa_energy_device(ctx, d_pv, nv, d_pc, nc, d_ev, d_ec, nvb, n_eig, tol, d_om, d_wt, n_w, keep_m, e_c_out, lambda_out,
+                             per_freq, stage_ms);
+  ctx->ws = save_ws; ctx->ws_bytes = save_bytes;
+  return rc;
+}
+
+}  // extern "C"

@@ -1,0 +1,320 @@
+// (a3) Static subspace basis: the n_eig eigenpairs of the Hermitian negative-semidefinite chi~0(0) with the greatest
+// |lambda| (reading R9).  Block subspace iteration with CholeskyQR orthonormalisation and an on-device
+// one-sided (Hestenes) Jacobi Rayleigh-Ritz, as north_star prescribes; when the block (n_eig + guard vectors) would
+// cover more than half of the matrix the iteration degenerates to its p = n case: Jacobi on chi~0(0) itself.
+//
+// Row convention throughout: a "vector" is a contiguous row.  Acol[i][:] is the i-th column of G V (G = -H >= 0),
+// Vcol[i][:] the i-th column of V.  Because G is Hermitian, Acol starts as conj(G).
+#include <algorithm>
+#include <cmath>
+#include <numeric>
+
+#include "rpa_internal.h"
+
+namespace {
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// block-wide sum of NV doubles per thread; result valid in all threads
+template <int NV>
+__device__ __forceinline__ void block_sum(double (&v)[NV], double* sh /* [NV][32] */) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+#pragma unroll
+  for (int k = 0; k < NV; k++) {
+    v[k] = warp_sum(v[k]);
+    if (lane == 0) sh[k * 32 + warp] = v[k];
+  }
+  __syncthreads();
+#pragma unroll
+  for (int k = 0; k < NV; k++) {
+    double x = lane < nw ? sh[k * 32 + lane] : 0.0;
+    v[k] = warp_sum(x);
+  }
+  __syncthreads();
+}
+
+// Acol = -conj(src) (src row-major n x n with leading dimension ld), Vcol = identity
+__global__ void jacobi_init_kernel(const cplx* __restrict__ src, long long ld, int n, cplx* __restrict__ A,
+                                   cplx* __restrict__ V, int negate_conj) {
+  const int i = blockIdx.x;
+  for (int k = threadIdx.x; k < n; k += blockDim.x) {
+    cplx x = src[(long long)i * ld + k];
+    A[(long long)i * n + k] = negate_conj ? make_double2(-x.x, x.y) : make_double2(-x.x, -x.y);
+    V[(long long)i * n + k] = make_double2(i == k ? 1.0 : 0.0, 0.0);
+  }
+}
+
+__global__ void row_norm2_max_kernel(const cplx* __restrict__ A, int n, double* out) {
+  __shared__ double sh[32];
+  double v[1] = {0.0};
+  const cplx* a = A + (long long)blockIdx.x * n;
+  for (int k = threadIdx.x; k < n; k += blockDim.x) v[0] += a[k].x * a[k].x + a[k].y * a[k].y;
+  block_sum<1>(v, sh);
+  if (threadIdx.x == 0) atomicMax((unsigned long long*)out, (unsigned long long)__double_as_longlong(v[0]));
+}
+
+// one round of the round-robin ordering: CTA k rotates the pair (i,j) of columns
+__global__ void __launch_bounds__(256) jacobi_round_kernel(cplx* __restrict__ A, cplx* __restrict__ V, int n, int m_even,
+                                                          int round, double rot_tol, const double* __restrict__ gmax,
+                                                          double* __restrict__ off_max) {
+  __shared__ double sh[4 * 32];
+  const int k = blockIdx.x;
+  int i, j;
+  if (k == 0) { i = m_even - 1; j = round; }
+  else { i = (round + k) % (m_even - 1); j = (round - k + (m_even - 1)) % (m_even - 1); }
+  if (i >= n || j >= n) return;
+  if (i > j) { int t = i; i = j; j = t; }
+  cplx* ai = A + (long long)i * n;
+  cplx* aj = A + (long long)j * n;
+  double v[4] = {0, 0, 0, 0};
+  for (int t = threadIdx.x; t < n; t += blockDim.x) {
+    cplx x = ai[t], y = aj[t];
+    v[0] += x.x * x.x + x.y * x.y;
+    v[1] += y.x * y.x + y.y * y.y;
+    v[2] += x.x * y.x + x.y * y.y;   // Re conj(x) y
+    v[3] += x.x * y.y - x.y * y.x;   // Im conj(x) y
+  }
+  block_sum<4>(v, sh);
+  const double alpha = v[0], beta = v[1];
+  const double gabs = sqrt(v[2] * v[2] + v[3] * v[3]);
+  const double null2 = 1e-24 * gmax[0];
+  if (alpha <= null2 && beta <= null2) return;   // two numerically null columns: nothing to resolve
+  const double denom = sqrt(alpha * beta);
+  if (!(denom > 0.0) || gabs == 0.0) return;
+  const double off = gabs / denom;
+  if (threadIdx.x == 0) atomicMax((unsigned long long*)off_max, (unsigned long long)__double_as_longlong(off));
+  if (off <= rot_tol) return;
+  const double zeta = (beta - alpha) / (2.0 * gabs);
+  const double t = (zeta >= 0.0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
+  const double c = 1.0 / sqrt(1.0 + t * t), s = c * t;
+  const double pr = v[2] / gabs, pi = v[3] / gabs;   // e^{i phi}
+  // a_i' = c a_i - s e^{-i phi} a_j ;  a_j' = s e^{i phi} a_i + c a_j
+  cplx* vi = V + (long long)i * n;
+  cplx* vj = V + (long long)j * n;
+  for (int tt = threadIdx.x; tt < 2 * n; tt += blockDim.x) {
+    cplx* pi_ = tt < n ? ai + tt : vi + (tt - n);
+    cplx* pj_ = tt < n ? aj + tt : vj + (tt - n);
+    cplx x = *pi_, y = *pj_;
+    cplx ey = make_double2(pr * y.x + pi * y.y, pr * y.y - pi * y.x);   // e^{-i phi} y
+    cplx ex = make_double2(pr * x.x - pi * x.y, pr * x.y + pi * x.x);   // e^{+i phi} x
+    *pi_ = make_double2(c * x.x - s * ey.x, c * x.y - s * ey.y);
+    *pj_ = make_double2(s * ex.x + c * y.x, s * ex.y + c * y.y);
+  }
+}
+
+// theta_i = Re v_i^H a_i (eigenvalue of G); lambda = -theta
+__global__ void rayleigh_kernel(const cplx* __restrict__ A, const cplx* __restrict__ V, int n, double* lam) {
+  __shared__ double sh[32];
+  double v[1] = {0.0};
+  const cplx* a = A + (long long)blockIdx.x * n;
+  const cplx* w = V + (long long)blockIdx.x * n;
+  for (int k = threadIdx.x; k < n; k += blockDim.x) v[0] += w[k].x * a[k].x + w[k].y * a[k].y;
+  block_sum<1>(v, sh);
+  if (threadIdx.x == 0) lam[blockIdx.x] = -v[0];
+}
+
+__global__ void gather_rows_kernel(const cplx* __restrict__ src, long long lds, const int* __restrict__ order, int ncols,
+                                   cplx* __restrict__ dst, long long ldd) {
+  const cplx* s = src + (long long)order[blockIdx.x] * lds;
+  cplx* d = dst + (long long)blockIdx.x * ldd;
+  for (int k = threadIdx.x; k < ncols; k += blockDim.x) d[k] = s[k];
+}
+
+__global__ void random_rows_kernel(cplx* X, long long total, unsigned long long seed) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+    unsigned long long z = seed + 0x9E3779B97F4A7C15ull * (unsigned long long)(2 * i + 1);
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull; z = (z ^ (z >> 27)) * 0x94D049BB133111EBull; z ^= z >> 31;
+    unsigned long long y = z * 0xD6E8FEB86659FD93ull; y ^= y >> 32;
+    X[i] = make_double2((double)(z >> 11) * (1.0 / 9007199254740992.0) - 0.5,
+                        (double)(y >> 11) * (1.0 / 9007199254740992.0) - 0.5);
+  }
+}
+
+// res[i] = || Y[i] - theta_i X[i] ||_2  (theta = lam[i])
+__global__ void residual_kernel(const cplx* __restrict__ X, const cplx* __restrict__ Y, const double* __restrict__ lam, int n,
+                                double* res) {
+  __shared__ double sh[32];
+  double v[1] = {0.0};
+  const cplx* x = X + (long long)blockIdx.x * n;
+  const cplx* y = Y + (long long)blockIdx.x * n;
+  const double th = lam[blockIdx.x];
+  for (int k = threadIdx.x; k < n; k += blockDim.x) {
+    double a = y[k].x - th * x[k].x, b = y[k].y - th * x[k].y;
+    v[0] += a * a + b * b;
+  }
+  block_sum<1>(v, sh);
+  if (threadIdx.x == 0) res[blockIdx.x] = sqrt(v[0]);
+}
+
+struct JacobiWs {
+  cplx* A; cplx* V; double* lam; int* order; double* scal;  // scal[0] = gmax, scal[1] = off_max
+};
+
+// Eigen-decomposition of G = -H (H given as src, Hermitian n x n).  On return lam_sorted (device, ascending = most
+// negative H eigenvalue first) and order (device) index the rows of jw.V (eigenvectors as rows).
+int jacobi_eigh(rpa_ctx* ctx, const cplx* src, long long ld, int n, bool src_is_hc, JacobiWs& jw, std::vector<int>& order_h,
+                std::vector<double>& lam_h) {
+  // src_is_hc: src already holds Hc = H^T (RR matrix), so Acol = -src; otherwise src = H and Acol = -conj(H)
+  jacobi_init_kernel<<<n, 256, 0, ctx->stream>>>(src, ld, n, jw.A, jw.V, src_is_hc ? 0 : 1);
+  RPA_LAUNCH_CHECK(ctx);
+  RPA_CUDA(ctx, cudaMemsetAsync(jw.scal, 0, 2 * sizeof(double), ctx->stream));
+  row_norm2_max_kernel<<<n, 256, 0, ctx->stream>>>(jw.A, n, jw.scal);
+  RPA_LAUNCH_CHECK(ctx);
+  const int m_even = (n + 1) & ~1;
+  const double stop = std::max(1e-14, 4.0 * std::sqrt((double)n) * 1.1e-16);
+  bool converged = n < 2;
+  for (int sweep = 0; sweep < 60 && !converged; sweep++) {
+    RPA_CUDA(ctx, cudaMemsetAsync(jw.scal + 1, 0, sizeof(double), ctx->stream));
+    for (int r = 0; r < m_even - 1; r++) {
+      jacobi_round_kernel<<<m_even / 2, 256, 0, ctx->stream>>>(jw.A, jw.V, n, m_even, r, 1e-15, jw.scal, jw.scal + 1);
+      ctx->launches++;
+    }
+    RPA_CUDA(ctx, cudaGetLastError());
+    double off = 0.0;
+    RPA_CUDA(ctx, cudaMemcpyAsync(&off, jw.scal + 1, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    converged = off <= stop;
+  }
+  if (!converged) return rpa_fail(ctx, RPA_ERR_NO_CONVERGENCE, "one-sided Jacobi did not converge in 60 sweeps (n = %d)", n);
+  rayleigh_kernel<<<n, 256, 0, ctx->stream>>>(jw.A, jw.V, n, jw.lam);
+  RPA_LAUNCH_CHECK(ctx);
+  lam_h.resize(n);
+  RPA_CUDA(ctx, cudaMemcpyAsync(lam_h.data(), jw.lam, n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+  RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  order_h.resize(n);
+  std::iota(order_h.begin(), order_h.end(), 0);
+  std::stable_sort(order_h.begin(), order_h.end(), [&](int a, int b) { return lam_h[a] < lam_h[b]; });
+  RPA_CUDA(ctx, cudaMemcpyAsync(jw.order, order_h.data(), n * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
+  return RPA_OK;
+}
+
+int block_size(int n, int n_eig) {
+  int p = std::max(2 * n_eig, n_eig + 16);
+  return std::min(p, n);
+}
+bool use_direct(int n, int n_eig) { return 2 * block_size(n, n_eig) > n; }
+
+}  // namespace
+
+size_t basis_workspace_bytes(const rpa_ctx* ctx, int n, int n_eig) {
+  (void)ctx;
+  const size_t small = ws_round((size_t)n * sizeof(double)) * 3 + ws_round((size_t)n * sizeof(int)) + 4 * 256;
+  if (use_direct(n, n_eig)) return 2 * ws_round((size_t)n * n * sizeof(cplx)) + small;
+  const size_t p = block_size(n, n_eig);
+  return 3 * ws_round(p * n * sizeof(cplx)) + 4 * ws_round(p * p * sizeof(cplx)) + small;
+}
+
+int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, double tol, cplx* C, double* lambda,
+              int* iters_out) {
+  if (tol <= 0.0) tol = 1e-11;
+  std::vector<int> order_h;
+  std::vector<double> lam_h;
+  JacobiWs jw;
+  jw.lam = ws.get<double>(n);
+  double* d_lam_sorted = ws.get<double>(n);
+  double* d_res = ws.get<double>(n);
+  jw.order = ws.get<int>(n);
+  jw.scal = ws.get<double>(4);
+  int* d_info = ws.get<int>(4);
+  int rc;
+  if (use_direct(n, n_eig)) {
+    jw.A = ws.get<cplx>((size_t)n * n);
+    jw.V = ws.get<cplx>((size_t)n * n);
+    if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_subspace_basis: workspace too small (need %zu bytes)", ws.off);
+    if ((rc = jacobi_eigh(ctx, chi0, n, n, false, jw, order_h, lam_h))) return rc;
+    gather_rows_kernel<<<n_eig, 256, 0, ctx->stream>>>(jw.V, n, jw.order, n, C, n);
+    RPA_LAUNCH_CHECK(ctx);
+    std::vector<double> ls(n_eig);
+    for (int i = 0; i < n_eig; i++) ls[i] = lam_h[order_h[i]];
+    RPA_CUDA(ctx, cudaMemcpyAsync(lambda, ls.data(), n_eig * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (iters_out) *iters_out = 0;
+    return RPA_OK;
+  }
+
+  // ---- block subspace iteration ----
+  const int p = block_size(n, n_eig);
+  cplx* X = ws.get<cplx>((size_t)p * n);
+  cplx* Y = ws.get<cplx>((size_t)p * n);
+  cplx* Z = ws.get<cplx>((size_t)p * n);
+  cplx* S = ws.get<cplx>((size_t)p * p);
+  cplx* Vs = ws.get<cplx>((size_t)p * p);
+  jw.A = ws.get<cplx>((size_t)p * p);
+  jw.V = ws.get<cplx>((size_t)p * p);
+  if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_subspace_basis: workspace too small (need %zu bytes)", ws.off);
+
+  auto gemm_apply = [&](const cplx* Xin, cplx* Yout) {  // Yout[j][G] = sum_G' chi0[G][G'] Xin[j][G']
+    ZgemmParams g;
+    g.A = Xin; g.lda = n; g.a_km = false; g.B = chi0; g.ldb = n; g.b_kn = true; g.C = Yout; g.ldc = n;
+    g.M = p; g.N = n; g.K = n; g.conj_b = true;
+    return zgemm_dmma(ctx, g);
+  };
+  auto gram = [&](const cplx* Ain, const cplx* Bin, cplx* out) {  // out[i][j] = sum_G Ain[i][G] conj(Bin[j][G])
+    ZgemmParams g;
+    g.A = Ain; g.lda = n; g.a_km = false; g.B = Bin; g.ldb = n; g.b_kn = false; g.C = out; g.ldc = p;
+    g.M = p; g.N = p; g.K = n; g.conj_b = true; g.herm = (Ain == Bin);
+    return zgemm_dmma(ctx, g);
+  };
+  auto rotate = [&](const cplx* Q, const cplx* Xin, cplx* Xout) {  // Xout[i][G] = sum_j Q[i][j] Xin[j][G]
+    ZgemmParams g;
+    g.A = Q; g.lda = p; g.a_km = false; g.B = Xin; g.ldb = n; g.b_kn = true; g.C = Xout; g.ldc = n;
+    g.M = p; g.N = n; g.K = p; g.conj_b = false;
+    return zgemm_dmma(ctx, g);
+  };
+  auto orthonormalise = [&](cplx* W) -> int {  // CholeskyQR: W W^H = L L^H, W <- L^{-1} W
+    int r;
+    if ((r = gram(W, W, S))) return r;
+    if ((r = zpotrf_batched(ctx, S, p, p, 1, 0, d_info))) return r;
+    if ((r = ztrsm_left_lower(ctx, S, p, p, W, n, n))) return r;
+    return RPA_OK;
+  };
+
+  random_rows_kernel<<<ctx->sm_count * 4, 256, 0, ctx->stream>>>(X, (long long)p * n, 0x2405ull);
+  RPA_LAUNCH_CHECK(ctx);
+  if ((rc = orthonormalise(X))) return rc;
+  if ((rc = orthonormalise(X))) return rc;
+  const int max_it = 400, rr_every = 6;
+  int it = 0;
+  bool done = false;
+  double worst = 0.0;
+  while (it < max_it && !done) {
+    for (int s = 0; s < rr_every; s++, it++) {   // power steps: X <- orth(chi0 X)
+      if ((rc = gemm_apply(X, Y))) return rc;
+      std::swap(X, Y);
+      if ((rc = orthonormalise(X))) return rc;
+    }
+    if ((rc = orthonormalise(X))) return rc;     // second pass (CholeskyQR2) before Rayleigh-Ritz
+    if ((rc = gemm_apply(X, Y))) return rc;      // Y = chi0 X
+    if ((rc = gram(Y, X, S))) return rc;         // Hc[i][j] = x_j^H chi0 x_i
+    if ((rc = jacobi_eigh(ctx, S, p, p, true, jw, order_h, lam_h))) return rc;
+    gather_rows_kernel<<<p, 256, 0, ctx->stream>>>(jw.V, p, jw.order, p, Vs, p);
+    RPA_LAUNCH_CHECK(ctx);
+    if ((rc = rotate(Vs, X, Z))) return rc;      // Ritz vectors
+    std::swap(X, Z);
+    if ((rc = rotate(Vs, Y, Z))) return rc;      // chi0 applied to the Ritz vectors
+    std::swap(Y, Z);
+    std::vector<double> ls(p);
+    for (int i = 0; i < p; i++) ls[i] = lam_h[order_h[i]];
+    RPA_CUDA(ctx, cudaMemcpyAsync(d_lam_sorted, ls.data(), p * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    residual_kernel<<<n_eig, 256, 0, ctx->stream>>>(X, Y, d_lam_sorted, n, d_res);
+    RPA_LAUNCH_CHECK(ctx);
+    std::vector<double> res(n_eig);
+    RPA_CUDA(ctx, cudaMemcpyAsync(res.data(), d_res, n_eig * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    worst = *std::max_element(res.begin(), res.end());
+    done = worst <= tol * std::fabs(ls[0]);
+  }
+  if (iters_out) *iters_out = it;
+  if (!done)
+    return rpa_fail(ctx, RPA_ERR_NO_CONVERGENCE, "subspace iteration: residual %.3e after %d iterations (target %.3e)", worst,
+                    it, tol);
+  RPA_CUDA(ctx, cudaMemcpy2DAsync(C, (size_t)n * sizeof(cplx), X, (size_t)n * sizeof(cplx), (size_t)n * sizeof(cplx), n_eig,
+                                  cudaMemcpyDeviceToDevice, ctx->stream));
+  RPA_CUDA(ctx, cudaMemcpyAsync(lambda, d_lam_sorted, n_eig * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+  RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  return RPA_OK;
+}

@@ -1,0 +1,394 @@
+// MTXEL (step a1): M[v][c][G] = (1/N_r) sum_r conj(u_v(r)) u_c(r) e^{-iG.r}, G on the epsilon sphere.
+// PAPER.md:52 eq. 3, :96, :104-110 ("batched FFT algorithm"); readings R7/R8 of DESIGN.md.
+//
+// B200 design (differs from the paper's vendor-FFT offload):
+//   * real-space functions u_n are stored plane-major [z][x][y] so one z-plane is contiguous;
+//   * pair_plane_kernel: one CTA per (conduction band c, plane z) keeps u_c(:,:,z) in shared memory and loops over
+//     the valence bands of the block: product, y-FFT, x-FFT restricted to the kept y-frequencies, and writes only
+//     the nk1 x nk2 kept (x,y)-frequencies: an ~11x data reduction before anything goes back to global memory;
+//   * z_fft_scatter: the remaining 1-D transforms along z on the pruned columns, fused with the gather onto the
+//     epsilon sphere and the 1/N_r normalisation.
+// All transforms are the hand-written shared-memory radix-8/4/2/3/5 FFT of fft_smem.cuh.
+#include <algorithm>
+#include <cmath>
+
+#include "fft_smem.cuh"
+#include "rpa_internal.h"
+
+using fftsm::Plan;
+
+struct AxisPlan {
+  int n = 0, n_pass = 0;
+  int radix[fftsm::MAX_PASS];
+  cplx* d_tw_fwd = nullptr;
+  cplx* d_tw_inv = nullptr;
+  int* d_perm = nullptr;
+  int nk = 0;            // number of distinct epsilon-sphere Miller indices on this axis
+  int* d_kpos = nullptr; // [nk] position (after the in-place passes) of each kept frequency
+  Plan fwd() const { Plan p; p.n = n; p.n_pass = n_pass; for (int i = 0; i < n_pass; i++) p.radix[i] = radix[i]; p.tw = d_tw_fwd; p.perm = d_perm; return p; }
+  Plan inv() const { Plan p = fwd(); p.tw = d_tw_inv; return p; }
+};
+
+struct MtxelPlan {
+  AxisPlan ax[3];        // 0: x (N1), 1: y (N2), 2: z (N3)
+  int* d_wfn_box = nullptr;  // [n_pw] index of each wavefunction G in the [z][x][y] box
+  int* d_inv_map = nullptr;  // [nk1*nk2*nk3] epsilon-sphere index of pruned-box point ((i1*nk2+i2)*nk3+i3), or -1
+};
+
+static bool factorize(int n, AxisPlan& ap) {
+  ap.n = n; ap.n_pass = 0;
+  const int rad[5] = {8, 4, 2, 3, 5};
+  for (int f : rad)
+    while (n % f == 0) {
+      if (ap.n_pass >= fftsm::MAX_PASS) return false;
+      ap.radix[ap.n_pass++] = f; n /= f;
+    }
+  return n == 1;
+}
+
+static int upload(rpa_ctx* ctx, void** dst, const void* src, size_t bytes) {
+  RPA_CUDA(ctx, cudaMalloc(dst, bytes ? bytes : 16));
+  if (bytes) RPA_CUDA(ctx, cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice));
+  return RPA_OK;
+}
+
+int mtxel_plan_create(rpa_ctx* ctx, const int32_t* g_eps, const int32_t* g_wfn) {
+  MtxelPlan* mp = new MtxelPlan();
+  ctx->mtxel = mp;
+  const int N[3] = {ctx->fft[0], ctx->fft[1], ctx->fft[2]};
+  std::vector<int> kidx[3];  // sorted distinct Miller indices per axis
+  for (int a = 0; a < 3; a++) {
+    AxisPlan& ap = mp->ax[a];
+    if (N[a] < 1 || N[a] > 1024 || !factorize(N[a], ap))
+      return rpa_fail(ctx, RPA_ERR_INVALID, "fft axis %d = %d must factor into 2,3,5 and be <= 1024", a, N[a]);
+    const int n = N[a];
+    std::vector<cplx> twf(n), twi(n);
+    for (int k = 0; k < n; k++) {
+      long double ang = 2.0L * 3.14159265358979323846264338327950288L * (long double)k / (long double)n;
+      twf[k] = make_double2((double)cosl(ang), (double)(-sinl(ang)));
+      twi[k] = make_double2((double)cosl(ang), (double)sinl(ang));
+    }
+    std::vector<int> perm(n);
+    for (int k = 0; k < n; k++) {
+      int kk = k, nn = n, pos = 0;
+      for (int ps = 0; ps < ap.n_pass; ps++) { int r = ap.radix[ps]; pos += (kk % r) * (nn / r); kk /= r; nn /= r; }
+      perm[k] = pos;
+    }
+    for (int g = 0; g < ctx->n_g; g++) {
+      int m = g_eps[3 * g + a];
+      if (2 * std::abs(m) >= n) return rpa_fail(ctx, RPA_ERR_INVALID, "g_eps[%d] axis %d index %d outside the grid", g, a, m);
+      kidx[a].push_back(m);
+    }
+    std::sort(kidx[a].begin(), kidx[a].end());
+    kidx[a].erase(std::unique(kidx[a].begin(), kidx[a].end()), kidx[a].end());
+    ap.nk = (int)kidx[a].size();
+    std::vector<int> kpos(ap.nk);
+    for (int i = 0; i < ap.nk; i++) kpos[i] = perm[((kidx[a][i] % n) + n) % n];
+    int rc;
+    if ((rc = upload(ctx, (void**)&ap.d_tw_fwd, twf.data(), n * sizeof(cplx)))) return rc;
+    if ((rc = upload(ctx, (void**)&ap.d_tw_inv, twi.data(), n * sizeof(cplx)))) return rc;
+    if ((rc = upload(ctx, (void**)&ap.d_perm, perm.data(), n * sizeof(int)))) return rc;
+    if ((rc = upload(ctx, (void**)&ap.d_kpos, kpos.data(), ap.nk * sizeof(int)))) return rc;
+  }
+  std::vector<int> box(ctx->n_pw);
+  for (int g = 0; g < ctx->n_pw; g++) {
+    int i[3];
+    for (int a = 0; a < 3; a++) {
+      int m = g_wfn[3 * g + a];
+      if (2 * std::abs(m) >= N[a]) return rpa_fail(ctx, RPA_ERR_INVALID, "g_wfn[%d] axis %d index %d outside the grid", g, a, m);
+      i[a] = ((m % N[a]) + N[a]) % N[a];
+    }
+    box[g] = (i[2] * N[0] + i[0]) * N[1] + i[1];
+  }
+  const int nk1 = mp->ax[0].nk, nk2 = mp->ax[1].nk, nk3 = mp->ax[2].nk;
+  std::vector<int> inv((size_t)nk1 * nk2 * nk3, -1);
+  for (int g = 0; g < ctx->n_g; g++) {
+    int i[3];
+    for (int a = 0; a < 3; a++)
+      i[a] = (int)(std::lower_bound(kidx[a].begin(), kidx[a].end(), g_eps[3 * g + a]) - kidx[a].begin());
+    size_t pb = ((size_t)i[0] * nk2 + i[1]) * nk3 + i[2];
+    if (inv[pb] >= 0) return rpa_fail(ctx, RPA_ERR_INVALID, "g_eps has a duplicate entry at %d", g);
+    inv[pb] = g;
+  }
+  int rc;
+  if ((rc = upload(ctx, (void**)&mp->d_wfn_box, box.data(), box.size() * sizeof(int)))) return rc;
+  if ((rc = upload(ctx, (void**)&mp->d_inv_map, inv.data(), inv.size() * sizeof(int)))) return rc;
+  return RPA_OK;
+}
+
+void mtxel_plan_destroy(rpa_ctx* ctx) {
+  MtxelPlan* mp = ctx->mtxel;
+  if (!mp) return;
+  for (int a = 0; a < 3; a++) {
+    cudaFree(mp->ax[a].d_tw_fwd); cudaFree(mp->ax[a].d_tw_inv); cudaFree(mp->ax[a].d_perm); cudaFree(mp->ax[a].d_kpos);
+  }
+  cudaFree(mp->d_wfn_box); cudaFree(mp->d_inv_map);
+  delete mp;
+  ctx->mtxel = nullptr;
+}
+
+// ---------------------------------------------------------------------------------------------
+// kernels
+namespace {
+
+// psi [nb][n_pw] -> zero-initialised boxes [nb][N_r] at box[g]
+__global__ void scatter_wfn_kernel(const cplx* __restrict__ psi, const int* __restrict__ box, int n_pw, long long n_r,
+                                   cplx* __restrict__ u) {
+  const int b = blockIdx.y;
+  for (int g = blockIdx.x * blockDim.x + threadIdx.x; g < n_pw; g += gridDim.x * blockDim.x)
+    u[(long long)b * n_r + box[g]] = psi[(long long)b * n_pw + g];
+}
+
+// Batched 1-D transform along one axis of data viewed as [outer][n][inner], TL lines per CTA in shared memory.
+// MODE 0: in place, natural-order write-back (inverse transforms of the wavefunctions).
+// MODE 1: forward along z of T[pair][z][J]; writes only the kept k3 and scatters them onto the epsilon sphere:
+//         M[(v*nc + c0 + cl)*n_g + g] = X * scale, pair = v*ncc + cl.
+struct ZScatter {
+  const int* kpos3; int nk3; const int* inv_map; cplx* M; int ncc, nc, c0, n_g; double scale;
+};
+template <bool INV, int MODE>
+__global__ void fft_axis_kernel(cplx* __restrict__ data, Plan pl, long long n_lines, int inner, int TL, ZScatter zs) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx* s = reinterpret_cast<cplx*>(smem_raw);
+  const int n = pl.n, pitch = n | 1;
+  const int tid = threadIdx.x, nthr = blockDim.x;
+  const long long line0 = (long long)blockIdx.x * TL;
+  const int nl = (int)min((long long)TL, n_lines - line0);
+  if (inner == 1) {
+    for (int idx = tid; idx < nl * n; idx += nthr) {
+      int l = idx / n, e = idx - l * n;
+      s[l * pitch + e] = data[(line0 + l) * n + e];
+    }
+  } else {
+    for (int idx = tid; idx < nl * n; idx += nthr) {
+      int e = idx / nl, l = idx - e * nl;
+      long long line = line0 + l, o = line / inner;
+      int i = (int)(line - o * inner);
+      s[l * pitch + e] = data[(o * n + e) * inner + i];
+    }
+  }
+  __syncthreads();
+  fftsm::fft_lines<INV>(s, pl, nl, nullptr, pitch, 1, tid, nthr);
+  if (MODE == 0) {
+    if (inner == 1) {
+      for (int idx = tid; idx < nl * n; idx += nthr) {
+        int l = idx / n, e = idx - l * n;
+        data[(line0 + l) * n + e] = s[l * pitch + pl.perm[e]];
+      }
+    } else {
+      for (int idx = tid; idx < nl * n; idx += nthr) {
+        int e = idx / nl, l = idx - e * nl;
+        long long line = line0 + l, o = line / inner;
+        int i = (int)(line - o * inner);
+        data[(o * n + e) * inner + i] = s[l * pitch + pl.perm[e]];
+      }
+    }
+  } else {
+    for (int idx = tid; idx < nl * zs.nk3; idx += nthr) {
+      int l = idx / zs.nk3, i3 = idx - l * zs.nk3;
+      long long line = line0 + l, pair = line / inner;
+      int j = (int)(line - pair * inner);
+      int g = zs.inv_map[j * zs.nk3 + i3];
+      if (g >= 0) {
+        long long v = pair / zs.ncc; int cl = (int)(pair - v * zs.ncc);
+        cplx x = s[l * pitch + zs.kpos3[i3]];
+        zs.M[(v * zs.nc + zs.c0 + cl) * zs.n_g + g] = make_double2(x.x * zs.scale, x.y * zs.scale);
+      }
+    }
+  }
+}
+
+// One CTA per (c, z): u_c plane resident in shared memory, loop over the valence bands of the block.
+//   T[((v*ncc + c)*N3 + z)*J + i1*nk2 + i2] = sum_{x,y} conj(u_v) u_c e^{-i(k1 x/N1 + k2 y/N2) 2 pi}
+template <int EPT>
+__global__ void pair_plane_kernel(const cplx* __restrict__ u_v, const cplx* __restrict__ u_c, int nvb, int ncc, int N1,
+                                  int N2, int N3, Plan px, Plan py, const int* __restrict__ kpos1,
+                                  const int* __restrict__ kpos2, int nk1, int nk2, cplx* __restrict__ T) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int P1 = N1 | 1, P2 = N2 | 1;
+  cplx* sc = reinterpret_cast<cplx*>(smem_raw);       // [N1][P2] u_c plane
+  cplx* wk = sc + N1 * P2;                            // [N1][P2] work plane
+  cplx* cb = wk + N1 * P2;                            // [nk2][P1] compacted kept-y columns, x contiguous
+  int* s_k1 = reinterpret_cast<int*>(cb + nk2 * P1);  // [nk1]
+  int* s_k2 = s_k1 + nk1;                             // [nk2]
+  const int tid = threadIdx.x, nthr = blockDim.x;
+  const int z = blockIdx.x / ncc, c = blockIdx.x - z * ncc;
+  const int plane = N1 * N2;
+  const long long n_r = (long long)plane * N3;
+  const cplx* ucp = u_c + (long long)c * n_r + (long long)z * plane;
+  for (int idx = tid; idx < plane; idx += nthr) {
+    int x = idx / N2, y = idx - x * N2;
+    sc[x * P2 + y] = ucp[idx];
+  }
+  for (int i = tid; i < nk1; i += nthr) s_k1[i] = kpos1[i];
+  for (int i = tid; i < nk2; i += nthr) s_k2[i] = kpos2[i];
+  cplx nxt[EPT > 0 ? EPT : 1];
+  const cplx* uvp = u_v + (long long)z * plane;
+  if (EPT > 0) {
+#pragma unroll
+    for (int e = 0; e < EPT; e++) {
+      int idx = tid + e * nthr;
+      if (idx < plane) nxt[e] = uvp[idx];
+    }
+  }
+  __syncthreads();
+  const int J = nk1 * nk2;
+  for (int v = 0; v < nvb; v++) {
+    // (a) product
+    if (EPT > 0) {
+#pragma unroll
+      for (int e = 0; e < EPT; e++) {
+        int idx = tid + e * nthr;
+        if (idx < plane) {
+          int x = idx / N2, y = idx - x * N2;
+          cplx a = nxt[e], b = sc[x * P2 + y];
+          wk[x * P2 + y] = make_double2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x);
+        }
+      }
+      if (v + 1 < nvb) {
+        const cplx* nx = uvp + (long long)(v + 1) * n_r;
+#pragma unroll
+        for (int e = 0; e < EPT; e++) {
+          int idx = tid + e * nthr;
+          if (idx < plane) nxt[e] = nx[idx];
+        }
+      }
+    } else {
+      const cplx* cur = uvp + (long long)v * n_r;
+      for (int idx = tid; idx < plane; idx += nthr) {
+        int x = idx / N2, y = idx - x * N2;
+        cplx a = cur[idx], b = sc[x * P2 + y];
+        wk[x * P2 + y] = make_double2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x);
+      }
+    }
+    __syncthreads();
+    // (b) y transforms on all N1 rows
+    fftsm::fft_lines<false>(wk, py, N1, nullptr, P2, 1, tid, nthr);
+    // (c) keep the nk2 needed y-frequencies, transposed so x is contiguous
+    for (int idx = tid; idx < nk2 * N1; idx += nthr) {
+      int i2 = idx / N1, x = idx - i2 * N1;
+      cb[i2 * P1 + x] = wk[x * P2 + s_k2[i2]];
+    }
+    __syncthreads();
+    // (d) x transforms on the nk2 kept columns
+    fftsm::fft_lines<false>(cb, px, nk2, nullptr, P1, 1, tid, nthr);
+    // (e) write the nk1 x nk2 kept frequencies of this plane
+    cplx* dst = T + (((long long)v * ncc + c) * N3 + z) * J;
+    for (int idx = tid; idx < J; idx += nthr) {
+      int i1 = idx / nk2, i2 = idx - i1 * nk2;
+      dst[idx] = cb[i2 * P1 + s_k1[i1]];
+    }
+  }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------
+// host side
+namespace {
+
+struct MtxelSizes {
+  int ncc;             // conduction bands per chunk
+  size_t u_v, u_c, t;  // bytes
+};
+
+MtxelSizes mtxel_sizes(const rpa_ctx* ctx, int nvb, int nc) {
+  const MtxelPlan* mp = ctx->mtxel;
+  const size_t n_r = (size_t)ctx->n_r;
+  const size_t J = (size_t)mp->ax[0].nk * mp->ax[1].nk;
+  const size_t per_c = n_r * sizeof(cplx) + (size_t)nvb * ctx->fft[2] * J * sizeof(cplx);
+  size_t budget = (size_t)1536 << 20;  // chunk the conduction bands so that u_c + T stay near 1.5 GB
+  int ncc = (int)std::max<size_t>(16, budget / per_c);
+  if (ncc > nc) ncc = nc;
+  MtxelSizes s;
+  s.ncc = ncc;
+  s.u_v = ws_round((size_t)nvb * n_r * sizeof(cplx));
+  s.u_c = ws_round((size_t)ncc * n_r * sizeof(cplx));
+  s.t = ws_round((size_t)nvb * ncc * ctx->fft[2] * J * sizeof(cplx));
+  return s;
+}
+
+int axis_tile_lines(int n) {
+  int pitch = n | 1;
+  int tl = (int)((64 * 1024) / (pitch * sizeof(cplx)));
+  tl &= ~7;
+  if (tl < 8) tl = 8;
+  if (tl > 64) tl = 64;
+  return tl;
+}
+
+template <bool INV, int MODE>
+int launch_axis(rpa_ctx* ctx, cplx* data, const Plan& pl, long long n_lines, int inner, const ZScatter& zs) {
+  const int tl = axis_tile_lines(pl.n);
+  const size_t smem = (size_t)tl * (pl.n | 1) * sizeof(cplx);
+  auto kern = fft_axis_kernel<INV, MODE>;
+  static bool attr = false;
+  if (!attr) { RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)); attr = true; }
+  const long long blocks = (n_lines + tl - 1) / tl;
+  if (blocks > 2147483647LL) return rpa_fail(ctx, RPA_ERR_INVALID, "fft grid too large");
+  kern<<<(unsigned)blocks, 256, smem, ctx->stream>>>(data, pl, n_lines, inner, tl, zs);
+  RPA_LAUNCH_CHECK(ctx);
+  return RPA_OK;
+}
+
+// psi [nb][n_pw] -> u [nb][z][x][y]
+int wfn_to_realspace(rpa_ctx* ctx, const cplx* psi, int nb, cplx* u) {
+  const MtxelPlan* mp = ctx->mtxel;
+  const int N1 = ctx->fft[0], N2 = ctx->fft[1], N3 = ctx->fft[2];
+  const long long n_r = ctx->n_r;
+  RPA_CUDA(ctx, cudaMemsetAsync(u, 0, (size_t)nb * n_r * sizeof(cplx), ctx->stream));
+  dim3 grid((ctx->n_pw + 255) / 256, nb);
+  scatter_wfn_kernel<<<grid, 256, 0, ctx->stream>>>(psi, mp->d_wfn_box, ctx->n_pw, n_r, u);
+  RPA_LAUNCH_CHECK(ctx);
+  ZScatter zs{};
+  int rc;
+  if ((rc = launch_axis<true, 0>(ctx, u, mp->ax[1].inv(), (long long)nb * N3 * N1, 1, zs))) return rc;        // y
+  if ((rc = launch_axis<true, 0>(ctx, u, mp->ax[0].inv(), (long long)nb * N3 * N2, N2, zs))) return rc;       // x
+  if ((rc = launch_axis<true, 0>(ctx, u, mp->ax[2].inv(), (long long)nb * N1 * N2, N1 * N2, zs))) return rc;  // z
+  return RPA_OK;
+}
+
+}  // namespace
+
+size_t mtxel_workspace_bytes(const rpa_ctx* ctx, int nvb, int nc) {
+  MtxelSizes s = mtxel_sizes(ctx, nvb, nc);
+  return s.u_v + s.u_c + s.t;
+}
+
+int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx* psi_c, int nc, cplx* M) {
+  const MtxelPlan* mp = ctx->mtxel;
+  const int N1 = ctx->fft[0], N2 = ctx->fft[1], N3 = ctx->fft[2];
+  const long long n_r = ctx->n_r;
+  const MtxelSizes sz = mtxel_sizes(ctx, nvb, nc);
+  cplx* u_v = ws.get<cplx>((size_t)nvb * n_r);
+  cplx* u_c = ws.get<cplx>((size_t)sz.ncc * n_r);
+  const int nk1 = mp->ax[0].nk, nk2 = mp->ax[1].nk, nk3 = mp->ax[2].nk, J = nk1 * nk2;
+  cplx* T = ws.get<cplx>((size_t)nvb * sz.ncc * N3 * J);
+  if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_mtxel: workspace too small (need %zu bytes)", ws.off);
+
+  const int plane = N1 * N2, P1 = N1 | 1, P2 = N2 | 1;
+  const size_t smem = ((size_t)2 * N1 * P2 + (size_t)nk2 * P1) * sizeof(cplx) + (size_t)(nk1 + nk2) * sizeof(int);
+  if (smem > 227 * 1024)
+    return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_mtxel: an xy plane of %d x %d does not fit in shared memory", N1, N2);
+  int nthr = ((plane / 8 + 31) / 32) * 32;
+  nthr = std::max(64, std::min(512, nthr));
+  const bool prefetch = plane <= 8 * nthr;
+  auto kern = prefetch ? pair_plane_kernel<8> : pair_plane_kernel<0>;
+  RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+
+  int rc;
+  if ((rc = wfn_to_realspace(ctx, psi_v, nvb, u_v))) return rc;
+  for (int c0 = 0; c0 < nc; c0 += sz.ncc) {
+    const int ncc = std::min(sz.ncc, nc - c0);
+    if ((rc = wfn_to_realspace(ctx, psi_c + (long long)c0 * ctx->n_pw, ncc, u_c))) return rc;
+    kern<<<(unsigned)(ncc * N3), nthr, smem, ctx->stream>>>(u_v, u_c, nvb, ncc, N1, N2, N3, mp->ax[0].fwd(),
+                                                            mp->ax[1].fwd(), mp->ax[0].d_kpos, mp->ax[1].d_kpos, nk1,
+                                                            nk2, T);
+    RPA_LAUNCH_CHECK(ctx);
+    ZScatter zs;
+    zs.kpos3 = mp->ax[2].d_kpos; zs.nk3 = nk3; zs.inv_map = mp->d_inv_map; zs.M = M;
+    zs.ncc = ncc; zs.nc = nc; zs.c0 = c0; zs.n_g = ctx->n_g; zs.scale = 1.0 / (double)n_r;
+    if ((rc = launch_axis<false, 1>(ctx, T, mp->ax[2].fwd(), (long long)nvb * ncc * J, J, zs))) return rc;
+  }
+  return RPA_OK;
+}

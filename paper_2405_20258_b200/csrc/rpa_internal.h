@@ -1,0 +1,116 @@
+// Internal declarations shared by the translation units of librpa_b200.so (not part of the C-ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdarg>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "rpa_b200.h"
+
+typedef double2 cplx;  // interleaved (re, im), same bytes as cuDoubleComplex / torch.complex128
+
+struct rpa_ctx {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  std::string err;
+  long long launches = 0;
+  int sm_count = 148;
+
+  // problem statement
+  double cell[9];
+  int fft[3];
+  int n_r = 0, n_g = 0, n_pw = 0;
+
+  // plans (device, owned)
+  struct MtxelPlan* mtxel = nullptr;  // FFT plans, index maps (mtxel.cu)
+  double* d_vsqrt = nullptr;           // [n_g]  v^1/2
+
+  // workspace lent by the caller
+  char* ws = nullptr;
+  size_t ws_bytes = 0;
+
+  cudaEvent_t ev[12];
+  bool ev_ok = false;
+};
+
+int rpa_fail(rpa_ctx* ctx, int code, const char* fmt, ...);
+#define RPA_CUDA(ctx, call)                                                              \
+  do {                                                                                   \
+    cudaError_t e__ = (call);                                                            \
+    if (e__ != cudaSuccess)                                                              \
+      return rpa_fail(ctx, RPA_ERR_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e__), \
+                      __FILE__, __LINE__);                                               \
+  } while (0)
+#define RPA_LAUNCH_CHECK(ctx)                                                            \
+  do {                                                                                   \
+    (ctx)->launches++;                                                                   \
+    cudaError_t e__ = cudaGetLastError();                                                \
+    if (e__ != cudaSuccess)                                                              \
+      return rpa_fail(ctx, RPA_ERR_CUDA, "kernel launch failed: %s (%s:%d)", cudaGetErrorString(e__), \
+                      __FILE__, __LINE__);                                               \
+  } while (0)
+
+// bump allocator over the caller's workspace (256-byte aligned)
+struct WsAlloc {
+  char* base;
+  size_t cap, off = 0;
+  bool ok = true;
+  WsAlloc(char* b, size_t c) : base(b), cap(c) {}
+  template <class T>
+  T* get(size_t n) {
+    size_t bytes = (n * sizeof(T) + 255) & ~size_t(255);
+    if (!base || off + bytes > cap) { ok = false; off += bytes; return nullptr; }
+    T* p = reinterpret_cast<T*>(base + off);
+    off += bytes;
+    return p;
+  }
+};
+static inline size_t ws_round(size_t bytes) { return (bytes + 255) & ~size_t(255); }
+
+// ---------------------------------------------------------------------------------------------
+// Complex FP64 GEMM on the DMMA (mma.sync m8n8k4 f64) path -- zgemm_dmma.cu
+//   C[m][n] (+)= alpha * rs[m] * cs[n] * sum_k w_k * A^(m,k) * opB(B^(n,k)),  opB = conj or identity.
+struct ZgemmParams {
+  const cplx* A = nullptr; long long lda = 0; bool a_km = false;  // a_km: A stored [k][m] (m fastest) else [m][k]
+  const cplx* B = nullptr; long long ldb = 0; bool b_kn = false;
+  cplx* C = nullptr; long long ldc = 0;
+  int M = 0, N = 0, K = 0;
+  bool conj_b = true;
+  bool herm = false;          // A^ == B^ rows: compute tiles with tile_m >= tile_n only, mirror the rest
+  bool accumulate = false;
+  double alpha = 1.0;
+  const double* rs = nullptr; // [M] optional
+  const double* cs = nullptr; // [N] optional
+  // k weights: mode 0 none, 1 pair weights 2 D/(D^2+w^2) with D = e_c[k % nc] - e_v[k / nc], 2 vector wk[k]
+  int wmode = 0;
+  const double* e_v = nullptr; const double* e_c = nullptr; int nc = 1;
+  const double* omega = nullptr;  // dev, [batch] (mode 1; nullptr = 0)
+  const double* wk = nullptr;
+  int batch = 1; long long strideA = 0, strideB = 0, strideC = 0;
+  int split_k = 0;            // 0 = choose automatically
+};
+int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p);
+int fp64_peak_kernel(rpa_ctx* ctx, int kind, int iters, double* tflops);
+
+// mtxel.cu
+int mtxel_plan_create(rpa_ctx* ctx, const int32_t* g_eps, const int32_t* g_wfn);
+void mtxel_plan_destroy(rpa_ctx* ctx);
+size_t mtxel_workspace_bytes(const rpa_ctx* ctx, int nvb, int nc);
+int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx* psi_c, int nc, cplx* M);
+
+// basis.cu
+size_t basis_workspace_bytes(const rpa_ctx* ctx, int n, int n_eig);
+int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, double tol, cplx* C, double* lambda,
+              int* iters_out);
+
+// energy.cu
+size_t energy_workspace_bytes(const rpa_ctx* ctx, int n_eig, int n_w);
+int energy_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi_s, int n_eig, const double* weight, int n_w, double* e_c,
+               double* per_freq);
+
+// chol.cu
+int zpotrf_batched(rpa_ctx* ctx, cplx* A, int n, long long lda, int batch, long long stride, int* d_info);
+int ztrsm_left_lower(rpa_ctx* ctx, const cplx* L, long long ldl, int p, cplx* X, long long ldx, int ncols);

@@ -1,0 +1,342 @@
+// Complex-FP64 GEMM / HERK on the FP64 tensor-core path of sm_100a (mma.sync.m8n8k4.f64 -> SASS DMMA.8x8x4).
+//
+// Serves CHI_SUM (PAPER.md:75 eq. 6, :127 eq. 13, :152 eq. 15), the projection M_s = M C_s (eq. 7),
+// chi_s = M_s^H Delta M_s (eq. 8) and the dense products of the subspace iteration.
+//
+//   C[m][n] (+)= alpha rs[m] cs[n] sum_k w_k A^(m,k) opB(B^(n,k))
+//
+// One complex MAC = 4 real DMMAs on (re, im) fragments:  Cre += Ar Br + Ai Bi ; Cim += Ai Br - Ar Bi  (opB = conj).
+// The diagonal weight w_k (Delta of eq. 5 in the D(i omega) form) is fused into the A fragment after it is read
+// from shared memory; v^1/2 is fused into the epilogue (rs, cs).  Operand tiles are staged global -> shared with
+// cp.async (16 B = one complex element) in a 2-3 stage ring, in their native interleaved layout; padding makes the
+// 128-bit fragment loads bank-conflict free (leading dimension = 2 mod 8 elements for [k][m], 4 mod 8 for [m][k]).
+#include "rpa_internal.h"
+
+namespace {
+
+constexpr int BM = 64, BN = 64, BK = 16;
+constexpr int NTHREADS = 128;          // 4 warps, 2 x 2, warp tile 32 x 32 complex
+constexpr int LD_KM = BM + 2;          // [k][m] layout: elements per k row
+constexpr int LD_MK = BK + 4;          // [m][k] layout: elements per m row
+constexpr int TILE_KM = BK * LD_KM;    // 1056 elements
+constexpr int TILE_MK = BM * LD_MK;    // 1280 elements
+
+__device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+               : "+d"(d0), "+d"(d1)
+               : "d"(a), "d"(b));
+}
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem, bool valid) {
+  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  int sz = valid ? 16 : 0;
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(sz));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+struct KArgs {
+  const cplx* A; long long lda;
+  const cplx* B; long long ldb;
+  cplx* C; long long ldc;
+  int M, N, K;
+  int conj_b, herm, accumulate, atomic;
+  double alpha;
+  const double* rs; const double* cs;
+  int wmode; const double* e_v; const double* e_c; int nc; const double* omega; const double* wk;
+  long long strideA, strideB, strideC;
+  int tiles_n, kt_per_split, n_kt;
+};
+
+template <bool KM>
+__device__ __forceinline__ void load_tile(cplx* s, const cplx* g, long long ld, int r0, int rmax, int k0, int kmax,
+                                          int tid) {
+  // r = the m (or n) index, k = contraction index.  8 x 16-byte cp.async per thread.
+#pragma unroll
+  for (int i = 0; i < (BM * BK) / NTHREADS; i++) {
+    int idx = tid + i * NTHREADS;
+    int r, k;
+    if (KM) { k = idx / BM; r = idx % BM; } else { r = idx / BK; k = idx % BK; }
+    bool ok = (r0 + r < rmax) && (k0 + k < kmax);
+    const cplx* src = g;
+    if (ok) src = KM ? g + (long long)(k0 + k) * ld + (r0 + r) : g + (long long)(r0 + r) * ld + (k0 + k);
+    cplx* dst = KM ? s + k * LD_KM + r : s + r * LD_MK + k;
+    cp_async16(dst, src, ok);
+  }
+}
+
+template <bool A_KM, bool B_KN, int STAGES>
+__global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int TA = A_KM ? TILE_KM : TILE_MK;
+  constexpr int TB = B_KN ? TILE_KM : TILE_MK;
+  cplx* sA = reinterpret_cast<cplx*>(smem_raw);
+  cplx* sB = sA + STAGES * TA;
+  double* sW = reinterpret_cast<double*>(sB + STAGES * TB);
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wm = warp >> 1, wn = warp & 1;
+  const int g = lane >> 2, q = lane & 3;
+
+  // tile coordinates
+  int tm, tn;
+  if (p.herm) {
+    int t = blockIdx.x;
+    tm = (int)((sqrt(8.0 * t + 1.0) - 1.0) * 0.5);
+    while ((tm + 1) * (tm + 2) / 2 <= t) tm++;
+    while (tm * (tm + 1) / 2 > t) tm--;
+    tn = t - tm * (tm + 1) / 2;
+  } else {
+    tm = blockIdx.x / p.tiles_n;
+    tn = blockIdx.x % p.tiles_n;
+  }
+  const int m0 = tm * BM, n0 = tn * BN;
+  const int batch = blockIdx.z;
+  const cplx* A = p.A + batch * p.strideA;
+  const cplx* B = p.B + batch * p.strideB;
+  cplx* C = p.C + batch * p.strideC;
+  const int kt0 = blockIdx.y * p.kt_per_split;
+  const int kt1 = min(p.n_kt, kt0 + p.kt_per_split);
+  const int nkt = kt1 - kt0;
+  if (nkt <= 0) return;
+  double om2 = 0.0;
+  if (p.wmode == 1 && p.omega) { double w = p.omega[batch]; om2 = w * w; }
+
+  auto load_stage = [&](int stage, int kt) {
+    const int k0 = kt * BK;
+    load_tile<A_KM>(sA + stage * TA, A, p.lda, m0, p.M, k0, p.K, tid);
+    load_tile<B_KN>(sB + stage * TB, B, p.ldb, n0, p.N, k0, p.K, tid);
+    if (tid < BK) {
+      double w = 1.0;
+      int kk = k0 + tid;
+      if (kk >= p.K) w = 0.0;
+      else if (p.wmode == 1) {
+        int v = kk / p.nc, c = kk - v * p.nc;
+        double d = p.e_c[c] - p.e_v[v];
+        w = 2.0 * d / (d * d + om2);
+      } else if (p.wmode == 2) w = p.wk[kk];
+      sW[stage * BK + tid] = w;
+    }
+  };
+
+  double cre[4][4][2], cim[4][4][2];
+#pragma unroll
+  for (int i = 0; i < 4; i++)
+#pragma unroll
+    for (int j = 0; j < 4; j++) { cre[i][j][0] = cre[i][j][1] = 0.0; cim[i][j][0] = cim[i][j][1] = 0.0; }
+
+#pragma unroll
+  for (int s = 0; s < STAGES - 1; s++) {
+    if (s < nkt) load_stage(s, kt0 + s);
+    cp_async_commit();
+  }
+
+  for (int it = 0; it < nkt; it++) {
+    cp_async_wait<STAGES - 2>();
+    __syncthreads();
+    {
+      int nx = it + STAGES - 1;
+      if (nx < nkt) load_stage(nx % STAGES, kt0 + nx);
+      cp_async_commit();
+    }
+    const int st = it % STAGES;
+    const cplx* a_s = sA + st * TA;
+    const cplx* b_s = sB + st * TB;
+    const double* w_s = sW + st * BK;
+#pragma unroll
+    for (int k4 = 0; k4 < BK / 4; k4++) {
+      const int k = k4 * 4 + q;
+      const double w = w_s[k];
+      double ar[4], ai[4], nar[4], br[4], bi[4];
+#pragma unroll
+      for (int i = 0; i < 4; i++) {
+        const int m = wm * 32 + i * 8 + g;
+        cplx a = A_KM ? a_s[k * LD_KM + m] : a_s[m * LD_MK + k];
+        ar[i] = a.x * w; ai[i] = a.y * w; nar[i] = -ar[i];
+      }
+#pragma unroll
+      for (int j = 0; j < 4; j++) {
+        const int n = wn * 32 + j * 8 + g;
+        cplx b = B_KN ? b_s[k * LD_KM + n] : b_s[n * LD_MK + k];
+        br[j] = b.x; bi[j] = p.conj_b ? b.y : -b.y;
+      }
+#pragma unroll
+      for (int i = 0; i < 4; i++)
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+          dmma(cre[i][j][0], cre[i][j][1], ar[i], br[j]);
+          dmma(cim[i][j][0], cim[i][j][1], ai[i], br[j]);
+          dmma(cre[i][j][0], cre[i][j][1], ai[i], bi[j]);
+          dmma(cim[i][j][0], cim[i][j][1], nar[i], bi[j]);
+        }
+    }
+  }
+  cp_async_wait<0>();
+
+  // epilogue: scale, (mirror,) store / accumulate
+  const bool diag_tile = p.herm && (tm == tn);
+#pragma unroll
+  for (int i = 0; i < 4; i++) {
+    const int r = m0 + wm * 32 + i * 8 + g;
+    if (r >= p.M) continue;
+    const double sr = p.alpha * (p.rs ? p.rs[r] : 1.0);
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+#pragma unroll
+      for (int e = 0; e < 2; e++) {
+        const int c = n0 + wn * 32 + j * 8 + 2 * q + e;
+        if (c >= p.N) continue;
+        const double sc = sr * (p.cs ? p.cs[c] : 1.0);
+        double vr = sc * cre[i][j][e], vi = sc * cim[i][j][e];
+        if (diag_tile && r == c) vi = 0.0;
+        cplx* dst = C + (long long)r * p.ldc + c;
+        if (p.atomic) {
+          atomicAdd(&dst->x, vr); atomicAdd(&dst->y, vi);
+        } else if (p.accumulate) {
+          cplx o = *dst; o.x += vr; o.y += vi; *dst = o;
+        } else {
+          *dst = make_double2(vr, vi);
+        }
+        if (p.herm && !diag_tile) {
+          cplx* dm = C + (long long)c * p.ldc + r;
+          if (p.atomic) {
+            atomicAdd(&dm->x, vr); atomicAdd(&dm->y, -vi);
+          } else if (p.accumulate) {
+            cplx o = *dm; o.x += vr; o.y -= vi; *dm = o;
+          } else {
+            *dm = make_double2(vr, -vi);
+          }
+        }
+      }
+    }
+  }
+}
+
+template <bool A_KM, bool B_KN>
+int launch(rpa_ctx* ctx, const KArgs& ka, dim3 grid) {
+  constexpr int STAGES = (A_KM || B_KN) ? 3 : 2;
+  constexpr int TA = A_KM ? TILE_KM : TILE_MK;
+  constexpr int TB = B_KN ? TILE_KM : TILE_MK;
+  constexpr size_t smem = (size_t)STAGES * (TA + TB) * sizeof(cplx) + STAGES * BK * sizeof(double);
+  auto kern = zgemm_dmma_kernel<A_KM, B_KN, STAGES>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_set = true;
+  }
+  kern<<<grid, NTHREADS, smem, ctx->stream>>>(ka);
+  RPA_LAUNCH_CHECK(ctx);
+  return RPA_OK;
+}
+
+}  // namespace
+
+int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
+  if (p.M <= 0 || p.N <= 0 || p.batch <= 0) return RPA_OK;
+  if (p.herm && p.M != p.N) return rpa_fail(ctx, RPA_ERR_INVALID, "zgemm_dmma: herm needs M == N");
+  KArgs ka;
+  ka.A = p.A; ka.lda = p.lda; ka.B = p.B; ka.ldb = p.ldb; ka.C = p.C; ka.ldc = p.ldc;
+  ka.M = p.M; ka.N = p.N; ka.K = p.K;
+  ka.conj_b = p.conj_b; ka.herm = p.herm; ka.accumulate = p.accumulate;
+  ka.alpha = p.alpha; ka.rs = p.rs; ka.cs = p.cs;
+  ka.wmode = p.wmode; ka.e_v = p.e_v; ka.e_c = p.e_c; ka.nc = p.nc > 0 ? p.nc : 1; ka.omega = p.omega; ka.wk = p.wk;
+  ka.strideA = p.strideA; ka.strideB = p.strideB; ka.strideC = p.strideC;
+  const int tiles_m = (p.M + BM - 1) / BM, tiles_n = (p.N + BN - 1) / BN;
+  ka.tiles_n = tiles_n;
+  const long long tiles = p.herm ? (long long)tiles_m * (tiles_m + 1) / 2 : (long long)tiles_m * tiles_n;
+  const int n_kt = (p.K + BK - 1) / BK;
+  ka.n_kt = n_kt;
+  int split = p.split_k;
+  if (split <= 0) {
+    const long long want = 2LL * ctx->sm_count;  // two resident CTAs per SM
+    split = 1;
+    if (tiles * p.batch < want && n_kt >= 16) {
+      split = (int)((want + tiles * p.batch - 1) / (tiles * p.batch));
+      int max_split = n_kt / 8;  // at least 8 k-tiles (128 k) per split
+      if (split > max_split) split = max_split;
+      if (split < 1) split = 1;
+    }
+  }
+  if (n_kt == 0) split = 1;
+  ka.kt_per_split = n_kt > 0 ? (n_kt + split - 1) / split : 1;
+  split = n_kt > 0 ? (n_kt + ka.kt_per_split - 1) / ka.kt_per_split : 1;
+  ka.atomic = split > 1;
+  if (n_kt == 0 || (ka.atomic && !p.accumulate)) {
+    // zero C first (K == 0 gives C = 0 when not accumulating)
+    if (!p.accumulate) {
+      for (int b = 0; b < p.batch; b++)
+        RPA_CUDA(ctx, cudaMemset2DAsync(p.C + b * p.strideC, p.ldc * sizeof(cplx), 0, (size_t)p.N * sizeof(cplx), p.M,
+                                        ctx->stream));
+    }
+    if (n_kt == 0) return RPA_OK;
+  }
+  if (tiles > 2147483647LL || p.batch > 65535 || split > 65535)
+    return rpa_fail(ctx, RPA_ERR_INVALID, "zgemm_dmma: grid too large");
+  dim3 grid((unsigned)tiles, (unsigned)split, (unsigned)p.batch);
+  if (p.a_km && p.b_kn) return launch<true, true>(ctx, ka, grid);
+  if (p.a_km && !p.b_kn) return launch<true, false>(ctx, ka, grid);
+  if (!p.a_km && p.b_kn) return launch<false, true>(ctx, ka, grid);
+  return launch<false, false>(ctx, ka, grid);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Register-only FP64 peak microbenchmarks (rpa_fp64_peak): the roofline denominators for CHI_SUM (DMMA) and the
+// FFT butterflies (DFMA).  MEASURED_PEAKS.json has no FP64 entry, so bench.py measures these on the box.
+namespace {
+constexpr int PEAK_ITERS = 4096;
+__global__ void __launch_bounds__(256) dmma_peak_kernel(double* out) {
+  double acc[16][2];
+#pragma unroll
+  for (int i = 0; i < 16; i++) acc[i][0] = acc[i][1] = 0.0;
+  double a = 1.0 + threadIdx.x * 1e-9, b = 1.0 - threadIdx.x * 1e-9;
+  for (int it = 0; it < PEAK_ITERS; it++) {
+#pragma unroll
+    for (int i = 0; i < 16; i++) dmma(acc[i][0], acc[i][1], a, b);
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 16; i++) s += acc[i][0] + acc[i][1];
+  if (s == 123.456) out[0] = s;
+}
+__global__ void __launch_bounds__(256) dfma_peak_kernel(double* out) {
+  double acc[16];
+#pragma unroll
+  for (int i = 0; i < 16; i++) acc[i] = threadIdx.x * 1e-3 + i;
+  double a = 1.0 + threadIdx.x * 1e-12, b = 1e-9;
+  for (int it = 0; it < PEAK_ITERS; it++) {
+#pragma unroll
+    for (int i = 0; i < 16; i++) acc[i] = fma(acc[i], a, b);
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 16; i++) s += acc[i];
+  if (s == 123.456) out[0] = s;
+}
+}  // namespace
+
+int fp64_peak_kernel(rpa_ctx* ctx, int kind, int iters, double* tflops) {
+  if (!ctx->ws || ctx->ws_bytes < 8) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_fp64_peak needs a workspace");
+  if (iters < 1) iters = 1;
+  const int blocks = ctx->sm_count * 8;
+  cudaEvent_t e0, e1;
+  RPA_CUDA(ctx, cudaEventCreate(&e0));
+  RPA_CUDA(ctx, cudaEventCreate(&e1));
+  for (int rep = 0; rep < 2; rep++) {  // rep 0 = warm-up
+    RPA_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
+    for (int i = 0; i < iters; i++) {
+      if (kind == 0) dmma_peak_kernel<<<blocks, 256, 0, ctx->stream>>>((double*)ctx->ws);
+      else dfma_peak_kernel<<<blocks, 256, 0, ctx->stream>>>((double*)ctx->ws);
+      ctx->launches++;
+    }
+    RPA_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
+    RPA_CUDA(ctx, cudaEventSynchronize(e1));
+  }
+  float ms = 0;
+  RPA_CUDA(ctx, cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  const double warps = (double)blocks * 8;
+  const double flops = kind == 0 ? warps * PEAK_ITERS * 16.0 * (2.0 * 8 * 8 * 4) : warps * 32.0 * PEAK_ITERS * 16.0 * 2.0;
+  *tflops = flops * iters / (ms * 1e-3) / 1e12;
+  return RPA_OK;
+}
