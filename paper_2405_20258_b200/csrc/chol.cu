@@ -17,7 +17,10 @@ __device__ __forceinline__ cplx cmul_(cplx a, cplx b) {
 }
 
 // factor the nb x nb diagonal block at (k0,k0) of each matrix of the batch
-__global__ void __launch_bounds__(256) potf2_kernel(cplx* A, long long lda, long long stride, int k0, int nb, int* info) {
+// shift != 0: the stored diagonal is A_ii - 1 (deviation from the identity), pivots are 1 + stored, and the pivot
+// deviations d_i = L_ii^2 - 1 go to dvec (so ln det = sum log1p(d_i) keeps full relative accuracy for A close to 1).
+__global__ void __launch_bounds__(256) potf2_kernel(cplx* A, long long lda, long long stride, int k0, int nb, int* info,
+                                                    int shift, double* dvec, long long dstride) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx* s = reinterpret_cast<cplx*>(smem_raw);  // [nb][LDB]
   cplx* a = A + blockIdx.x * stride + (long long)k0 * lda + k0;
@@ -28,7 +31,9 @@ __global__ void __launch_bounds__(256) potf2_kernel(cplx* A, long long lda, long
   }
   __syncthreads();
   for (int j = 0; j < nb; j++) {
-    double d = s[j * LDB + j].x;
+    const double dev = s[j * LDB + j].x;
+    double d = shift ? 1.0 + dev : dev;
+    if (shift && dvec && tid == 0) dvec[blockIdx.x * dstride + k0 + j] = dev;
     if (!(d > 0.0)) {
       if (tid == 0 && info[blockIdx.x] == 0) info[blockIdx.x] = k0 + j + 1;
       d = 1.0;  // keep going with finite numbers; the caller reads info
@@ -121,8 +126,9 @@ __global__ void __launch_bounds__(TC) diag_solve_kernel(const cplx* L, long long
 }  // namespace
 
 // Lower Cholesky of `batch` Hermitian n x n matrices (row-major, lower triangle read), in place.  d_info[b] = 0 or
-// 1 + the first column with a non-positive pivot.
-int zpotrf_batched(rpa_ctx* ctx, cplx* A, int n, long long lda, int batch, long long stride, int* d_info) {
+// 1 + the first column with a non-positive pivot.  shift/dvec: see potf2_kernel (dvec is [batch][n]).
+int zpotrf_batched(rpa_ctx* ctx, cplx* A, int n, long long lda, int batch, long long stride, int* d_info, int shift,
+                   double* dvec) {
   RPA_CUDA(ctx, cudaMemsetAsync(d_info, 0, batch * sizeof(int), ctx->stream));
   const size_t smem = (size_t)NB * LDB * sizeof(cplx);
   static bool attr = false;
@@ -133,7 +139,7 @@ int zpotrf_batched(rpa_ctx* ctx, cplx* A, int n, long long lda, int batch, long 
   }
   for (int k0 = 0; k0 < n; k0 += NB) {
     const int nb = n - k0 < NB ? n - k0 : NB;
-    potf2_kernel<<<batch, 256, smem, ctx->stream>>>(A, lda, stride, k0, nb, d_info);
+    potf2_kernel<<<batch, 256, smem, ctx->stream>>>(A, lda, stride, k0, nb, d_info, shift, dvec, (long long)n);
     RPA_LAUNCH_CHECK(ctx);
     const int rem = n - k0 - nb;
     if (rem <= 0) break;

@@ -112,5 +112,6 @@ int energy_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi_s, int n_eig, const do
                double* per_freq);
 
 // chol.cu
-int zpotrf_batched(rpa_ctx* ctx, cplx* A, int n, long long lda, int batch, long long stride, int* d_info);
+int zpotrf_batched(rpa_ctx* ctx, cplx* A, int n, long long lda, int batch, long long stride, int* d_info, int shift = 0,
+                   double* dvec = nullptr);
 int ztrsm_left_lower(rpa_ctx* ctx, const cplx* L, long long ldl, int p, cplx* X, long long ldx, int ncols);
