@@ -116,8 +116,10 @@ __device__ __forceinline__ void pass(cplx* base, int n, int L, const cplx* __res
   }
 }
 
-// Full in-place transform of n_lines lines; ends with __syncthreads().
-template <bool INV>
+// Full in-place transform of n_lines lines.  WARP = false: all threads of the CTA take part (tid/nthr = thread index
+// and count), every pass ends with __syncthreads().  WARP = true: one warp transforms its own lines (tid = lane,
+// nthr = 32) and only __syncwarp() separates the passes, so warps run unsynchronised with each other.
+template <bool INV, bool WARP = false>
 __device__ __forceinline__ void fft_lines(cplx* base, const Plan& pl, int n_lines, const int* line_idx, int line_pitch,
                                           int elem_pitch, int tid, int nthr) {
   int L = pl.n;
@@ -131,7 +133,7 @@ __device__ __forceinline__ void fft_lines(cplx* base, const Plan& pl, int n_line
       default: pass<5, INV>(base, pl.n, L, pl.tw, n_lines, line_idx, line_pitch, elem_pitch, tid, nthr); break;
     }
     L /= r;
-    __syncthreads();
+    if (WARP) __syncwarp(); else __syncthreads();
   }
 }
 

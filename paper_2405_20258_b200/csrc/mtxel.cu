@@ -198,8 +198,12 @@ __global__ void fft_axis_kernel(cplx* __restrict__ data, Plan pl, long long n_li
   }
 }
 
-// One CTA per (c, z): u_c plane resident in shared memory, loop over the valence bands of the block.
-//   T[((v*ncc + c)*N3 + z)*J + i1*nk2 + i2] = sum_{x,y} conj(u_v) u_c e^{-i(k1 x/N1 + k2 y/N2) 2 pi}
+// One CTA per (c, z): the u_c plane stays in shared memory while the CTA loops over the valence bands of the block.
+//   T[((v*ncc + c)*N3 + z)*J + i1*nk2 + i2] = sum_{x,y} conj(u_v) u_c e^{-2 pi i (k1 x/N1 + k2 y/N2)}
+// Warp-private rows: warp w owns rows [w*LW, (w+1)*LW) of the plane; it forms the product for them, transforms them
+// along y and copies the nk2 kept y-frequencies into the (double-buffered, transposed) column buffer -- with only
+// __syncwarp() in between.  One __syncthreads() per valence band then separates that from the x transforms, which are
+// again distributed over the warps (LX kept columns each).  u_v rows of the next band are prefetched into registers.
 template <int EPT>
 __global__ void pair_plane_kernel(const cplx* __restrict__ u_v, const cplx* __restrict__ u_c, int nvb, int ncc, int N1,
                                   int N2, int N3, Plan px, Plan py, const int* __restrict__ kpos1,
@@ -207,11 +211,11 @@ __global__ void pair_plane_kernel(const cplx* __restrict__ u_v, const cplx* __re
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int P1 = N1 | 1, P2 = N2 | 1;
   cplx* sc = reinterpret_cast<cplx*>(smem_raw);       // [N1][P2] u_c plane
-  cplx* wk = sc + N1 * P2;                            // [N1][P2] work plane
-  cplx* cb = wk + N1 * P2;                            // [nk2][P1] compacted kept-y columns, x contiguous
-  int* s_k1 = reinterpret_cast<int*>(cb + nk2 * P1);  // [nk1]
+  cplx* wk = sc + N1 * P2;                            // [N1][P2] work plane (rows private to their warp)
+  cplx* cb0 = wk + N1 * P2;                           // 2 x [nk2][P1] kept y-frequencies, x contiguous
+  int* s_k1 = reinterpret_cast<int*>(cb0 + 2 * nk2 * P1);  // [nk1]
   int* s_k2 = s_k1 + nk1;                             // [nk2]
-  const int tid = threadIdx.x, nthr = blockDim.x;
+  const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
   const int z = blockIdx.x / ncc, c = blockIdx.x - z * ncc;
   const int plane = N1 * N2;
   const long long n_r = (long long)plane * N3;
@@ -222,61 +226,70 @@ __global__ void pair_plane_kernel(const cplx* __restrict__ u_v, const cplx* __re
   }
   for (int i = tid; i < nk1; i += nthr) s_k1[i] = kpos1[i];
   for (int i = tid; i < nk2; i += nthr) s_k2[i] = kpos2[i];
+  // this warp's rows (y transforms) and kept columns (x transforms)
+  const int LW = (N1 + nwarp - 1) / nwarp;
+  const int r0 = min(N1, warp * LW), r1 = min(N1, r0 + LW), nrow = r1 - r0;
+  const int LX = (nk2 + nwarp - 1) / nwarp;
+  const int j0 = min(nk2, warp * LX), j1 = min(nk2, j0 + LX), ncol = j1 - j0;
+  const int nel = nrow * N2;                          // contiguous elements of the plane owned by this warp
+  const cplx* uvp = u_v + (long long)z * plane + (long long)r0 * N2;
   cplx nxt[EPT > 0 ? EPT : 1];
-  const cplx* uvp = u_v + (long long)z * plane;
   if (EPT > 0) {
 #pragma unroll
     for (int e = 0; e < EPT; e++) {
-      int idx = tid + e * nthr;
-      if (idx < plane) nxt[e] = uvp[idx];
+      int idx = lane + e * 32;
+      if (idx < nel) nxt[e] = uvp[idx];
     }
   }
   __syncthreads();
   const int J = nk1 * nk2;
   for (int v = 0; v < nvb; v++) {
-    // (a) product
-    if (EPT > 0) {
+    cplx* cb = cb0 + (v & 1) * nk2 * P1;
+    if (nrow > 0) {
+      // (a) product on the warp's rows
+      if (EPT > 0) {
 #pragma unroll
-      for (int e = 0; e < EPT; e++) {
-        int idx = tid + e * nthr;
-        if (idx < plane) {
-          int x = idx / N2, y = idx - x * N2;
-          cplx a = nxt[e], b = sc[x * P2 + y];
+        for (int e = 0; e < EPT; e++) {
+          int idx = lane + e * 32;
+          if (idx < nel) {
+            int x = r0 + idx / N2, y = idx % N2;
+            cplx a = nxt[e], b = sc[x * P2 + y];
+            wk[x * P2 + y] = make_double2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x);
+          }
+        }
+        if (v + 1 < nvb) {
+          const cplx* nx = uvp + (long long)(v + 1) * n_r;
+#pragma unroll
+          for (int e = 0; e < EPT; e++) {
+            int idx = lane + e * 32;
+            if (idx < nel) nxt[e] = nx[idx];
+          }
+        }
+      } else {
+        const cplx* cur = uvp + (long long)v * n_r;
+        for (int idx = lane; idx < nel; idx += 32) {
+          int x = r0 + idx / N2, y = idx % N2;
+          cplx a = cur[idx], b = sc[x * P2 + y];
           wk[x * P2 + y] = make_double2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x);
         }
       }
-      if (v + 1 < nvb) {
-        const cplx* nx = uvp + (long long)(v + 1) * n_r;
-#pragma unroll
-        for (int e = 0; e < EPT; e++) {
-          int idx = tid + e * nthr;
-          if (idx < plane) nxt[e] = nx[idx];
-        }
-      }
-    } else {
-      const cplx* cur = uvp + (long long)v * n_r;
-      for (int idx = tid; idx < plane; idx += nthr) {
-        int x = idx / N2, y = idx - x * N2;
-        cplx a = cur[idx], b = sc[x * P2 + y];
-        wk[x * P2 + y] = make_double2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x);
+      __syncwarp();
+      // (b) y transforms of the warp's rows, then keep the nk2 needed y-frequencies (transposed: x contiguous)
+      fftsm::fft_lines<false, true>(wk + r0 * P2, py, nrow, nullptr, P2, 1, lane, 32);
+      for (int idx = lane; idx < nrow * nk2; idx += 32) {
+        int xr = idx % nrow, i2 = idx / nrow;
+        cb[i2 * P1 + r0 + xr] = wk[(r0 + xr) * P2 + s_k2[i2]];
       }
     }
     __syncthreads();
-    // (b) y transforms on all N1 rows
-    fftsm::fft_lines<false>(wk, py, N1, nullptr, P2, 1, tid, nthr);
-    // (c) keep the nk2 needed y-frequencies, transposed so x is contiguous
-    for (int idx = tid; idx < nk2 * N1; idx += nthr) {
-      int i2 = idx / N1, x = idx - i2 * N1;
-      cb[i2 * P1 + x] = wk[x * P2 + s_k2[i2]];
-    }
-    __syncthreads();
-    // (d) x transforms on the nk2 kept columns
-    fftsm::fft_lines<false>(cb, px, nk2, nullptr, P1, 1, tid, nthr);
-    // (e) write the nk1 x nk2 kept frequencies of this plane
-    cplx* dst = T + (((long long)v * ncc + c) * N3 + z) * J;
-    for (int idx = tid; idx < J; idx += nthr) {
-      int i1 = idx / nk2, i2 = idx - i1 * nk2;
-      dst[idx] = cb[i2 * P1 + s_k1[i1]];
+    if (ncol > 0) {
+      // (c) x transforms on the warp's kept columns, then write the nk1 kept x-frequencies
+      fftsm::fft_lines<false, true>(cb + j0 * P1, px, ncol, nullptr, P1, 1, lane, 32);
+      cplx* dst = T + (((long long)v * ncc + c) * N3 + z) * J;
+      for (int idx = lane; idx < ncol * nk1; idx += 32) {
+        int jc = idx % ncol, i1 = idx / ncol;
+        dst[i1 * nk2 + j0 + jc] = cb[(j0 + jc) * P1 + s_k1[i1]];
+      }
     }
   }
 }
@@ -367,12 +380,16 @@ int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx*
   if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_mtxel: workspace too small (need %zu bytes)", ws.off);
 
   const int plane = N1 * N2, P1 = N1 | 1, P2 = N2 | 1;
-  const size_t smem = ((size_t)2 * N1 * P2 + (size_t)nk2 * P1) * sizeof(cplx) + (size_t)(nk1 + nk2) * sizeof(int);
+  const size_t smem = ((size_t)2 * N1 * P2 + (size_t)2 * nk2 * P1) * sizeof(cplx) + (size_t)(nk1 + nk2) * sizeof(int);
   if (smem > 227 * 1024)
     return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_mtxel: an xy plane of %d x %d does not fit in shared memory", N1, N2);
-  int nthr = ((plane / 8 + 31) / 32) * 32;
-  nthr = std::max(64, std::min(512, nthr));
-  const bool prefetch = plane <= 8 * nthr;
+  // warps: about 32 lanes' worth of butterflies per warp in a radix-8 pass over its rows
+  int nwarp = (plane / 8 + 31) / 32;
+  nwarp = std::max(2, std::min(16, nwarp));
+  if (nwarp > N1) nwarp = N1;
+  const int nthr = nwarp * 32;
+  const int LW = (N1 + nwarp - 1) / nwarp;
+  const bool prefetch = LW * N2 <= 8 * 32;
   auto kern = prefetch ? pair_plane_kernel<8> : pair_plane_kernel<0>;
   RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
 

@@ -189,26 +189,32 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
         const double sc = sr * (p.cs ? p.cs[c] : 1.0);
         double vr = sc * cre[i][j][e], vi = sc * cim[i][j][e];
         if (diag_tile && r == c) vi = 0.0;
+        // Hermitian mode: the lower triangle (c <= r) is the truth, the upper one its exact conjugate mirror
+        // (w_k is fused into the A side only, so (r,c) and (c,r) computed separately would differ in the last bit).
+        if (p.herm && c > r) continue;
         cplx* dst = C + (long long)r * p.ldc + c;
         if (p.atomic) {
+          // split-K: partial sums meet in global memory; herm_mirror_kernel fills the upper triangle afterwards
           atomicAdd(&dst->x, vr); atomicAdd(&dst->y, vi);
-        } else if (p.accumulate) {
-          cplx o = *dst; o.x += vr; o.y += vi; *dst = o;
-        } else {
-          *dst = make_double2(vr, vi);
+          continue;
         }
-        if (p.herm && !diag_tile) {
-          cplx* dm = C + (long long)c * p.ldc + r;
-          if (p.atomic) {
-            atomicAdd(&dm->x, vr); atomicAdd(&dm->y, -vi);
-          } else if (p.accumulate) {
-            cplx o = *dm; o.x += vr; o.y -= vi; *dm = o;
-          } else {
-            *dm = make_double2(vr, -vi);
-          }
+        if (p.accumulate) {
+          cplx o = *dst; o.x += vr; o.y += vi; vr = o.x; vi = o.y;
         }
+        *dst = make_double2(vr, vi);
+        if (p.herm && c < r) C[(long long)c * p.ldc + r] = make_double2(vr, -vi);
       }
     }
+  }
+}
+
+// C[c][r] = conj(C[r][c]) for c > r (after a split-K Hermitian accumulation)
+__global__ void herm_mirror_kernel(cplx* C, long long ldc, long long strideC, int n) {
+  cplx* c = C + blockIdx.z * strideC;
+  const int col = blockIdx.x * blockDim.x + threadIdx.x, row = blockIdx.y;   // row < col: upper element
+  if (col < n && col > row) {
+    cplx v = c[(long long)col * ldc + row];
+    c[(long long)row * ldc + col] = make_double2(v.x, -v.y);
   }
 }
 
@@ -248,13 +254,20 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
   ka.n_kt = n_kt;
   int split = p.split_k;
   if (split <= 0) {
-    const long long want = 2LL * ctx->sm_count;  // two resident CTAs per SM
+    // pick the split that fills whole waves of (2 CTAs per SM): maximise CTAs / (waves * slots)
+    const long long slots = 2LL * ctx->sm_count;
+    const long long base = tiles * p.batch;
     split = 1;
-    if (tiles * p.batch < want && n_kt >= 16) {
-      split = (int)((want + tiles * p.batch - 1) / (tiles * p.batch));
-      int max_split = n_kt / 8;  // at least 8 k-tiles (128 k) per split
-      if (split > max_split) split = max_split;
-      if (split < 1) split = 1;
+    const int max_split = n_kt / 8;  // at least 8 k-tiles (128 k) per split
+    if (max_split > 1 && base < 8 * slots) {
+      double best = 0.0;
+      for (int s = 1; s <= max_split && s <= 64; s++) {
+        const long long ctas = base * s;
+        const long long waves = (ctas + slots - 1) / slots;
+        double eff = (double)ctas / (double)(waves * slots);
+        eff -= 0.002 * s;  // mild preference for fewer splits (less atomic traffic)
+        if (eff > best + 1e-9) { best = eff; split = s; }
+      }
     }
   }
   if (n_kt == 0) split = 1;
@@ -273,10 +286,18 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
   if (tiles > 2147483647LL || p.batch > 65535 || split > 65535)
     return rpa_fail(ctx, RPA_ERR_INVALID, "zgemm_dmma: grid too large");
   dim3 grid((unsigned)tiles, (unsigned)split, (unsigned)p.batch);
-  if (p.a_km && p.b_kn) return launch<true, true>(ctx, ka, grid);
-  if (p.a_km && !p.b_kn) return launch<true, false>(ctx, ka, grid);
-  if (!p.a_km && p.b_kn) return launch<false, true>(ctx, ka, grid);
-  return launch<false, false>(ctx, ka, grid);
+  int rc;
+  if (p.a_km && p.b_kn) rc = launch<true, true>(ctx, ka, grid);
+  else if (p.a_km && !p.b_kn) rc = launch<true, false>(ctx, ka, grid);
+  else if (!p.a_km && p.b_kn) rc = launch<false, true>(ctx, ka, grid);
+  else rc = launch<false, false>(ctx, ka, grid);
+  if (rc) return rc;
+  if (ka.atomic && p.herm) {
+    dim3 mg((p.N + 255) / 256, p.N, p.batch);
+    herm_mirror_kernel<<<mg, 256, 0, ctx->stream>>>(p.C, p.ldc, p.strideC, p.N);
+    RPA_LAUNCH_CHECK(ctx);
+  }
+  return RPA_OK;
 }
 
 // ---------------------------------------------------------------------------------------------
