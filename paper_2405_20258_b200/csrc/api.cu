@@ -2,6 +2,7 @@
 // (PAPER.md:139-158).  All arithmetic of the hot path runs in the CUDA kernels of the other translation units.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 
 #include "rpa_internal.h"
 
@@ -113,6 +114,7 @@ int rpa_create(rpa_ctx** out, const double cell[9], const int fft[3], int n_g, c
   memcpy(ctx->cell, cell, sizeof(ctx->cell));
   for (int a = 0; a < 3; a++) ctx->fft[a] = fft[a];
   ctx->n_g = n_g; ctx->n_pw = n_pw;
+  { const char* e = getenv("RPA_GENERIC_FFT"); ctx->force_generic_fft = e && e[0] == '1'; }
   auto fail = [&](int rc) { g_null_err = ctx->err; rpa_destroy(ctx); return rc; };
   if ((e = cudaSetDevice(device)) != cudaSuccess) return fail(rpa_fail(ctx, RPA_ERR_CUDA, "cudaSetDevice: %s", cudaGetErrorString(e)));
   cudaDeviceProp prop;

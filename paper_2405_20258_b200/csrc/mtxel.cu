@@ -13,6 +13,7 @@
 #include <cmath>
 
 #include "fft_smem.cuh"
+#include "pair_plane_fft8.cuh"
 #include "rpa_internal.h"
 
 using fftsm::Plan;
@@ -25,6 +26,7 @@ struct AxisPlan {
   int* d_perm = nullptr;
   int nk = 0;            // number of distinct epsilon-sphere Miller indices on this axis
   int* d_kpos = nullptr; // [nk] position (after the in-place passes) of each kept frequency
+  int* d_kfreq = nullptr; // [nk] the kept frequencies themselves, in 0..n-1
   Plan fwd() const { Plan p; p.n = n; p.n_pass = n_pass; for (int i = 0; i < n_pass; i++) p.radix[i] = radix[i]; p.tw = d_tw_fwd; p.perm = d_perm; return p; }
   Plan inv() const { Plan p = fwd(); p.tw = d_tw_inv; return p; }
 };
@@ -83,12 +85,14 @@ int mtxel_plan_create(rpa_ctx* ctx, const int32_t* g_eps, const int32_t* g_wfn) 
     kidx[a].erase(std::unique(kidx[a].begin(), kidx[a].end()), kidx[a].end());
     ap.nk = (int)kidx[a].size();
     std::vector<int> kpos(ap.nk);
-    for (int i = 0; i < ap.nk; i++) kpos[i] = perm[((kidx[a][i] % n) + n) % n];
+    std::vector<int> kfreq(ap.nk);
+    for (int i = 0; i < ap.nk; i++) { kfreq[i] = ((kidx[a][i] % n) + n) % n; kpos[i] = perm[kfreq[i]]; }
     int rc;
     if ((rc = upload(ctx, (void**)&ap.d_tw_fwd, twf.data(), n * sizeof(cplx)))) return rc;
     if ((rc = upload(ctx, (void**)&ap.d_tw_inv, twi.data(), n * sizeof(cplx)))) return rc;
     if ((rc = upload(ctx, (void**)&ap.d_perm, perm.data(), n * sizeof(int)))) return rc;
     if ((rc = upload(ctx, (void**)&ap.d_kpos, kpos.data(), ap.nk * sizeof(int)))) return rc;
+    if ((rc = upload(ctx, (void**)&ap.d_kfreq, kfreq.data(), ap.nk * sizeof(int)))) return rc;
   }
   std::vector<int> box(ctx->n_pw);
   for (int g = 0; g < ctx->n_pw; g++) {
@@ -120,7 +124,7 @@ void mtxel_plan_destroy(rpa_ctx* ctx) {
   MtxelPlan* mp = ctx->mtxel;
   if (!mp) return;
   for (int a = 0; a < 3; a++) {
-    cudaFree(mp->ax[a].d_tw_fwd); cudaFree(mp->ax[a].d_tw_inv); cudaFree(mp->ax[a].d_perm); cudaFree(mp->ax[a].d_kpos);
+    cudaFree(mp->ax[a].d_tw_fwd); cudaFree(mp->ax[a].d_tw_inv); cudaFree(mp->ax[a].d_perm); cudaFree(mp->ax[a].d_kpos); cudaFree(mp->ax[a].d_kfreq);
   }
   cudaFree(mp->d_wfn_box); cudaFree(mp->d_inv_map);
   delete mp;
@@ -361,6 +365,35 @@ int wfn_to_realspace(rpa_ctx* ctx, const cplx* psi, int nb, cplx* u) {
   return RPA_OK;
 }
 
+template <int N>
+int launch_fft8(rpa_ctx* ctx, const cplx* u_v, const cplx* u_c, int nvb, int ncc, int N3, const MtxelPlan* mp, cplx* T) {
+  const int nk1 = mp->ax[0].nk, nk2 = mp->ax[1].nk;
+  const size_t smem = fft8::smem_bytes<N>(nk1, nk2);
+  auto kern = fft8::pair_plane_fft8_kernel<N>;
+  static bool attr = false;
+  if (!attr) { RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024)); attr = true; }
+  kern<<<(unsigned)(ncc * N3), fft8::Geo<N>::NWARP * 32, smem, ctx->stream>>>(u_v, u_c, nvb, ncc, N3, mp->ax[0].d_tw_fwd,
+                                                                             mp->ax[0].d_kfreq, mp->ax[1].d_kfreq, nk1, nk2, T);
+  RPA_LAUNCH_CHECK(ctx);
+  return RPA_OK;
+}
+
+// 0 = no specialised kernel for this plane size (or it does not fit): use the generic pair_plane_kernel
+int fft8_plane_size(const rpa_ctx* ctx) {
+  const int N1 = ctx->fft[0], N2 = ctx->fft[1];
+  if (N1 != N2) return 0;
+  const int nk1 = ctx->mtxel->ax[0].nk, nk2 = ctx->mtxel->ax[1].nk;
+  size_t smem = 0;
+  switch (N1) {
+    case 24: smem = fft8::smem_bytes<24>(nk1, nk2); break;
+    case 40: smem = fft8::smem_bytes<40>(nk1, nk2); break;
+    case 48: smem = fft8::smem_bytes<48>(nk1, nk2); break;
+    case 64: smem = fft8::smem_bytes<64>(nk1, nk2); break;
+    default: return 0;
+  }
+  return smem <= 227 * 1024 ? N1 : 0;
+}
+
 }  // namespace
 
 size_t mtxel_workspace_bytes(const rpa_ctx* ctx, int nvb, int nc) {
@@ -381,7 +414,8 @@ int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx*
 
   const int plane = N1 * N2, P1 = N1 | 1, P2 = N2 | 1;
   const size_t smem = ((size_t)2 * N1 * P2 + (size_t)2 * nk2 * P1) * sizeof(cplx) + (size_t)(nk1 + nk2) * sizeof(int);
-  if (smem > 227 * 1024)
+  const int n8 = ctx->force_generic_fft ? 0 : fft8_plane_size(ctx);
+  if (n8 == 0 && smem > 227 * 1024)
     return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_mtxel: an xy plane of %d x %d does not fit in shared memory", N1, N2);
   // warps: about 32 lanes' worth of butterflies per warp in a radix-8 pass over its rows
   int nwarp = (plane / 8 + 31) / 32;
@@ -398,10 +432,19 @@ int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx*
   for (int c0 = 0; c0 < nc; c0 += sz.ncc) {
     const int ncc = std::min(sz.ncc, nc - c0);
     if ((rc = wfn_to_realspace(ctx, psi_c + (long long)c0 * ctx->n_pw, ncc, u_c))) return rc;
-    kern<<<(unsigned)(ncc * N3), nthr, smem, ctx->stream>>>(u_v, u_c, nvb, ncc, N1, N2, N3, mp->ax[0].fwd(),
-                                                            mp->ax[1].fwd(), mp->ax[0].d_kpos, mp->ax[1].d_kpos, nk1,
-                                                            nk2, T);
-    RPA_LAUNCH_CHECK(ctx);
+    switch (n8) {
+      case 24: rc = launch_fft8<24>(ctx, u_v, u_c, nvb, ncc, N3, mp, T); break;
+      case 40: rc = launch_fft8<40>(ctx, u_v, u_c, nvb, ncc, N3, mp, T); break;
+      case 48: rc = launch_fft8<48>(ctx, u_v, u_c, nvb, ncc, N3, mp, T); break;
+      case 64: rc = launch_fft8<64>(ctx, u_v, u_c, nvb, ncc, N3, mp, T); break;
+      default:
+        kern<<<(unsigned)(ncc * N3), nthr, smem, ctx->stream>>>(u_v, u_c, nvb, ncc, N1, N2, N3, mp->ax[0].fwd(),
+                                                                mp->ax[1].fwd(), mp->ax[0].d_kpos, mp->ax[1].d_kpos, nk1,
+                                                                nk2, T);
+        RPA_LAUNCH_CHECK(ctx);
+        rc = RPA_OK;
+    }
+    if (rc) return rc;
     ZScatter zs;
     zs.kpos3 = mp->ax[2].d_kpos; zs.nk3 = nk3; zs.inv_map = mp->d_inv_map; zs.M = M;
     zs.ncc = ncc; zs.nc = nc; zs.c0 = c0; zs.n_g = ctx->n_g; zs.scale = 1.0 / (double)n_r;

@@ -17,6 +17,7 @@ struct rpa_ctx {
   cudaStream_t stream = nullptr;
   std::string err;
   long long launches = 0;
+  bool force_generic_fft = false;  // RPA_GENERIC_FFT=1: use the generic MTXEL plane kernel (tests)
   int sm_count = 148;
 
   // problem statement

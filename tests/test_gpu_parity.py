@@ -69,12 +69,15 @@ def test_tiny_config_valence_blocks_and_full_subspace():
 
 @pytest.mark.parametrize("fft,cell", [((24, 40, 48), (7.0, 9.0, 11.0)), ((64, 15, 20), (11.0, 5.0, 6.0)),
                                       ((12, 18, 120), (5.0, 6.0, 30.0)), ((10, 16, 160), (5.0, 6.0, 40.0)),
-                                      ((30, 27, 25), (8.0, 8.0, 8.0))])
+                                      ((30, 27, 25), (8.0, 8.0, 8.0)), ((48, 48, 12), (12.0, 12.0, 3.0)),
+                                      ((64, 64, 12), (14.0, 14.0, 3.0)), ((40, 40, 10), (9.0, 9.0, 3.0)),
+                                      ((24, 24, 160), (6.0, 6.0, 40.0))])
 def test_mtxel_every_axis_length_and_radix(fft, cell):
     """FFT parity for every axis length of the configs (24, 40, 48, 120, 64, 160) and odd radix-3/5 composites."""
     import paper_2405_20258_b200 as rpa
     import torch
-    inp = make_inputs(cfg_small_grid(fft, cell, 1.4, 0.8))
+    square = fft[0] == fft[1]          # square planes take the specialised radix-8 x R2 kernel: use bigger spheres
+    inp = make_inputs(cfg_small_grid(fft, cell, 3.0 if square else 1.4, 1.5 if square else 0.8))
     ctx = make_ctx(inp, 3, 9, 4, 6)
     try:
         M = torch.empty((3, 9, inp.n_g), dtype=torch.complex128, device="cuda")
@@ -86,6 +89,23 @@ def test_mtxel_every_axis_length_and_radix(fft, cell):
     assert maxnorm_rel(got, ref) <= 1e-12
     g0 = int(np.where((inp.g_eps == 0).all(axis=1))[0][0])
     assert np.abs(got[:, :, g0]).max() < 1e-14                 # P4: <v|c> = 0
+
+
+def test_generic_plane_kernel_on_square_grid(monkeypatch):
+    """RPA_GENERIC_FFT=1 forces the generic (any 2/3/5-smooth size) plane kernel on a grid that normally takes the
+    specialised one; both must agree with the oracle."""
+    import paper_2405_20258_b200 as rpa
+    import torch
+    monkeypatch.setenv("RPA_GENERIC_FFT", "1")
+    inp = make_inputs(0, n_v=3, n_c=11)
+    ctx = make_ctx(inp, 3, 11, 4, 6)
+    try:
+        M = torch.empty((3, 11, inp.n_g), dtype=torch.complex128, device="cuda")
+        rpa.rpa_mtxel(ctx, dev(inp.psi_v), dev(inp.psi_c), M)
+        got = M.cpu().numpy()
+    finally:
+        rpa.rpa_destroy(ctx)
+    assert maxnorm_rel(got, orc.mtxel(inp.psi_v, inp.psi_c, inp.g_wfn, inp.g_eps, inp.fft)) <= 1e-12
 
 
 def test_small_config_twin_all_stages():
