@@ -7,9 +7,14 @@
 // Vcol[i][:] the i-th column of V.  Because G is Hermitian, Acol starts as conj(G).
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <numeric>
 
+#include <cooperative_groups.h>
+
 #include "rpa_internal.h"
+
+namespace cg = cooperative_groups;
 
 namespace {
 
@@ -39,12 +44,12 @@ __device__ __forceinline__ void block_sum(double (&v)[NV], double* sh /* [NV][32
 
 // Acol = -conj(src) (src row-major n x n with leading dimension ld), Vcol = identity
 __global__ void jacobi_init_kernel(const cplx* __restrict__ src, long long ld, int n, cplx* __restrict__ A,
-                                   cplx* __restrict__ V, int negate_conj) {
+                                   cplx* __restrict__ V, int negate_conj, int with_v) {
   const int i = blockIdx.x;
   for (int k = threadIdx.x; k < n; k += blockDim.x) {
     cplx x = src[(long long)i * ld + k];
     A[(long long)i * n + k] = negate_conj ? make_double2(-x.x, x.y) : make_double2(-x.x, -x.y);
-    V[(long long)i * n + k] = make_double2(i == k ? 1.0 : 0.0, 0.0);
+    if (with_v) V[(long long)i * n + k] = make_double2(i == k ? 1.0 : 0.0, 0.0);
   }
 }
 
@@ -57,12 +62,14 @@ __global__ void row_norm2_max_kernel(const cplx* __restrict__ A, int n, double* 
   if (threadIdx.x == 0) atomicMax((unsigned long long*)out, (unsigned long long)__double_as_longlong(v[0]));
 }
 
-// one round of the round-robin ordering: CTA k rotates the pair (i,j) of columns
-__global__ void __launch_bounds__(256) jacobi_round_kernel(cplx* __restrict__ A, cplx* __restrict__ V, int n, int m_even,
-                                                          int round, double rot_tol, const double* __restrict__ gmax,
-                                                          double* __restrict__ off_max) {
-  __shared__ double sh[4 * 32];
-  const int k = blockIdx.x;
+// one round of the round-robin ordering: CTA k rotates the pair (i,j) of columns.
+// WITH_V: also rotate the accumulated V (needed only when eigenvectors of numerically null eigenvalues are wanted;
+// otherwise the eigenvectors are the normalised columns of the converged A = G V, and V is never touched, which halves
+// the traffic).  STASH: the two columns are kept in shared memory between the dot products and the update.
+template <bool WITH_V, bool STASH>
+__device__ __forceinline__ void rotate_pair(cplx* __restrict__ A, cplx* __restrict__ V, int n, int m_even, int round, int k,
+                                            double rot_tol, const double* __restrict__ gmax, double* __restrict__ off_max,
+                                            cplx* st, double* sh) {
   int i, j;
   if (k == 0) { i = m_even - 1; j = round; }
   else { i = (round + k) % (m_even - 1); j = (round - k + (m_even - 1)) % (m_even - 1); }
@@ -73,6 +80,7 @@ __global__ void __launch_bounds__(256) jacobi_round_kernel(cplx* __restrict__ A,
   double v[4] = {0, 0, 0, 0};
   for (int t = threadIdx.x; t < n; t += blockDim.x) {
     cplx x = ai[t], y = aj[t];
+    if (STASH) { st[t] = x; st[n + t] = y; }
     v[0] += x.x * x.x + x.y * x.y;
     v[1] += y.x * y.x + y.y * y.y;
     v[2] += x.x * y.x + x.y * y.y;   // Re conj(x) y
@@ -95,10 +103,12 @@ __global__ void __launch_bounds__(256) jacobi_round_kernel(cplx* __restrict__ A,
   // a_i' = c a_i - s e^{-i phi} a_j ;  a_j' = s e^{i phi} a_i + c a_j
   cplx* vi = V + (long long)i * n;
   cplx* vj = V + (long long)j * n;
-  for (int tt = threadIdx.x; tt < 2 * n; tt += blockDim.x) {
+  const int total = WITH_V ? 2 * n : n;
+  for (int tt = threadIdx.x; tt < total; tt += blockDim.x) {
     cplx* pi_ = tt < n ? ai + tt : vi + (tt - n);
     cplx* pj_ = tt < n ? aj + tt : vj + (tt - n);
-    cplx x = *pi_, y = *pj_;
+    cplx x, y;
+    if (STASH && tt < n) { x = st[tt]; y = st[n + tt]; } else { x = *pi_; y = *pj_; }
     cplx ey = make_double2(pr * y.x + pi * y.y, pr * y.y - pi * y.x);   // e^{-i phi} y
     cplx ex = make_double2(pr * x.x - pi * x.y, pr * x.y + pi * x.x);   // e^{+i phi} x
     *pi_ = make_double2(c * x.x - s * ey.x, c * x.y - s * ey.y);
@@ -106,15 +116,70 @@ __global__ void __launch_bounds__(256) jacobi_round_kernel(cplx* __restrict__ A,
   }
 }
 
-// theta_i = Re v_i^H a_i (eigenvalue of G); lambda = -theta
-__global__ void rayleigh_kernel(const cplx* __restrict__ A, const cplx* __restrict__ V, int n, double* lam) {
-  __shared__ double sh[32];
-  double v[1] = {0.0};
+template <bool WITH_V, bool STASH>
+__global__ void __launch_bounds__(256) jacobi_round_kernel(cplx* __restrict__ A, cplx* __restrict__ V, int n, int m_even,
+                                                          int round, double rot_tol, const double* __restrict__ gmax,
+                                                          double* __restrict__ off_max) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ double sh[4 * 32];
+  rotate_pair<WITH_V, STASH>(A, V, n, m_even, round, blockIdx.x, rot_tol, gmax, off_max, reinterpret_cast<cplx*>(smem_raw), sh);
+}
+
+// All sweeps in ONE cooperative launch: every round is followed by a grid-wide barrier instead of a kernel boundary,
+// and convergence is decided on the device (off[sweep] = largest |a_i^H a_j| / (|a_i||a_j|) seen in that sweep).
+// info[0] = sweeps done, info[1] = converged.
+template <bool WITH_V, bool STASH>
+__global__ void __launch_bounds__(256) jacobi_persistent_kernel(cplx* __restrict__ A, cplx* __restrict__ V, int n, int m_even,
+                                                               double rot_tol, double stop, int max_sweeps,
+                                                               const double* __restrict__ gmax, double* __restrict__ off,
+                                                               int* __restrict__ info) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ double sh[4 * 32];
+  cg::grid_group grid = cg::this_grid();
+  const int npairs = m_even / 2;
+  int sweep = 0;
+  bool conv = false;
+  for (; sweep < max_sweeps && !conv; sweep++) {
+    for (int r = 0; r < m_even - 1; r++) {
+      for (int k = blockIdx.x; k < npairs; k += gridDim.x) {
+        rotate_pair<WITH_V, STASH>(A, V, n, m_even, r, k, rot_tol, gmax, off + sweep, reinterpret_cast<cplx*>(smem_raw), sh);
+        __syncthreads();
+      }
+      grid.sync();
+    }
+    conv = ((volatile double*)off)[sweep] <= stop;
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) { info[0] = sweep; info[1] = conv ? 1 : 0; }
+}
+
+// WITH_V: theta_i = Re v_i^H a_i (eigenvalue of G, keeps the sign of tiny ones); otherwise theta_i = ||a_i|| (G >= 0).
+// lam = -theta;  scale[i] = 1/||a_i|| (0 for a null column)
+__global__ void rayleigh_kernel(const cplx* __restrict__ A, const cplx* __restrict__ V, int n, int with_v, double* lam,
+                                double* scale) {
+  __shared__ double sh[2 * 32];
+  double v[2] = {0.0, 0.0};
   const cplx* a = A + (long long)blockIdx.x * n;
   const cplx* w = V + (long long)blockIdx.x * n;
-  for (int k = threadIdx.x; k < n; k += blockDim.x) v[0] += w[k].x * a[k].x + w[k].y * a[k].y;
-  block_sum<1>(v, sh);
-  if (threadIdx.x == 0) lam[blockIdx.x] = -v[0];
+  for (int k = threadIdx.x; k < n; k += blockDim.x) {
+    v[0] += a[k].x * a[k].x + a[k].y * a[k].y;
+    if (with_v) v[1] += w[k].x * a[k].x + w[k].y * a[k].y;
+  }
+  block_sum<2>(v, sh);
+  if (threadIdx.x == 0) {
+    const double nrm = sqrt(v[0]);
+    lam[blockIdx.x] = with_v ? -v[1] : -nrm;
+    scale[blockIdx.x] = nrm > 0.0 ? 1.0 / nrm : 0.0;
+  }
+}
+
+// dst[r][:] = scale[order[r]] * src[order[r]][:]   (scale == nullptr: plain gather)
+__global__ void gather_scaled_rows_kernel(const cplx* __restrict__ src, long long lds, const int* __restrict__ order,
+                                          const double* __restrict__ scale, int ncols, cplx* __restrict__ dst, long long ldd) {
+  const int o = order[blockIdx.x];
+  const cplx* s = src + (long long)o * lds;
+  const double f = scale ? scale[o] : 1.0;
+  cplx* d = dst + (long long)blockIdx.x * ldd;
+  for (int k = threadIdx.x; k < ncols; k += blockDim.x) d[k] = make_double2(s[k].x * f, s[k].y * f);
 }
 
 __global__ void gather_rows_kernel(const cplx* __restrict__ src, long long lds, const int* __restrict__ order, int ncols,
@@ -151,44 +216,110 @@ __global__ void residual_kernel(const cplx* __restrict__ X, const cplx* __restri
 }
 
 struct JacobiWs {
-  cplx* A; cplx* V; double* lam; int* order; double* scal;  // scal[0] = gmax, scal[1] = off_max
+  cplx* A; cplx* V; double* lam; double* scale; int* order; double* scal;  // scal[0] = gmax, scal[1] = off_max
+  double* off; int* info;   // [64] per-sweep off-norm, [2] sweeps / converged (persistent kernel)
+  bool with_v = false;
 };
 
-// Eigen-decomposition of G = -H (H given as src, Hermitian n x n).  On return lam_sorted (device, ascending = most
-// negative H eigenvalue first) and order (device) index the rows of jw.V (eigenvectors as rows).
-int jacobi_eigh(rpa_ctx* ctx, const cplx* src, long long ld, int n, bool src_is_hc, JacobiWs& jw, std::vector<int>& order_h,
-                std::vector<double>& lam_h) {
-  // src_is_hc: src already holds Hc = H^T (RR matrix), so Acol = -src; otherwise src = H and Acol = -conj(H)
-  jacobi_init_kernel<<<n, 256, 0, ctx->stream>>>(src, ld, n, jw.A, jw.V, src_is_hc ? 0 : 1);
-  RPA_LAUNCH_CHECK(ctx);
-  RPA_CUDA(ctx, cudaMemsetAsync(jw.scal, 0, 2 * sizeof(double), ctx->stream));
-  row_norm2_max_kernel<<<n, 256, 0, ctx->stream>>>(jw.A, n, jw.scal);
-  RPA_LAUNCH_CHECK(ctx);
-  const int m_even = (n + 1) & ~1;
-  const double stop = std::max(1e-14, 4.0 * std::sqrt((double)n) * 1.1e-16);
-  bool converged = n < 2;
-  for (int sweep = 0; sweep < 60 && !converged; sweep++) {
-    RPA_CUDA(ctx, cudaMemsetAsync(jw.scal + 1, 0, sizeof(double), ctx->stream));
-    for (int r = 0; r < m_even - 1; r++) {
-      jacobi_round_kernel<<<m_even / 2, 256, 0, ctx->stream>>>(jw.A, jw.V, n, m_even, r, 1e-15, jw.scal, jw.scal + 1);
-      ctx->launches++;
-    }
-    RPA_CUDA(ctx, cudaGetLastError());
-    double off = 0.0;
-    RPA_CUDA(ctx, cudaMemcpyAsync(&off, jw.scal + 1, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
-    RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    converged = off <= stop;
+template <bool WITH_V, bool STASH>
+void launch_round(rpa_ctx* ctx, JacobiWs& jw, int n, int m_even, int r, size_t smem) {
+  jacobi_round_kernel<WITH_V, STASH><<<m_even / 2, 256, smem, ctx->stream>>>(jw.A, jw.V, n, m_even, r, 1e-15, jw.scal,
+                                                                              jw.scal + 1);
+  ctx->launches++;
+}
+
+// Eigen-decomposition of G = -H (H given as src, Hermitian negative semidefinite n x n) by one-sided Jacobi on the
+// columns of G.  On return lam_h / order_h (host) and jw.order (device) sort the eigenvalues of H ascending (most
+// negative first).  The leading n_need eigenvectors are then fetched with jacobi_vectors().  V is accumulated only if
+// some wanted eigenvalue is numerically null (its column of G V cannot be normalised); that case reruns with V.
+int jacobi_eigh(rpa_ctx* ctx, const cplx* src, long long ld, int n, bool src_is_hc, int n_need, bool try_without_v,
+                JacobiWs& jw, std::vector<int>& order_h, std::vector<double>& lam_h) {
+  static bool attr = false;
+  if (!attr) {
+    RPA_CUDA(ctx, cudaFuncSetAttribute(jacobi_round_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    RPA_CUDA(ctx, cudaFuncSetAttribute(jacobi_round_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    attr = true;
   }
-  if (!converged) return rpa_fail(ctx, RPA_ERR_NO_CONVERGENCE, "one-sided Jacobi did not converge in 60 sweeps (n = %d)", n);
-  rayleigh_kernel<<<n, 256, 0, ctx->stream>>>(jw.A, jw.V, n, jw.lam);
+  const bool verbose = getenv("RPA_VERBOSE") != nullptr;
+  for (int attempt = try_without_v ? 0 : 1; attempt < 2; attempt++) {
+    const bool with_v = attempt == 1;
+    jw.with_v = with_v;
+    // src_is_hc: src already holds Hc = H^T (RR matrix), so Acol = -src; otherwise src = H and Acol = -conj(H)
+    jacobi_init_kernel<<<n, 256, 0, ctx->stream>>>(src, ld, n, jw.A, jw.V, src_is_hc ? 0 : 1, with_v ? 1 : 0);
+    RPA_LAUNCH_CHECK(ctx);
+    RPA_CUDA(ctx, cudaMemsetAsync(jw.scal, 0, 2 * sizeof(double), ctx->stream));
+    row_norm2_max_kernel<<<n, 256, 0, ctx->stream>>>(jw.A, n, jw.scal);
+    RPA_LAUNCH_CHECK(ctx);
+    const int m_even = (n + 1) & ~1;
+    const double stop = std::max(1e-14, 4.0 * std::sqrt((double)n) * 1.1e-16);
+    const size_t stash_bytes = (size_t)2 * n * sizeof(cplx);
+    const bool stash = stash_bytes <= 96 * 1024;
+    bool converged = n < 2;
+    int sweep = 0;
+    bool persistent = false;
+    if (!converged && !getenv("RPA_JACOBI_LAUNCHES")) {
+      // one cooperative launch for all sweeps, if the device can co-schedule a useful number of CTAs
+      const void* fn = with_v ? (stash ? (const void*)jacobi_persistent_kernel<true, true> : (const void*)jacobi_persistent_kernel<true, false>)
+                              : (stash ? (const void*)jacobi_persistent_kernel<false, true> : (const void*)jacobi_persistent_kernel<false, false>);
+      const size_t smem = stash ? stash_bytes : 0;
+      int per_sm = 0, coop = 0;
+      cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device);
+      if (stash) cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+      if (coop && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 256, smem) == cudaSuccess && per_sm > 0) {
+        int grid = std::min(m_even / 2, per_sm * ctx->sm_count);
+        RPA_CUDA(ctx, cudaMemsetAsync(jw.off, 0, 64 * sizeof(double), ctx->stream));
+        cplx* A_ = jw.A; cplx* V_ = jw.V; int n_ = n, me = m_even, maxs = 60;
+        double rt = 1e-15, st_ = stop;
+        const double* gm = jw.scal; double* off_ = jw.off; int* info_ = jw.info;
+        void* args[] = {&A_, &V_, &n_, &me, &rt, &st_, &maxs, &gm, &off_, &info_};
+        cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(256), args, smem, ctx->stream);
+        if (e == cudaSuccess) {
+          ctx->launches++;
+          int info_h[2] = {0, 0};
+          RPA_CUDA(ctx, cudaMemcpyAsync(info_h, jw.info, 2 * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+          RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+          sweep = info_h[0]; converged = info_h[1] != 0; persistent = true;
+        } else {
+          (void)cudaGetLastError();   // fall back to one launch per round
+        }
+      }
+    }
+    for (; !persistent && sweep < 60 && !converged; sweep++) {
+      RPA_CUDA(ctx, cudaMemsetAsync(jw.scal + 1, 0, sizeof(double), ctx->stream));
+      for (int r = 0; r < m_even - 1; r++) {
+        if (with_v) { if (stash) launch_round<true, true>(ctx, jw, n, m_even, r, stash_bytes); else launch_round<true, false>(ctx, jw, n, m_even, r, 0); }
+        else { if (stash) launch_round<false, true>(ctx, jw, n, m_even, r, stash_bytes); else launch_round<false, false>(ctx, jw, n, m_even, r, 0); }
+      }
+      RPA_CUDA(ctx, cudaGetLastError());
+      double off = 0.0;
+      RPA_CUDA(ctx, cudaMemcpyAsync(&off, jw.scal + 1, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+      RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+      converged = off <= stop;
+    }
+    if (verbose) fprintf(stderr, "[rpa] jacobi n=%d with_v=%d stash=%d persistent=%d sweeps=%d\n", n, (int)with_v, (int)stash, (int)persistent, sweep);
+    if (!converged) return rpa_fail(ctx, RPA_ERR_NO_CONVERGENCE, "one-sided Jacobi did not converge in 60 sweeps (n = %d)", n);
+    rayleigh_kernel<<<n, 256, 0, ctx->stream>>>(jw.A, jw.V, n, with_v ? 1 : 0, jw.lam, jw.scale);
+    RPA_LAUNCH_CHECK(ctx);
+    lam_h.resize(n);
+    RPA_CUDA(ctx, cudaMemcpyAsync(lam_h.data(), jw.lam, n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    order_h.resize(n);
+    std::iota(order_h.begin(), order_h.end(), 0);
+    std::stable_sort(order_h.begin(), order_h.end(), [&](int a, int b) { return lam_h[a] < lam_h[b]; });
+    RPA_CUDA(ctx, cudaMemcpyAsync(jw.order, order_h.data(), n * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
+    if (with_v) break;
+    // without V the wanted eigenvectors are a_i / ||a_i||: fine unless a wanted eigenvalue is numerically null
+    const double smallest = std::fabs(lam_h[order_h[std::min(n_need, n) - 1]]);
+    if (smallest > 1e-9 * std::fabs(lam_h[order_h[0]])) break;
+  }
+  return RPA_OK;
+}
+
+// dst[r][:] (r < count) = eigenvector of the r-th smallest eigenvalue of H
+int jacobi_vectors(rpa_ctx* ctx, const JacobiWs& jw, int n, int count, cplx* dst, long long ldd) {
+  gather_scaled_rows_kernel<<<count, 256, 0, ctx->stream>>>(jw.with_v ? jw.V : jw.A, n, jw.order,
+                                                           jw.with_v ? nullptr : jw.scale, n, dst, ldd);
   RPA_LAUNCH_CHECK(ctx);
-  lam_h.resize(n);
-  RPA_CUDA(ctx, cudaMemcpyAsync(lam_h.data(), jw.lam, n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
-  RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-  order_h.resize(n);
-  std::iota(order_h.begin(), order_h.end(), 0);
-  std::stable_sort(order_h.begin(), order_h.end(), [&](int a, int b) { return lam_h[a] < lam_h[b]; });
-  RPA_CUDA(ctx, cudaMemcpyAsync(jw.order, order_h.data(), n * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
   return RPA_OK;
 }
 
@@ -202,7 +333,7 @@ bool use_direct(int n, int n_eig) { return 2 * block_size(n, n_eig) > n; }
 
 size_t basis_workspace_bytes(const rpa_ctx* ctx, int n, int n_eig) {
   (void)ctx;
-  const size_t small = ws_round((size_t)n * sizeof(double)) * 3 + ws_round((size_t)n * sizeof(int)) + 4 * 256;
+  const size_t small = ws_round((size_t)n * sizeof(double)) * 4 + ws_round((size_t)n * sizeof(int)) + 8 * 256;
   if (use_direct(n, n_eig)) return 2 * ws_round((size_t)n * n * sizeof(cplx)) + small;
   const size_t p = block_size(n, n_eig);
   return 3 * ws_round(p * n * sizeof(cplx)) + 4 * ws_round(p * p * sizeof(cplx)) + small;
@@ -215,19 +346,21 @@ int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, dou
   std::vector<double> lam_h;
   JacobiWs jw;
   jw.lam = ws.get<double>(n);
+  jw.scale = ws.get<double>(n);
   double* d_lam_sorted = ws.get<double>(n);
   double* d_res = ws.get<double>(n);
   jw.order = ws.get<int>(n);
   jw.scal = ws.get<double>(4);
+  jw.off = ws.get<double>(64);
+  jw.info = ws.get<int>(4);
   int* d_info = ws.get<int>(4);
   int rc;
   if (use_direct(n, n_eig)) {
     jw.A = ws.get<cplx>((size_t)n * n);
     jw.V = ws.get<cplx>((size_t)n * n);
     if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_subspace_basis: workspace too small (need %zu bytes)", ws.off);
-    if ((rc = jacobi_eigh(ctx, chi0, n, n, false, jw, order_h, lam_h))) return rc;
-    gather_rows_kernel<<<n_eig, 256, 0, ctx->stream>>>(jw.V, n, jw.order, n, C, n);
-    RPA_LAUNCH_CHECK(ctx);
+    if ((rc = jacobi_eigh(ctx, chi0, n, n, false, n_eig, n_eig < n, jw, order_h, lam_h))) return rc;
+    if ((rc = jacobi_vectors(ctx, jw, n, n_eig, C, n))) return rc;
     std::vector<double> ls(n_eig);
     for (int i = 0; i < n_eig; i++) ls[i] = lam_h[order_h[i]];
     RPA_CUDA(ctx, cudaMemcpyAsync(lambda, ls.data(), n_eig * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
@@ -290,9 +423,8 @@ int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, dou
     if ((rc = orthonormalise(X))) return rc;     // second pass (CholeskyQR2) before Rayleigh-Ritz
     if ((rc = gemm_apply(X, Y))) return rc;      // Y = chi0 X
     if ((rc = gram(Y, X, S))) return rc;         // Hc[i][j] = x_j^H chi0 x_i
-    if ((rc = jacobi_eigh(ctx, S, p, p, true, jw, order_h, lam_h))) return rc;
-    gather_rows_kernel<<<p, 256, 0, ctx->stream>>>(jw.V, p, jw.order, p, Vs, p);
-    RPA_LAUNCH_CHECK(ctx);
+    if ((rc = jacobi_eigh(ctx, S, p, p, true, p, true, jw, order_h, lam_h))) return rc;
+    if ((rc = jacobi_vectors(ctx, jw, p, p, Vs, p))) return rc;
     if ((rc = rotate(Vs, X, Z))) return rc;      // Ritz vectors
     std::swap(X, Z);
     if ((rc = rotate(Vs, Y, Z))) return rc;      // chi0 applied to the Ritz vectors

@@ -268,3 +268,40 @@ def test_energy_driver_device_and_host_match_stage_calls():
             assert all(v >= 0 for v in r["stage_ms"].values())
     finally:
         rpa.rpa_destroy(ctx)
+
+
+def test_small_config_full_against_golden():
+    """BASELINE configs[1] at FULL size, in the launch configuration bench.py times (rpa_energy_device, one valence
+    block), against oracle values stored by tests/golden/make_golden.py (oracle-only; 6 minutes of CPU): E_c, t_k, the
+    300 eigenvalues, the spectrum of chi_s at the first frequency, and 64 sampled chi0 elements."""
+    import json
+    import os
+    import paper_2405_20258_b200 as rpa
+    import torch
+    g = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "small_seed1.json")))
+    inp = make_inputs(1)
+    assert inp.n_g == g["n_g"] and inp.n_pw == g["n_pw"]
+    nv, nc, n_eig, n_w = 64, 1500, g["n_eig"], len(inp.omega)
+    ctx = rpa.rpa_create(inp.cell, inp.fft, inp.g_eps, inp.vcoul, inp.g_wfn)
+    try:
+        ws = torch.empty(rpa.rpa_energy_workspace_bytes(ctx, nv, nc, nv, n_eig, n_w), dtype=torch.uint8, device="cuda")
+        rpa.rpa_set_workspace(ctx, ws)
+        psi_v, psi_c, e_v, e_c = dev(inp.psi_v), dev(inp.psi_c), dev(inp.e_v), dev(inp.e_c)
+        r = rpa.rpa_energy_device(ctx, psi_v, psi_c, e_v, e_c, nv, n_eig, 0.0, dev(inp.omega), dev(inp.weight))
+        assert abs(r["E_c"] - g["E_c"]) <= TOL_E * abs(g["E_c"])
+        assert eig_rel(r["lam"], np.array(g["lam"])) <= TOL_LAM
+        t_ref = np.array(g["t"])
+        assert np.abs(r["t"] - t_ref).max() <= 1e-10 * np.abs(t_ref).max()
+        # sampled chi0 elements through the stage calls (valence blocks of 16, accumulated)
+        chi0 = torch.zeros((inp.n_g, inp.n_g), dtype=torch.complex128, device="cuda")
+        M = torch.empty((16, nc, inp.n_g), dtype=torch.complex128, device="cuda")
+        for b in range(0, nv, 16):
+            rpa.rpa_mtxel(ctx, psi_v[b:b + 16].contiguous(), psi_c, M)
+            rpa.rpa_chi0_static(ctx, M, e_v[b:b + 16].contiguous(), e_c, b > 0, chi0)
+        chi0 = chi0.cpu().numpy()
+        for i, j, re, im in g["chi0_samples"]:
+            assert abs(chi0[i, j] - complex(re, im)) <= TOL_CHI * g["chi0_maxabs"]
+    finally:
+        rpa.rpa_destroy(ctx)
+    # the method's own approximation at this config (reported, not a parity item): subspace vs full basis
+    assert g["E_c_full"] < g["E_c"] < 0
