@@ -10,8 +10,8 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librpa_b200.so")
 SOURCES = ["api.cu", "zgemm_dmma.cu", "mtxel.cu", "chol.cu", "basis.cu", "energy.cu"]
-HEADERS = [os.path.join(CSRC, "rpa_internal.h"), os.path.join(CSRC, "fft_smem.cuh"),
-           os.path.join(ROOT, "include", "rpa_b200.h")]
+HEADERS = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".h", ".cuh"))) + \
+    [os.path.join(ROOT, "include", "rpa_b200.h")]
 
 
 def _nvcc() -> str:

@@ -11,6 +11,7 @@
 // All transforms are the hand-written shared-memory radix-8/4/2/3/5 FFT of fft_smem.cuh.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 
 #include "fft_smem.cuh"
 #include "pair_plane_fft8.cuh"
@@ -34,7 +35,7 @@ struct AxisPlan {
 struct MtxelPlan {
   AxisPlan ax[3];        // 0: x (N1), 1: y (N2), 2: z (N3)
   int* d_wfn_box = nullptr;  // [n_pw] index of each wavefunction G in the [z][x][y] box
-  int* d_inv_map = nullptr;  // [nk1*nk2*nk3] epsilon-sphere index of pruned-box point ((i1*nk2+i2)*nk3+i3), or -1
+  int* d_inv_map = nullptr;  // [nk2*nk1*nk3] epsilon-sphere index of pruned-box point ((i2*nk1+i1)*nk3+i3), or -1
 };
 
 static bool factorize(int n, AxisPlan& ap) {
@@ -110,7 +111,7 @@ int mtxel_plan_create(rpa_ctx* ctx, const int32_t* g_eps, const int32_t* g_wfn) 
     int i[3];
     for (int a = 0; a < 3; a++)
       i[a] = (int)(std::lower_bound(kidx[a].begin(), kidx[a].end(), g_eps[3 * g + a]) - kidx[a].begin());
-    size_t pb = ((size_t)i[0] * nk2 + i[1]) * nk3 + i[2];
+    size_t pb = ((size_t)i[1] * nk1 + i[0]) * nk3 + i[2];
     if (inv[pb] >= 0) return rpa_fail(ctx, RPA_ERR_INVALID, "g_eps has a duplicate entry at %d", g);
     inv[pb] = g;
   }
@@ -203,7 +204,7 @@ __global__ void fft_axis_kernel(cplx* __restrict__ data, Plan pl, long long n_li
 }
 
 // One CTA per (c, z): the u_c plane stays in shared memory while the CTA loops over the valence bands of the block.
-//   T[((v*ncc + c)*N3 + z)*J + i1*nk2 + i2] = sum_{x,y} conj(u_v) u_c e^{-2 pi i (k1 x/N1 + k2 y/N2)}
+//   T[((v*ncc + c)*N3 + z)*J + i2*nk1 + i1] = sum_{x,y} conj(u_v) u_c e^{-2 pi i (k1 x/N1 + k2 y/N2)}
 // Warp-private rows: warp w owns rows [w*LW, (w+1)*LW) of the plane; it forms the product for them, transforms them
 // along y and copies the nk2 kept y-frequencies into the (double-buffered, transposed) column buffer -- with only
 // __syncwarp() in between.  One __syncthreads() per valence band then separates that from the x transforms, which are
@@ -291,8 +292,8 @@ __global__ void pair_plane_kernel(const cplx* __restrict__ u_v, const cplx* __re
       fftsm::fft_lines<false, true>(cb + j0 * P1, px, ncol, nullptr, P1, 1, lane, 32);
       cplx* dst = T + (((long long)v * ncc + c) * N3 + z) * J;
       for (int idx = lane; idx < ncol * nk1; idx += 32) {
-        int jc = idx % ncol, i1 = idx / ncol;
-        dst[i1 * nk2 + j0 + jc] = cb[(j0 + jc) * P1 + s_k1[i1]];
+        int i1 = idx % nk1, jc = idx / nk1;
+        dst[(j0 + jc) * nk1 + i1] = cb[(j0 + jc) * P1 + s_k1[i1]];
       }
     }
   }
@@ -369,9 +370,18 @@ template <int N>
 int launch_fft8(rpa_ctx* ctx, const cplx* u_v, const cplx* u_c, int nvb, int ncc, int N3, const MtxelPlan* mp, cplx* T) {
   const int nk1 = mp->ax[0].nk, nk2 = mp->ax[1].nk;
   const size_t smem = fft8::smem_bytes<N>(nk1, nk2);
-  auto kern = fft8::pair_plane_fft8_kernel<N>;
+  auto kern = fft8::Geo<N>::MAXREG > 0 ? fft8::pair_plane_fft8_kernel_r<N> : fft8::pair_plane_fft8_kernel_b<N>;
   static bool attr = false;
-  if (!attr) { RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024)); attr = true; }
+  if (!attr) {
+    RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    attr = true;
+    if (getenv("RPA_VERBOSE")) {
+      cudaFuncAttributes fa;
+      cudaFuncGetAttributes(&fa, kern);
+      fprintf(stderr, "[rpa] pair_plane_fft8_kernel<%d>: %d regs, max %d threads/block, launching %d threads, %zu B smem\n", N,
+              fa.numRegs, fa.maxThreadsPerBlock, fft8::Geo<N>::NWARP * 32, smem);
+    }
+  }
   kern<<<(unsigned)(ncc * N3), fft8::Geo<N>::NWARP * 32, smem, ctx->stream>>>(u_v, u_c, nvb, ncc, N3, mp->ax[0].d_tw_fwd,
                                                                              mp->ax[0].d_kfreq, mp->ax[1].d_kfreq, nk1, nk2, T);
   RPA_LAUNCH_CHECK(ctx);

@@ -1,18 +1,25 @@
 // pair_plane_fft8_kernel<N>: the hot kernel of MTXEL for square xy planes with N = 8 * R2 (N = 24, 40, 48, 64: every
-// config of BASELINE.json).  Same role as the generic pair_plane_kernel (see mtxel.cu), but the two 1-D transforms of a
-// plane are a compile-time two-pass decimation-in-frequency FFT held in registers:
+// config of BASELINE.json).  Same role as the generic pair_plane_kernel (see mtxel.cu): for one (conduction band c,
+// plane z) and every valence band v of the block,
 //
-//   pass A (radix 8):   thread (line, j), j < R2, takes x[j + q R2], q < 8, from the line, does an 8-point butterfly and
-//                       multiplies by w_N^{j s}; y_s goes back in place to position s R2 + j.
-//   pass B (pruned):    only the kept frequencies k are formed:  X[k] = sum_q z[s R2 + q] w_R2^{q s2},  s = k mod 8,
-//                       s2 = k / 8 -- the last radix-R2 pass restricted to the epsilon-sphere outputs (eq. 3
-//                       evaluated on the epsilon sphere only).
+//   T[v][c][z][i2][i1] = sum_{x,y} conj(u_v(x,y,z)) u_c(x,y,z) e^{-2 pi i (k1[i1] x + k2[i2] y)/N}
 //
-// Per valence band: [product fused into the loads of pass A on the rows | pass A | pass B -> kept y-frequencies,
-// transposed] __syncthreads [pass A on the kept columns] __syncthreads [pass B -> the nk1 x nk2 kept plane
-// frequencies, written to T].  Rows are private to a warp, so passes A and B of the row transforms are separated by
-// __syncwarp() only; the twiddles w_N^{j s} live in registers for the whole valence loop and the next band's u_v
-// elements are prefetched into registers while the current band is transformed.
+// on the kept (epsilon-sphere) frequencies only -- PAPER.md:52 eq. 3 before the z transform.  Each 1-D transform is a
+// two-pass decimation-in-frequency FFT, N = 8 x R2:
+//
+//   pass A (radix 8):  thread (line, j), j < R2, holds x[j + q R2], q < 8, in registers, does an 8-point butterfly and
+//                      multiplies by w_N^{j s}; y_s goes to shared memory at position s G + j of the line (G = R2 or
+//                      R2 + 1: an odd group pitch keeps pass B bank-conflict free).
+//   pass B (radix R2): task (line, s) loads the R2 values of group s, does an R2-point butterfly in registers and
+//                      stores only the kept frequencies k = s + 8 s2 (the pruning to the epsilon sphere).
+//
+// Rows (y transforms) are private to a warp: product fused into the pass-A loads, passes A and B separated by
+// __syncwarp() only; pass B writes the kept y-frequencies transposed (x contiguous) into a double-buffered column
+// buffer.  Bands are taken VB at a time: the x transforms of the previous VB bands run in the same loop iteration as the
+// rows of the current VB bands (software pipeline), on the other half of the buffer, again warp-private -- so there is
+// ONE block barrier per VB valence bands, and the VB x nk2 kept columns are dealt to the warps in full batches.  The twiddles
+// w_N^{j s} live in registers for the whole valence loop and the next band's u_v elements are prefetched into
+// registers while the current band is transformed.
 #pragma once
 #include "fft_smem.cuh"
 
@@ -20,29 +27,60 @@ namespace fft8 {
 
 using fftsm::cplx;
 
+constexpr int up_mod8(int x, int r) { return x + (((r - x) % 8) + 8) % 8; }   // smallest y >= x with y = r (mod 8)
+
 template <int N>
 struct Geo {
   static constexpr int R2 = N / 8;            // lanes per line in pass A
   static constexpr int RW = 32 / R2;          // lines per warp
   static constexpr int NWARP = (N + RW - 1) / RW;
-  // line pitch (16-byte elements): odd so that lanes on consecutive lines never share a bank group in pass B, and
-  // = R2 (mod 8) where possible so that pass A is conflict free too
-  static constexpr int P = (R2 == 8) ? N + 1 : ((R2 & 1) ? N + R2 : N + 1);
+  // register cap (__maxnreg__) where a whole number of CTAs per SM needs one: 5 CTAs of 96 threads (N = 24), 2 of 224
+  // (N = 40), 1 of 512 (N = 64); 0 = plain __launch_bounds__ (N = 48: 1 CTA of 320 threads, no cap needed)
+  static constexpr int MAXREG = N <= 24 ? 128 : (N <= 40 ? 128 : (N <= 48 ? 0 : 128));
+  // valence bands per loop iteration: one block barrier per VB bands, and the VB x nk2 kept columns of an iteration
+  // fill whole warps of the x transforms (bounded by shared memory: 2 CTAs/SM at N = 40, 1 at N = 48, 64)
+  static constexpr int VB = N <= 24 ? 4 : (N <= 48 ? 3 : 1);
+  static constexpr int G = (R2 & 1) ? R2 : R2 + 1;   // pitch of an s-group in a pass-A output line (odd)
+  static constexpr int LW = 8 * G;                   // length of a pass-A output line
+  // pitches in 16-byte elements.  P = R2 (mod 8) makes (line, j) -> bank group linear in the lane index, so the
+  // 128-bit pass-A accesses are conflict free; an odd pitch makes the transposed stores of pass B conflict free.
+  static constexpr int PS = up_mod8(N, R2);          // u_c plane
+  static constexpr int PW = up_mod8(LW, R2);         // row work lines
+  static constexpr int PC = (R2 & 1) ? up_mod8(LW > N ? LW : N, R2) : ((LW > N ? LW : N) | 1);   // column lines
 };
 
+// natural-order R-point DFT in registers (forward)
+template <int R>
+__device__ __forceinline__ void dft_small(cplx* z) {
+  if (R == 3) fftsm::bfly3<false>(z);
+  else if (R == 5) fftsm::bfly5<false>(z);
+  else if (R == 8) fftsm::bfly8<false>(z);
+  else if (R == 6) {
+    cplx e[3] = {z[0], z[2], z[4]}, o[3] = {z[1], z[3], z[5]};
+    fftsm::bfly3<false>(e);
+    fftsm::bfly3<false>(o);
+    const double h = 0.5, s = 0.86602540378443864676;
+    cplx o1 = make_double2(h * o[1].x + s * o[1].y, h * o[1].y - s * o[1].x);      // w6   = ( 1/2, -sqrt3/2)
+    cplx o2 = make_double2(-h * o[2].x + s * o[2].y, -h * o[2].y - s * o[2].x);    // w6^2 = (-1/2, -sqrt3/2)
+    z[0] = fftsm::cadd(e[0], o[0]); z[3] = fftsm::csub(e[0], o[0]);
+    z[1] = fftsm::cadd(e[1], o1);   z[4] = fftsm::csub(e[1], o1);
+    z[2] = fftsm::cadd(e[2], o2);   z[5] = fftsm::csub(e[2], o2);
+  }
+}
+
 template <int N>
-__global__ void __launch_bounds__(Geo<N>::NWARP * 32)
-pair_plane_fft8_kernel(const cplx* __restrict__ u_v, const cplx* __restrict__ u_c, int nvb, int ncc, int N3,
+__device__ __forceinline__ void pair_plane_fft8_body(const cplx* __restrict__ u_v, const cplx* __restrict__ u_c, int nvb, int ncc, int N3,
                        const cplx* __restrict__ tw /* [N] exp(-2 pi i k/N) */, const int* __restrict__ kfreq1,
                        const int* __restrict__ kfreq2, int nk1, int nk2, cplx* __restrict__ T) {
-  constexpr int R2 = Geo<N>::R2, RW = Geo<N>::RW, P = Geo<N>::P, NTHR = Geo<N>::NWARP * 32;
+  using GE = Geo<N>;
+  constexpr int R2 = GE::R2, RW = GE::RW, NWARP = GE::NWARP, G = GE::G, PS = GE::PS, PW = GE::PW, PC = GE::PC, VB = GE::VB;
+  constexpr int NTHR = NWARP * 32;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  cplx* sc = reinterpret_cast<cplx*>(smem_raw);   // [N][P]  u_c plane
-  cplx* wk = sc + N * P;                          // [N][P]  rows being transformed
-  cplx* cb0 = wk + N * P;                         // 2 x [nk2][P] kept y-frequencies, x contiguous
-  cplx* root = cb0 + 2 * nk2 * P;                 // [R2]  w_R2^t
-  int* s_k1 = reinterpret_cast<int*>(root + R2);  // [nk1] (s | s2 << 8) of the kept x-frequencies
-  int* s_k2 = s_k1 + nk1;                         // [nk2]
+  cplx* sc = reinterpret_cast<cplx*>(smem_raw);   // [N][PS]  u_c plane
+  cplx* wk = sc + N * PS;                         // [N][PW]  pass-A output of the rows (warp-private rows)
+  cplx* cb0 = wk + N * PW;                        // 2 x [VB][nk2][PC] kept y-frequencies, x contiguous
+  unsigned long long* slot2 = reinterpret_cast<unsigned long long*>(cb0 + 2 * VB * nk2 * PC);   // [8]: byte s2 = i2 or 0xff
+  unsigned long long* slot1 = slot2 + 8;                                                   // [8]: byte s2 = i1 or 0xff
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int z = blockIdx.x / ncc, c = blockIdx.x - z * ncc;
   constexpr int plane = N * N;
@@ -50,21 +88,27 @@ pair_plane_fft8_kernel(const cplx* __restrict__ u_v, const cplx* __restrict__ u_
   const cplx* ucp = u_c + (long long)c * n_r + (long long)z * plane;
   for (int idx = tid; idx < plane; idx += NTHR) {
     int x = idx / N, y = idx - x * N;
-    sc[x * P + y] = ucp[idx];
+    sc[x * PS + y] = ucp[idx];
   }
-  for (int i = tid; i < R2; i += NTHR) root[i] = tw[i * 8];
-  for (int i = tid; i < nk1; i += NTHR) { int k = kfreq1[i]; s_k1[i] = (k & 7) | ((k >> 3) << 8); }
-  for (int i = tid; i < nk2; i += NTHR) { int k = kfreq2[i]; s_k2[i] = (k & 7) | ((k >> 3) << 8); }
+  if (tid < 16) {
+    // slot tables: which frequencies k = s + 8 s2 of group s are kept, and where they go
+    const int* kf = tid < 8 ? kfreq2 : kfreq1;
+    const int nk = tid < 8 ? nk2 : nk1, s = tid & 7;
+    unsigned long long m = ~0ull;
+    for (int i = 0; i < nk; i++) {
+      const int k = kf[i];
+      if ((k & 7) == s) { const int sh = 8 * (k >> 3); m = (m & ~(0xffull << sh)) | ((unsigned long long)i << sh); }
+    }
+    (tid < 8 ? slot2 : slot1)[s] = m;
+  }
 
-  // role of this lane in pass A: line slot ls (row r0 + ls, or kept column c0 + ls), position j
+  // role of this lane in pass A: line slot ls (row r0 + ls, or line l0 + ls of the column buffer), position j
   const int ls = lane / R2, j = lane - ls * R2;
   const bool lane_on = lane < RW * R2;
   const int r0 = warp * RW;                       // first row of this warp
   const int row = r0 + ls;
   const bool row_on = lane_on && row < N;
   const int nrow = min(RW, N - r0);               // > 0 for every warp by construction
-  const int col = warp * RW + ls;                 // kept column handled in the x transforms
-  const bool col_on = lane_on && col < nk2;
   cplx twj[8];
 #pragma unroll
   for (int s = 1; s < 8; s++) twj[s] = tw[(j * s) % N];
@@ -75,78 +119,115 @@ pair_plane_fft8_kernel(const cplx* __restrict__ u_v, const cplx* __restrict__ u_
     for (int q = 0; q < 8; q++) nxt[q] = uvp[q * R2];
   }
   __syncthreads();
-  const int J = nk1 * nk2;
-  for (int v = 0; v < nvb; v++) {
-    cplx* cb = cb0 + (v & 1) * nk2 * P;
-    // ---- rows: product + pass A
-    if (row_on) {
-      cplx x[8];
+  const long long J = (long long)nk1 * nk2;
+  const int cbsz = VB * nk2 * PC;                 // one half of the column buffer: VB bands x nk2 lines
+  const int n_it = (nvb + VB - 1) / VB;
+  for (int it = 0; it <= n_it; it++) {
+    // ---------------- rows of bands it VB .. it VB + VB - 1 -> cb[it & 1]
+    if (it < n_it) {
+      const int v0 = it * VB, nb = min(VB, nvb - v0);
+      for (int u = 0; u < nb; u++) {
+        cplx* cb = cb0 + (it & 1) * cbsz + u * nk2 * PC;
+        if (row_on) {
+          cplx x[8];
 #pragma unroll
-      for (int q = 0; q < 8; q++) {
-        cplx a = nxt[q], b = sc[row * P + j + q * R2];
-        x[q] = make_double2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x);   // conj(u_v) u_c
-      }
-      if (v + 1 < nvb) {
-        const cplx* nx = uvp + (long long)(v + 1) * n_r;
+          for (int q = 0; q < 8; q++) {
+            cplx a = nxt[q], b = sc[row * PS + j + q * R2];
+            x[q] = make_double2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x);   // conj(u_v) u_c
+          }
+          if (v0 + u + 1 < nvb) {
+            const cplx* nx = uvp + (long long)(v0 + u + 1) * n_r;
 #pragma unroll
-        for (int q = 0; q < 8; q++) nxt[q] = nx[q * R2];
-      }
-      fftsm::bfly8<false>(x);
-      wk[row * P + j] = x[0];
+            for (int q = 0; q < 8; q++) nxt[q] = nx[q * R2];
+          }
+          fftsm::bfly8<false>(x);
+          cplx* line = wk + row * PW + j;
+          line[0] = x[0];
 #pragma unroll
-      for (int s = 1; s < 8; s++) wk[row * P + s * R2 + j] = fftsm::cmul(x[s], twj[s]);
-    }
-    __syncwarp();
-    // ---- rows: pass B on the kept y-frequencies, transposed into cb[i2][x]
-    for (int idx = lane; idx < RW * nk2; idx += 32) {
-      const int xr = idx % RW, i2 = idx / RW;
-      if (xr < nrow) {
-        const int ss = s_k2[i2], s = ss & 255, s2 = ss >> 8;
-        const cplx* zrow = wk + (r0 + xr) * P + s * R2;
-        cplx acc = zrow[0];
-#pragma unroll
-        for (int q = 1; q < R2; q++) {
-          cplx w = root[(q * s2) % R2], zz = zrow[q];
-          acc.x += zz.x * w.x - zz.y * w.y;
-          acc.y += zz.x * w.y + zz.y * w.x;
+          for (int s = 1; s < 8; s++) line[s * G] = fftsm::cmul(x[s], twj[s]);
         }
-        cb[i2 * P + r0 + xr] = acc;
+        __syncwarp();
+        for (int t = lane; t < nrow * 8; t += 32) {
+          const int l = t >> 3, s = t & 7;
+          const cplx* grp = wk + (r0 + l) * PW + s * G;
+          cplx zz[R2];
+#pragma unroll
+          for (int q = 0; q < R2; q++) zz[q] = grp[q];
+          dft_small<R2>(zz);
+          const unsigned long long sl = slot2[s];
+          cplx* dst = cb + r0 + l;
+#pragma unroll
+          for (int s2 = 0; s2 < R2; s2++) {
+            const int i2 = (int)((sl >> (8 * s2)) & 0xff);
+            if (i2 != 0xff) dst[i2 * PC] = zz[s2];
+          }
+        }
+        __syncwarp();                               // wk rows are reused by the next band of this iteration
+      }
+    }
+    // ---------------- x transforms of the kept columns of the previous iteration's bands <- cb[(it - 1) & 1]
+    // The nbp * nk2 lines of that half are one flat list, dealt to the warps in batches of RW lines.
+    if (it > 0) {
+      const int v0 = (it - 1) * VB, nbp = min(VB, nvb - v0);
+      cplx* cb = cb0 + ((it - 1) & 1) * cbsz;
+      const int nline = nbp * nk2;
+      for (int l0 = (NWARP - 1 - warp) * RW; l0 < nline; l0 += NWARP * RW) {
+        const int nl = min(RW, nline - l0);
+        const bool col_on = lane_on && ls < nl;
+        cplx x[8];
+        cplx* line = cb + (l0 + ls) * PC;
+        if (col_on) {
+#pragma unroll
+          for (int q = 0; q < 8; q++) x[q] = line[j + q * R2];
+          fftsm::bfly8<false>(x);
+        }
+        __syncwarp();                               // pass A is in place with a different layout: read all, then write
+        if (col_on) {
+          line[j] = x[0];
+#pragma unroll
+          for (int s = 1; s < 8; s++) line[s * G + j] = fftsm::cmul(x[s], twj[s]);
+        }
+        __syncwarp();
+        for (int t = lane; t < nl * 8; t += 32) {
+          const int l = l0 + (t >> 3), s = t & 7;
+          const cplx* grp = cb + l * PC + s * G;
+          cplx zz[R2];
+#pragma unroll
+          for (int q = 0; q < R2; q++) zz[q] = grp[q];
+          dft_small<R2>(zz);
+          const unsigned long long sl = slot1[s];
+          const int u = l / nk2, i2 = l - u * nk2;
+          cplx* dst = T + (((long long)(v0 + u) * ncc + c) * N3 + z) * J + (long long)i2 * nk1;
+#pragma unroll
+          for (int s2 = 0; s2 < R2; s2++) {
+            const int i1 = (int)((sl >> (8 * s2)) & 0xff);
+            if (i1 != 0xff) dst[i1] = zz[s2];
+          }
+        }
+        __syncwarp();
       }
     }
     __syncthreads();
-    // ---- kept columns: pass A (in place in cb)
-    if (col_on) {
-      cplx x[8];
-      cplx* line = cb + col * P + j;
-#pragma unroll
-      for (int q = 0; q < 8; q++) x[q] = line[q * R2];
-      fftsm::bfly8<false>(x);
-      line[0] = x[0];
-#pragma unroll
-      for (int s = 1; s < 8; s++) line[s * R2] = fftsm::cmul(x[s], twj[s]);
-    }
-    __syncthreads();
-    // ---- kept columns: pass B on the kept x-frequencies -> T
-    cplx* dst = T + (((long long)v * ncc + c) * N3 + z) * J;
-    for (int idx = tid; idx < J; idx += NTHR) {
-      const int i1 = idx / nk2, i2 = idx - i1 * nk2;
-      const int ss = s_k1[i1], s = ss & 255, s2 = ss >> 8;
-      const cplx* zc = cb + i2 * P + s * R2;
-      cplx acc = zc[0];
-#pragma unroll
-      for (int q = 1; q < R2; q++) {
-        cplx w = root[(q * s2) % R2], zz = zc[q];
-        acc.x += zz.x * w.x - zz.y * w.y;
-        acc.y += zz.x * w.y + zz.y * w.x;
-      }
-      dst[idx] = acc;
-    }
   }
 }
 
+#define RPA_FFT8_ARGS                                                                                              \
+  const cplx *__restrict__ u_v, const cplx *__restrict__ u_c, int nvb, int ncc, int N3, const cplx *__restrict__ tw, \
+      const int *__restrict__ kfreq1, const int *__restrict__ kfreq2, int nk1, int nk2, cplx *__restrict__ T
+template <int N>
+__global__ void __maxnreg__(Geo<N>::MAXREG > 0 ? Geo<N>::MAXREG : 255) pair_plane_fft8_kernel_r(RPA_FFT8_ARGS) {
+  pair_plane_fft8_body<N>(u_v, u_c, nvb, ncc, N3, tw, kfreq1, kfreq2, nk1, nk2, T);
+}
+template <int N>
+__global__ void __launch_bounds__(Geo<N>::NWARP * 32) pair_plane_fft8_kernel_b(RPA_FFT8_ARGS) {
+  pair_plane_fft8_body<N>(u_v, u_c, nvb, ncc, N3, tw, kfreq1, kfreq2, nk1, nk2, T);
+}
+#undef RPA_FFT8_ARGS
+
 template <int N>
 size_t smem_bytes(int nk1, int nk2) {
-  return ((size_t)2 * N * Geo<N>::P + (size_t)2 * nk2 * Geo<N>::P + Geo<N>::R2) * sizeof(cplx) + (size_t)(nk1 + nk2) * sizeof(int);
+  (void)nk1;
+  return ((size_t)N * Geo<N>::PS + (size_t)N * Geo<N>::PW + (size_t)2 * Geo<N>::VB * nk2 * Geo<N>::PC) * sizeof(cplx) + 16 * sizeof(unsigned long long);
 }
 
 }  // namespace fft8
