@@ -156,18 +156,19 @@ __global__ void __launch_bounds__(256) jacobi_persistent_kernel(cplx* __restrict
 // lam = -theta;  scale[i] = 1/||a_i|| (0 for a null column)
 __global__ void rayleigh_kernel(const cplx* __restrict__ A, const cplx* __restrict__ V, int n, int with_v, double* lam,
                                 double* scale) {
-  __shared__ double sh[2 * 32];
-  double v[2] = {0.0, 0.0};
+  __shared__ double sh[3 * 32];
+  double v[3] = {0.0, 0.0, 0.0};
   const cplx* a = A + (long long)blockIdx.x * n;
   const cplx* w = V + (long long)blockIdx.x * n;
   for (int k = threadIdx.x; k < n; k += blockDim.x) {
     v[0] += a[k].x * a[k].x + a[k].y * a[k].y;
-    if (with_v) v[1] += w[k].x * a[k].x + w[k].y * a[k].y;
+    if (with_v) { v[1] += w[k].x * a[k].x + w[k].y * a[k].y; v[2] += w[k].x * w[k].x + w[k].y * w[k].y; }
   }
-  block_sum<2>(v, sh);
+  block_sum<3>(v, sh);
   if (threadIdx.x == 0) {
     const double nrm = sqrt(v[0]);
-    lam[blockIdx.x] = with_v ? -v[1] : -nrm;
+    // a zero row of V is a padding vector of the block iteration, not an eigenvector: it sorts after everything
+    lam[blockIdx.x] = with_v ? (v[2] < 0.5 ? 1.0 : -v[1]) : -nrm;
     scale[blockIdx.x] = nrm > 0.0 ? 1.0 / nrm : 0.0;
   }
 }
@@ -218,6 +219,7 @@ __global__ void residual_kernel(const cplx* __restrict__ X, const cplx* __restri
 struct JacobiWs {
   cplx* A; cplx* V; double* lam; double* scale; int* order; double* scal;  // scal[0] = gmax, scal[1] = off_max
   double* off; int* info;   // [64] per-sweep off-norm, [2] sweeps / converged (persistent kernel)
+  cplx* Wb = nullptr; cplx* Ub = nullptr;   // [n_pad/64][64][64] Gram matrices / rotations of the block iteration
   bool with_v = false;
 };
 
@@ -226,6 +228,140 @@ void launch_round(rpa_ctx* ctx, JacobiWs& jw, int n, int m_even, int r, size_t s
   jacobi_round_kernel<WITH_V, STASH><<<m_even / 2, 256, smem, ctx->stream>>>(jw.A, jw.V, n, m_even, r, 1e-15, jw.scal,
                                                                               jw.scal + 1);
   ctx->launches++;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Block one-sided Jacobi (GEMM-rich form of the Hestenes iteration above): the vectors are taken in blocks of JB = 32;
+// a step pairs adjacent blocks, forms the 64 x 64 Gram matrix W of each pair with the DMMA GEMM, runs one cyclic sweep
+// of two-sided Jacobi rotations on W in shared memory accumulating the unitary U (pair_rotations_kernel), and applies
+// A_pair <- U A_pair with the DMMA GEMM.  Odd-even transposition ordering: even steps pair blocks (0,1),(2,3),...,
+// odd steps (1,2),(3,4),..., and the two blocks of a pair always swap places, so after nblk steps every pair of
+// blocks has met exactly once and pairs are always contiguous in memory.
+constexpr int JB = 32, JP = 2 * JB, JLD = JP + 1;
+
+__global__ void __launch_bounds__(256) pair_rotations_kernel(const cplx* __restrict__ Wg, cplx* __restrict__ Ug, double rot_tol,
+                                                             const double* __restrict__ gmax, double* __restrict__ off_max) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx* W = reinterpret_cast<cplx*>(smem_raw);   // [JP][JLD]
+  cplx* U = W + JP * JLD;                        // [JP][JLD]
+  __shared__ double rc_[JB], rs_[JB], rx_[JB], ry_[JB];
+  __shared__ int rp_[JB], rq_[JB];
+  __shared__ double sh[32];
+  const int tid = threadIdx.x;
+  const cplx* wg = Wg + (long long)blockIdx.x * JP * JP;
+  for (int idx = tid; idx < JP * JP; idx += 256) {
+    const int i = idx / JP, k = idx - i * JP;
+    W[i * JLD + k] = wg[idx];
+    U[i * JLD + k] = make_double2(i == k ? 1.0 : 0.0, 0.0);
+  }
+  __syncthreads();
+  const double null2 = 1e-24 * gmax[0];
+  {  // largest normalised off-diagonal element of this pair's Gram matrix (convergence measure of the sweep)
+    double off = 0.0;
+    for (int idx = tid; idx < JP * JP; idx += 256) {
+      const int i = idx / JP, k = idx - i * JP;
+      if (k < i) {
+        const double a = W[i * JLD + i].x, b = W[k * JLD + k].x;
+        if (a > null2 && b > null2) {   // a numerically null vector has no direction to converge
+          const double den = sqrt(a * b);
+          const cplx w = W[i * JLD + k];
+          if (den > 0.0) off = fmax(off, sqrt(w.x * w.x + w.y * w.y) / den);
+        }
+      }
+    }
+    for (int o = 16; o > 0; o >>= 1) off = fmax(off, __shfl_xor_sync(0xffffffffu, off, o));
+    if ((tid & 31) == 0) sh[tid >> 5] = off;
+    __syncthreads();
+    if (tid == 0) {
+      for (int w = 1; w < 8; w++) off = fmax(off, sh[w]);
+      atomicMax((unsigned long long*)off_max, (unsigned long long)__double_as_longlong(off));
+    }
+  }
+  for (int r = 0; r < JP - 1; r++) {
+    if (tid < JB) {
+      int i, j;
+      if (tid == 0) { i = JP - 1; j = r; }
+      else { i = (r + tid) % (JP - 1); j = (r - tid + (JP - 1)) % (JP - 1); }
+      if (i > j) { int t = i; i = j; j = t; }
+      const double alpha = W[i * JLD + i].x, beta = W[j * JLD + j].x;
+      const cplx w = W[i * JLD + j];
+      const double gabs = sqrt(w.x * w.x + w.y * w.y);
+      double c = 1.0, s = 0.0, ex = 1.0, ey = 0.0;
+      const double den = sqrt(alpha * beta);
+      if (!(alpha <= null2 && beta <= null2) && den > 0.0 && gabs > rot_tol * den) {
+        const double zeta = (beta - alpha) / (2.0 * gabs);
+        const double t = (zeta >= 0.0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
+        c = 1.0 / sqrt(1.0 + t * t); s = c * t;
+        ex = w.x / gabs; ey = w.y / gabs;          // e^{i theta} = W_ij / |W_ij|
+      }
+      rp_[tid] = i; rq_[tid] = j; rc_[tid] = c; rs_[tid] = s; rx_[tid] = ex; ry_[tid] = ey;
+    }
+    __syncthreads();
+    // rows i, j of W and U:  x_i' = c x_i - s e^{i theta} x_j ;  x_j' = s x_i + c e^{i theta} x_j
+    for (int idx = tid; idx < 2 * JB * JP; idx += 256) {
+      const int half = idx / (JB * JP), rem = idx - half * (JB * JP);
+      const int k = rem / JP, col = rem - k * JP;
+      cplx* X = half ? U : W;
+      const int i = rp_[k], j = rq_[k];
+      const double c = rc_[k], s = rs_[k], ex = rx_[k], ey = ry_[k];
+      const cplx xi = X[i * JLD + col], xj = X[j * JLD + col];
+      const cplx ej = make_double2(ex * xj.x - ey * xj.y, ex * xj.y + ey * xj.x);   // e^{i theta} x_j
+      X[i * JLD + col] = make_double2(c * xi.x - s * ej.x, c * xi.y - s * ej.y);
+      X[j * JLD + col] = make_double2(s * xi.x + c * ej.x, s * xi.y + c * ej.y);
+    }
+    __syncthreads();
+    // columns i, j of W:  y_i' = c y_i - s e^{-i theta} y_j ;  y_j' = s y_i + c e^{-i theta} y_j
+    for (int idx = tid; idx < JB * JP; idx += 256) {
+      const int k = idx / JP, row = idx - k * JP;
+      const int i = rp_[k], j = rq_[k];
+      const double c = rc_[k], s = rs_[k], ex = rx_[k], ey = ry_[k];
+      const cplx yi = W[row * JLD + i], yj = W[row * JLD + j];
+      const cplx ej = make_double2(ex * yj.x + ey * yj.y, ex * yj.y - ey * yj.x);   // e^{-i theta} y_j
+      W[row * JLD + i] = make_double2(c * yi.x - s * ej.x, c * yi.y - s * ej.y);
+      W[row * JLD + j] = make_double2(s * yi.x + c * ej.x, s * yi.y + c * ej.y);
+    }
+    __syncthreads();
+  }
+  // U with its two row blocks swapped: the blocks of the pair exchange places (odd-even transposition ordering)
+  cplx* ug = Ug + (long long)blockIdx.x * JP * JP;
+  for (int idx = tid; idx < JP * JP; idx += 256) {
+    const int i = idx / JP, k = idx - i * JP;
+    ug[idx] = U[((i + JB) % JP) * JLD + k];
+  }
+}
+
+int jacobi_block_min() {   // matrices smaller than this use the vector iteration (RPA_JACOBI_BLOCK_MIN overrides)
+  const char* e = getenv("RPA_JACOBI_BLOCK_MIN");
+  return e ? atoi(e) : 1024;
+}
+
+// One sweep (nblk steps) of the block iteration on the n_pad = nblk * JB vectors of length n in A (and V if with_v).
+int block_jacobi_sweep(rpa_ctx* ctx, cplx* A, cplx* V, bool with_v, int n, int nblk, cplx* Wb, cplx* Ub, const double* gmax,
+                       double* off_slot) {
+  const size_t smem = (size_t)2 * JP * JLD * sizeof(cplx);
+  for (int step = 0; step < nblk; step++) {
+    const int b0 = step & 1;
+    const int npairs = (nblk - b0) / 2;
+    if (npairs <= 0) continue;
+    cplx* a0 = A + (long long)b0 * JB * n;
+    ZgemmParams g;   // W[pair] = A_pair A_pair^H
+    g.A = a0; g.lda = n; g.a_km = false; g.B = a0; g.ldb = n; g.b_kn = false; g.C = Wb; g.ldc = JP;
+    g.M = JP; g.N = JP; g.K = n; g.conj_b = true; g.herm = true;
+    g.batch = npairs; g.strideA = (long long)JP * n; g.strideB = g.strideA; g.strideC = JP * JP;
+    int rc = zgemm_dmma(ctx, g);
+    if (rc) return rc;
+    pair_rotations_kernel<<<npairs, 256, smem, ctx->stream>>>(Wb, Ub, 1e-15, gmax, off_slot);
+    RPA_LAUNCH_CHECK(ctx);
+    for (int which = 0; which < (with_v ? 2 : 1); which++) {   // X_pair <- U X_pair, in place (a CTA reads its whole
+      cplx* x0 = (which ? V : A) + (long long)b0 * JB * n;     // 64-row column strip before it writes it)
+      ZgemmParams u;
+      u.A = Ub; u.lda = JP; u.a_km = false; u.B = x0; u.ldb = n; u.b_kn = true; u.C = x0; u.ldc = n;
+      u.M = JP; u.N = n; u.K = JP; u.conj_b = false; u.split_k = 1;
+      u.batch = npairs; u.strideA = JP * JP; u.strideB = (long long)JP * n; u.strideC = u.strideB;
+      if ((rc = zgemm_dmma(ctx, u))) return rc;
+    }
+  }
+  return RPA_OK;
 }
 
 // Eigen-decomposition of G = -H (H given as src, Hermitian negative semidefinite n x n) by one-sided Jacobi on the
@@ -238,6 +374,8 @@ int jacobi_eigh(rpa_ctx* ctx, const cplx* src, long long ld, int n, bool src_is_
   if (!attr) {
     RPA_CUDA(ctx, cudaFuncSetAttribute(jacobi_round_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
     RPA_CUDA(ctx, cudaFuncSetAttribute(jacobi_round_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    RPA_CUDA(ctx, cudaFuncSetAttribute(pair_rotations_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)((size_t)2 * JP * JLD * sizeof(cplx))));
     attr = true;
   }
   const bool verbose = getenv("RPA_VERBOSE") != nullptr;
@@ -252,12 +390,36 @@ int jacobi_eigh(rpa_ctx* ctx, const cplx* src, long long ld, int n, bool src_is_
     RPA_LAUNCH_CHECK(ctx);
     const int m_even = (n + 1) & ~1;
     const double stop = std::max(1e-14, 4.0 * std::sqrt((double)n) * 1.1e-16);
+    const bool block = jw.Wb != nullptr && n >= jacobi_block_min();
+    const int n_rows = block ? (n + JB - 1) / JB * JB : n;   // vectors held in jw.A (the block iteration pads with zeros)
     const size_t stash_bytes = (size_t)2 * n * sizeof(cplx);
     const bool stash = stash_bytes <= 96 * 1024;
     bool converged = n < 2;
     int sweep = 0;
     bool persistent = false;
-    if (!converged && !getenv("RPA_JACOBI_LAUNCHES")) {
+    if (block && !converged) {
+      // GEMM-rich block iteration; padding vectors (rows n .. n_rows) are zero and stay zero
+      if (n_rows > n) {
+        RPA_CUDA(ctx, cudaMemsetAsync(jw.A + (size_t)n * n, 0, (size_t)(n_rows - n) * n * sizeof(cplx), ctx->stream));
+        if (with_v) RPA_CUDA(ctx, cudaMemsetAsync(jw.V + (size_t)n * n, 0, (size_t)(n_rows - n) * n * sizeof(cplx), ctx->stream));
+      }
+      RPA_CUDA(ctx, cudaMemsetAsync(jw.off, 0, 64 * sizeof(double), ctx->stream));
+      double prev = 1e300;
+      for (; sweep < 60 && !converged; sweep++) {
+        int rc = block_jacobi_sweep(ctx, jw.A, jw.V, with_v, n, n_rows / JB, jw.Wb, jw.Ub, jw.scal, jw.off + sweep);
+        if (rc) return rc;
+        double off = 0.0;
+        RPA_CUDA(ctx, cudaMemcpyAsync(&off, jw.off + sweep, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        if (verbose) fprintf(stderr, "[rpa] block jacobi n=%d sweep %d off %.3e\n", n, sweep, off);
+        // off is measured on the Gram matrices BEFORE the sweep's rotations; rounding of the Gram sums floors it near
+        // sqrt(n) eps, so a sweep that no longer improves a tiny off also ends the iteration
+        converged = off <= stop || (off <= 1e-12 && off > 0.5 * prev);
+        prev = off;
+      }
+      persistent = true;   // skip the per-round launch loop below
+    }
+    if (!block && !converged && !getenv("RPA_JACOBI_LAUNCHES")) {
       // one cooperative launch for all sweeps, if the device can co-schedule a useful number of CTAs
       const void* fn = with_v ? (stash ? (const void*)jacobi_persistent_kernel<true, true> : (const void*)jacobi_persistent_kernel<true, false>)
                               : (stash ? (const void*)jacobi_persistent_kernel<false, true> : (const void*)jacobi_persistent_kernel<false, false>);
@@ -298,15 +460,15 @@ int jacobi_eigh(rpa_ctx* ctx, const cplx* src, long long ld, int n, bool src_is_
     }
     if (verbose) fprintf(stderr, "[rpa] jacobi n=%d with_v=%d stash=%d persistent=%d sweeps=%d\n", n, (int)with_v, (int)stash, (int)persistent, sweep);
     if (!converged) return rpa_fail(ctx, RPA_ERR_NO_CONVERGENCE, "one-sided Jacobi did not converge in 60 sweeps (n = %d)", n);
-    rayleigh_kernel<<<n, 256, 0, ctx->stream>>>(jw.A, jw.V, n, with_v ? 1 : 0, jw.lam, jw.scale);
+    rayleigh_kernel<<<n_rows, 256, 0, ctx->stream>>>(jw.A, jw.V, n, with_v ? 1 : 0, jw.lam, jw.scale);
     RPA_LAUNCH_CHECK(ctx);
-    lam_h.resize(n);
-    RPA_CUDA(ctx, cudaMemcpyAsync(lam_h.data(), jw.lam, n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    lam_h.resize(n_rows);
+    RPA_CUDA(ctx, cudaMemcpyAsync(lam_h.data(), jw.lam, n_rows * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    order_h.resize(n);
+    order_h.resize(n_rows);
     std::iota(order_h.begin(), order_h.end(), 0);
     std::stable_sort(order_h.begin(), order_h.end(), [&](int a, int b) { return lam_h[a] < lam_h[b]; });
-    RPA_CUDA(ctx, cudaMemcpyAsync(jw.order, order_h.data(), n * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
+    RPA_CUDA(ctx, cudaMemcpyAsync(jw.order, order_h.data(), n_rows * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
     if (with_v) break;
     // without V the wanted eigenvectors are a_i / ||a_i||: fine unless a wanted eigenvalue is numerically null
     const double smallest = std::fabs(lam_h[order_h[std::min(n_need, n) - 1]]);
@@ -333,10 +495,13 @@ bool use_direct(int n, int n_eig) { return 2 * block_size(n, n_eig) > n; }
 
 size_t basis_workspace_bytes(const rpa_ctx* ctx, int n, int n_eig) {
   (void)ctx;
-  const size_t small = ws_round((size_t)n * sizeof(double)) * 4 + ws_round((size_t)n * sizeof(int)) + 8 * 256;
-  if (use_direct(n, n_eig)) return 2 * ws_round((size_t)n * n * sizeof(cplx)) + small;
+  const size_t small = ws_round((size_t)(n + JB) * sizeof(double)) * 4 + ws_round((size_t)(n + JB) * sizeof(int)) + 8 * 256;
+  auto jac = [](size_t m) {   // A, V (padded to whole blocks) and the Gram / rotation matrices of the block iteration
+    return 2 * ws_round((m + JB) * m * sizeof(cplx)) + 2 * ws_round(((m + JB) / JP + 1) * JP * JP * sizeof(cplx));
+  };
+  if (use_direct(n, n_eig)) return jac(n) + small;
   const size_t p = block_size(n, n_eig);
-  return 3 * ws_round(p * n * sizeof(cplx)) + 4 * ws_round(p * p * sizeof(cplx)) + small;
+  return 3 * ws_round(p * n * sizeof(cplx)) + 2 * ws_round(p * p * sizeof(cplx)) + jac(p) + small;
 }
 
 int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, double tol, cplx* C, double* lambda,
@@ -345,19 +510,21 @@ int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, dou
   std::vector<int> order_h;
   std::vector<double> lam_h;
   JacobiWs jw;
-  jw.lam = ws.get<double>(n);
-  jw.scale = ws.get<double>(n);
+  jw.lam = ws.get<double>(n + JB);
+  jw.scale = ws.get<double>(n + JB);
   double* d_lam_sorted = ws.get<double>(n);
   double* d_res = ws.get<double>(n);
-  jw.order = ws.get<int>(n);
+  jw.order = ws.get<int>(n + JB);
   jw.scal = ws.get<double>(4);
   jw.off = ws.get<double>(64);
   jw.info = ws.get<int>(4);
   int* d_info = ws.get<int>(4);
   int rc;
   if (use_direct(n, n_eig)) {
-    jw.A = ws.get<cplx>((size_t)n * n);
-    jw.V = ws.get<cplx>((size_t)n * n);
+    jw.A = ws.get<cplx>((size_t)(n + JB) * n);
+    jw.V = ws.get<cplx>((size_t)(n + JB) * n);
+    jw.Wb = ws.get<cplx>((size_t)((n + JB) / JP + 1) * JP * JP);
+    jw.Ub = ws.get<cplx>((size_t)((n + JB) / JP + 1) * JP * JP);
     if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_subspace_basis: workspace too small (need %zu bytes)", ws.off);
     if ((rc = jacobi_eigh(ctx, chi0, n, n, false, n_eig, n_eig < n, jw, order_h, lam_h))) return rc;
     if ((rc = jacobi_vectors(ctx, jw, n, n_eig, C, n))) return rc;
@@ -376,8 +543,10 @@ int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, dou
   cplx* Z = ws.get<cplx>((size_t)p * n);
   cplx* S = ws.get<cplx>((size_t)p * p);
   cplx* Vs = ws.get<cplx>((size_t)p * p);
-  jw.A = ws.get<cplx>((size_t)p * p);
-  jw.V = ws.get<cplx>((size_t)p * p);
+  jw.A = ws.get<cplx>((size_t)(p + JB) * p);
+  jw.V = ws.get<cplx>((size_t)(p + JB) * p);
+  jw.Wb = ws.get<cplx>((size_t)((p + JB) / JP + 1) * JP * JP);
+  jw.Ub = ws.get<cplx>((size_t)((p + JB) / JP + 1) * JP * JP);
   if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_subspace_basis: workspace too small (need %zu bytes)", ws.off);
 
   auto gemm_apply = [&](const cplx* Xin, cplx* Yout) {  // Yout[j][G] = sum_G' chi0[G][G'] Xin[j][G']

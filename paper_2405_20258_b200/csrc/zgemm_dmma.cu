@@ -277,9 +277,13 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
   if (n_kt == 0 || (ka.atomic && !p.accumulate)) {
     // zero C first (K == 0 gives C = 0 when not accumulating)
     if (!p.accumulate) {
-      for (int b = 0; b < p.batch; b++)
-        RPA_CUDA(ctx, cudaMemset2DAsync(p.C + b * p.strideC, p.ldc * sizeof(cplx), 0, (size_t)p.N * sizeof(cplx), p.M,
-                                        ctx->stream));
+      if (p.ldc == p.N && (p.batch == 1 || p.strideC == (long long)p.M * p.N)) {   // one contiguous slab
+        RPA_CUDA(ctx, cudaMemsetAsync(p.C, 0, (size_t)p.batch * p.M * p.N * sizeof(cplx), ctx->stream));
+      } else {
+        for (int b = 0; b < p.batch; b++)
+          RPA_CUDA(ctx, cudaMemset2DAsync(p.C + b * p.strideC, p.ldc * sizeof(cplx), 0, (size_t)p.N * sizeof(cplx), p.M,
+                                          ctx->stream));
+      }
     }
     if (n_kt == 0) return RPA_OK;
   }

@@ -172,6 +172,19 @@ def test_chi_subspace_freq_random_basis():
 def test_subspace_basis_direct_and_iterative(n, n_eig):
     """a3 alone on random negative-semidefinite matrices with an n^-2/3-like spectrum: direct Jacobi path
     (2 p > n) and block subspace iteration (small n_eig); eigenvalues, residuals (P13), orthonormality."""
+    check_basis(n, n_eig)
+
+
+@pytest.mark.parametrize("n,n_eig", [(147, 60), (147, 147), (300, 40), (333, 333), (1100, 400)])
+def test_subspace_basis_block_jacobi(n, n_eig, monkeypatch):
+    """The same with the GEMM-rich block Jacobi iteration forced on small matrices (it is the default from
+    n = 1024 up; (1100, 400) takes it by default): ragged last block, zero padding vectors, null eigenvalues."""
+    if n < 1024:
+        monkeypatch.setenv("RPA_JACOBI_BLOCK_MIN", "32")
+    check_basis(n, n_eig)
+
+
+def check_basis(n, n_eig):
     import paper_2405_20258_b200 as rpa
     import torch
     rng = np.random.default_rng(n + n_eig)
@@ -181,7 +194,7 @@ def test_subspace_basis_direct_and_iterative(n, n_eig):
     H = (q * spec[None, :]) @ q.conj().T
     H = 0.5 * (H + H.conj().T)
     # the basis stage only needs n_g = n: build a context whose epsilon sphere has n points
-    cfgn = RpaConfig("b", 1, (30.0, 30.0, 30.0), (40, 40, 40), 0.3, 0.45, 1, 1, (-0.6, 0.0), (0.05, 3.0), 1, 2)
+    cfgn = RpaConfig("b", 1, (30.0, 30.0, 30.0), (40, 40, 40), 0.3, 0.45 if n <= 600 else 1.1, 1, 1, (-0.6, 0.0), (0.05, 3.0), 1, 2)
     base = make_inputs(cfgn)
     assert base.n_g >= n
     base = dataclasses.replace(base, g_eps=base.g_eps[:n], vcoul=base.vcoul[:n])
