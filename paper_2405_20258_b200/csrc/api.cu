@@ -32,31 +32,41 @@ size_t chi_freq_vchunk(const rpa_ctx* ctx, int nvb, int nc, int n_eig) {
   size_t vc = std::max<size_t>(1, budget / std::max<size_t>(per_v, 1));
   return std::min<size_t>(vc, (size_t)nvb);
 }
-size_t chi_freq_workspace(const rpa_ctx* ctx, int nvb, int nc, int n_eig) {
-  return ws_round(chi_freq_vchunk(ctx, nvb, nc, n_eig) * nc * n_eig * sizeof(cplx));
+size_t chi_freq_workspace(const rpa_ctx* ctx, int nvb, int nc, int n_eig, int n_w) {
+  return ws_round(chi_freq_vchunk(ctx, nvb, nc, n_eig) * nc * n_eig * sizeof(cplx)) + ws_round((size_t)n_w * nvb * nc * sizeof(double));
 }
+size_t chi0_static_workspace(int nvb, int nc) { return ws_round((size_t)nvb * nc * sizeof(double)); }
 
-int do_chi0_static(rpa_ctx* ctx, const cplx* M, int nvb, int nc, const double* e_v, const double* e_c, int accumulate,
-                   cplx* chi0) {
+int do_chi0_static(rpa_ctx* ctx, WsAlloc& ws, const cplx* M, int nvb, int nc, const double* e_v, const double* e_c,
+                   int accumulate, cplx* chi0) {
+  double* wk = ws.get<double>((size_t)nvb * nc);
+  if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_chi0_static: workspace too small (need %zu bytes)", ws.off);
+  int rc = pair_weights(ctx, e_v, e_c, nvb, nc, nullptr, 1, wk);   // D_vc(0) = 2/Delta_vc  (eq. 5)
+  if (rc) return rc;
   ZgemmParams g;
   g.A = M; g.lda = ctx->n_g; g.a_km = true; g.B = M; g.ldb = ctx->n_g; g.b_kn = true;
   g.C = chi0; g.ldc = ctx->n_g; g.M = ctx->n_g; g.N = ctx->n_g; g.K = nvb * nc;
   g.conj_b = true; g.herm = true; g.accumulate = accumulate != 0; g.alpha = -1.0;
   g.rs = ctx->d_vsqrt; g.cs = ctx->d_vsqrt;
-  g.wmode = 1; g.e_v = e_v; g.e_c = e_c; g.nc = nc; g.omega = nullptr;
+  g.wk = wk;
   return zgemm_dmma(ctx, g);
 }
 
 int do_chi_freq(rpa_ctx* ctx, WsAlloc& ws, const cplx* M, int nvb, int nc, const double* e_v, const double* e_c, const cplx* C,
                 int n_eig, const double* omega, int n_w, int accumulate, cplx* chi_s) {
   const int n_g = ctx->n_g;
+  const long long Pall = (long long)nvb * nc;
+  double* wk = ws.get<double>((size_t)n_w * Pall);   // D_vc(i omega_k) for the whole block, [k][v * nc + c]
+  if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_chi_subspace_freq: workspace too small (need %zu bytes)", ws.off);
+  int rc = pair_weights(ctx, e_v, e_c, nvb, nc, omega, n_w, wk);
+  if (rc) return rc;
   if (!C) {  // full basis: chi~0(i w_k) directly from M
     ZgemmParams g;
     g.A = M; g.lda = n_g; g.a_km = true; g.B = M; g.ldb = n_g; g.b_kn = true;
     g.C = chi_s; g.ldc = n_g; g.M = n_g; g.N = n_g; g.K = nvb * nc;
     g.conj_b = true; g.herm = true; g.accumulate = accumulate != 0; g.alpha = -1.0;
     g.rs = ctx->d_vsqrt; g.cs = ctx->d_vsqrt;
-    g.wmode = 1; g.e_v = e_v; g.e_c = e_c; g.nc = nc; g.omega = omega;
+    g.wk = wk; g.strideW = Pall;
     g.batch = n_w; g.strideC = (long long)n_g * n_g;
     return zgemm_dmma(ctx, g);
   }
@@ -71,15 +81,15 @@ int do_chi_freq(rpa_ctx* ctx, WsAlloc& ws, const cplx* M, int nvb, int nc, const
     g.A = M + (long long)v0 * nc * n_g; g.lda = n_g; g.a_km = false;
     g.B = C; g.ldb = n_g; g.b_kn = false;
     g.C = Bp; g.ldc = n_eig; g.M = P; g.N = n_eig; g.K = n_g; g.conj_b = true;
-    g.wmode = 2; g.wk = ctx->d_vsqrt;
-    int rc = zgemm_dmma(ctx, g);
+    g.wk = ctx->d_vsqrt;
+    rc = zgemm_dmma(ctx, g);
     if (rc) return rc;
     // chi_s[k] (+)= - sum_p Bp[p][:] D_p(w_k) Bp[p][:]^H                   (eq. 8)
     ZgemmParams h;
     h.A = Bp; h.lda = n_eig; h.a_km = true; h.B = Bp; h.ldb = n_eig; h.b_kn = true;
     h.C = chi_s; h.ldc = n_eig; h.M = n_eig; h.N = n_eig; h.K = P;
     h.conj_b = true; h.herm = true; h.accumulate = (accumulate != 0) || v0 > 0; h.alpha = -1.0;
-    h.wmode = 1; h.e_v = e_v + v0; h.e_c = e_c; h.nc = nc; h.omega = omega;
+    h.wk = wk + (long long)v0 * nc; h.strideW = Pall;
     h.batch = n_w; h.strideC = (long long)n_eig * n_eig;
     rc = zgemm_dmma(ctx, h);
     if (rc) return rc;
@@ -161,7 +171,8 @@ size_t rpa_workspace_bytes(const rpa_ctx* ctx, int nvb, int nc, int n_eig, int n
   if (!ctx || nvb < 1 || nc < 1 || n_eig < 1 || n_w < 1) return 0;
   size_t need = mtxel_workspace_bytes(ctx, nvb, nc);
   need = std::max(need, basis_workspace_bytes(ctx, ctx->n_g, n_eig));
-  need = std::max(need, chi_freq_workspace(ctx, nvb, nc, n_eig));
+  need = std::max(need, chi_freq_workspace(ctx, nvb, nc, n_eig, n_w));
+  need = std::max(need, chi0_static_workspace(nvb, nc));
   need = std::max(need, energy_workspace_bytes(ctx, n_eig, n_w));
   return need + 4096;
 }
@@ -189,7 +200,8 @@ int rpa_chi0_static(rpa_ctx* ctx, const void* M, int nvb, int nc, const double* 
   if (!M || !e_v || !e_c || !chi0 || nvb < 1 || nc < 1) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_chi0_static: invalid argument");
   if ((long long)nvb * nc > 2147483647LL) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_chi0_static: too many pairs");
   RPA_CUDA(ctx, cudaSetDevice(ctx->device));
-  return do_chi0_static(ctx, (const cplx*)M, nvb, nc, e_v, e_c, accumulate, (cplx*)chi0);
+  WsAlloc ws(ctx->ws, ctx->ws_bytes);
+  return do_chi0_static(ctx, ws, (const cplx*)M, nvb, nc, e_v, e_c, accumulate, (cplx*)chi0);
 }
 
 int rpa_subspace_basis(rpa_ctx* ctx, const void* chi0, int n_eig, double tol, void* C, double* lambda, int* iters_out) {
@@ -296,7 +308,8 @@ int rpa_energy_device(rpa_ctx* ctx, const void* psi_v_, int nv, const void* psi_
     WsAlloc s1(scratch, scratch_bytes);
     tic(0); rc = mtxel_run(ctx, s1, psi_v + (size_t)v0 * n_pw, nb, psi_c, nc, M); toc();
     if (rc) break;
-    tic(1); rc = do_chi0_static(ctx, M, nb, nc, e_v + v0, e_c, b > 0, chi0); toc();
+    WsAlloc s2(scratch, scratch_bytes);
+    tic(1); rc = do_chi0_static(ctx, s2, M, nb, nc, e_v + v0, e_c, b > 0, chi0); toc();
   }
   if (!rc) {
     WsAlloc s2(scratch, scratch_bytes);

@@ -85,15 +85,16 @@ struct ZgemmParams {
   double alpha = 1.0;
   const double* rs = nullptr; // [M] optional
   const double* cs = nullptr; // [N] optional
-  // k weights: mode 0 none, 1 pair weights 2 D/(D^2+w^2) with D = e_c[k % nc] - e_v[k / nc], 2 vector wk[k]
-  int wmode = 0;
-  const double* e_v = nullptr; const double* e_c = nullptr; int nc = 1;
-  const double* omega = nullptr;  // dev, [batch] (mode 1; nullptr = 0)
-  const double* wk = nullptr;
+  // k weights: wk == nullptr none, else w_k = wk[batch * strideW + k] (the pair weights D_vc(i omega) of eq. 5 written
+  // by pair_weights(), or v^1/2 for the projection)
+  const double* wk = nullptr; long long strideW = 0;
   int batch = 1; long long strideA = 0, strideB = 0, strideC = 0;
   int split_k = 0;            // 0 = choose automatically
 };
 int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p);
+// out[k][v * nc + c] = 2 D/(D^2 + omega_k^2), D = e_c[c] - e_v[v]  (eq. 5 in the reading R6); omega == nullptr: one
+// row with omega = 0
+int pair_weights(rpa_ctx* ctx, const double* e_v, const double* e_c, int nvb, int nc, const double* omega, int n_w, double* out);
 int fp64_peak_kernel(rpa_ctx* ctx, int kind, int iters, double* tflops);
 
 // mtxel.cu

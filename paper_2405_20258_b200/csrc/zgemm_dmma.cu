@@ -6,10 +6,13 @@
 //   C[m][n] (+)= alpha rs[m] cs[n] sum_k w_k A^(m,k) opB(B^(n,k))
 //
 // One complex MAC = 4 real DMMAs on (re, im) fragments:  Cre += Ar Br + Ai Bi ; Cim += Ai Br - Ar Bi  (opB = conj).
-// The diagonal weight w_k (Delta of eq. 5 in the D(i omega) form) is fused into the A fragment after it is read
+// The diagonal weight w_k (Delta of eq. 5 in the D(i omega) form, written once per block by pair_weights) rides the
+// cp.async ring with the operand tiles and is fused into the A fragment after it is read
 // from shared memory; v^1/2 is fused into the epilogue (rs, cs).  Operand tiles are staged global -> shared with
 // cp.async (16 B = one complex element) in a 2-3 stage ring, in their native interleaved layout; padding makes the
 // 128-bit fragment loads bank-conflict free (leading dimension = 2 mod 8 elements for [k][m], 4 mod 8 for [m][k]).
+#include <algorithm>
+
 #include "rpa_internal.h"
 
 namespace {
@@ -31,6 +34,11 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem, bool va
   int sz = valid ? 16 : 0;
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(sz));
 }
+__device__ __forceinline__ void cp_async8(void* smem, const void* gmem, bool valid) {   // one double, zero-filled if !valid
+  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  int sz = valid ? 8 : 0;
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(s), "l"(gmem), "r"(sz));
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
@@ -40,10 +48,10 @@ struct KArgs {
   const cplx* B; long long ldb;
   cplx* C; long long ldc;
   int M, N, K;
-  int conj_b, herm, accumulate, atomic;
+  int herm, accumulate, atomic;
   double alpha;
   const double* rs; const double* cs;
-  int wmode; const double* e_v; const double* e_c; int nc; const double* omega; const double* wk;
+  const double* wk; long long strideW;
   long long strideA, strideB, strideC;
   int tiles_n, kt_per_split, n_kt;
 };
@@ -65,7 +73,7 @@ __device__ __forceinline__ void load_tile(cplx* s, const cplx* g, long long ld, 
   }
 }
 
-template <bool A_KM, bool B_KN, int STAGES>
+template <bool A_KM, bool B_KN, bool CONJ_B, int STAGES>
 __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int TA = A_KM ? TILE_KM : TILE_MK;
@@ -99,23 +107,17 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
   const int kt1 = min(p.n_kt, kt0 + p.kt_per_split);
   const int nkt = kt1 - kt0;
   if (nkt <= 0) return;
-  double om2 = 0.0;
-  if (p.wmode == 1 && p.omega) { double w = p.omega[batch]; om2 = w * w; }
+  const double* wk = p.wk ? p.wk + batch * p.strideW : nullptr;
 
   auto load_stage = [&](int stage, int kt) {
     const int k0 = kt * BK;
     load_tile<A_KM>(sA + stage * TA, A, p.lda, m0, p.M, k0, p.K, tid);
     load_tile<B_KN>(sB + stage * TB, B, p.ldb, n0, p.N, k0, p.K, tid);
-    if (tid < BK) {
-      double w = 1.0;
-      int kk = k0 + tid;
-      if (kk >= p.K) w = 0.0;
-      else if (p.wmode == 1) {
-        int v = kk / p.nc, c = kk - v * p.nc;
-        double d = p.e_c[c] - p.e_v[v];
-        w = 2.0 * d / (d * d + om2);
-      } else if (p.wmode == 2) w = p.wk[kk];
-      sW[stage * BK + tid] = w;
+    if (tid < BK) {   // the BK weights of this k-tile (zero beyond K, so ragged tiles add nothing)
+      double* dst = sW + stage * BK + tid;
+      const int kk = k0 + tid;
+      if (wk) cp_async8(dst, kk < p.K ? wk + kk : wk, kk < p.K);
+      else dst[0] = 1.0;   // operand tiles are zero-filled beyond K
     }
   };
 
@@ -147,27 +149,34 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
     for (int k4 = 0; k4 < BK / 4; k4++) {
       const int k = k4 * 4 + q;
       const double w = w_s[k];
-      double ar[4], ai[4], nar[4], br[4], bi[4];
+      double ar[4], ai[4], br[4], bi[4];
 #pragma unroll
       for (int i = 0; i < 4; i++) {
         const int m = wm * 32 + i * 8 + g;
         cplx a = A_KM ? a_s[k * LD_KM + m] : a_s[m * LD_MK + k];
-        ar[i] = a.x * w; ai[i] = a.y * w; nar[i] = -ar[i];
+        ar[i] = a.x * w; ai[i] = a.y * w;
       }
 #pragma unroll
       for (int j = 0; j < 4; j++) {
         const int n = wn * 32 + j * 8 + g;
         cplx b = B_KN ? b_s[k * LD_KM + n] : b_s[n * LD_MK + k];
-        br[j] = b.x; bi[j] = p.conj_b ? b.y : -b.y;
+        br[j] = b.x; bi[j] = b.y;
       }
+      // a conj(b): re += ar br + ai bi, im += ai br - ar bi;  a b: re += ar br - ai bi, im += ai br + ar bi.  The sign is
+      // a compile-time negation of the A operand, which DMMA takes as an operand modifier (no FP64 instruction).
 #pragma unroll
       for (int i = 0; i < 4; i++)
 #pragma unroll
         for (int j = 0; j < 4; j++) {
           dmma(cre[i][j][0], cre[i][j][1], ar[i], br[j]);
           dmma(cim[i][j][0], cim[i][j][1], ai[i], br[j]);
-          dmma(cre[i][j][0], cre[i][j][1], ai[i], bi[j]);
-          dmma(cim[i][j][0], cim[i][j][1], nar[i], bi[j]);
+        }
+#pragma unroll
+      for (int i = 0; i < 4; i++)
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+          dmma(cre[i][j][0], cre[i][j][1], CONJ_B ? ai[i] : -ai[i], bi[j]);
+          dmma(cim[i][j][0], cim[i][j][1], CONJ_B ? -ar[i] : ar[i], bi[j]);
         }
     }
   }
@@ -218,13 +227,13 @@ __global__ void herm_mirror_kernel(cplx* C, long long ldc, long long strideC, in
   }
 }
 
-template <bool A_KM, bool B_KN>
+template <bool A_KM, bool B_KN, bool CONJ_B>
 int launch(rpa_ctx* ctx, const KArgs& ka, dim3 grid) {
   constexpr int STAGES = (A_KM || B_KN) ? 3 : 2;
   constexpr int TA = A_KM ? TILE_KM : TILE_MK;
   constexpr int TB = B_KN ? TILE_KM : TILE_MK;
   constexpr size_t smem = (size_t)STAGES * (TA + TB) * sizeof(cplx) + STAGES * BK * sizeof(double);
-  auto kern = zgemm_dmma_kernel<A_KM, B_KN, STAGES>;
+  auto kern = zgemm_dmma_kernel<A_KM, B_KN, CONJ_B, STAGES>;
   static bool attr_set = false;
   if (!attr_set) {
     RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -243,9 +252,9 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
   KArgs ka;
   ka.A = p.A; ka.lda = p.lda; ka.B = p.B; ka.ldb = p.ldb; ka.C = p.C; ka.ldc = p.ldc;
   ka.M = p.M; ka.N = p.N; ka.K = p.K;
-  ka.conj_b = p.conj_b; ka.herm = p.herm; ka.accumulate = p.accumulate;
+  ka.herm = p.herm; ka.accumulate = p.accumulate;
   ka.alpha = p.alpha; ka.rs = p.rs; ka.cs = p.cs;
-  ka.wmode = p.wmode; ka.e_v = p.e_v; ka.e_c = p.e_c; ka.nc = p.nc > 0 ? p.nc : 1; ka.omega = p.omega; ka.wk = p.wk;
+  ka.wk = p.wk; ka.strideW = p.strideW;
   ka.strideA = p.strideA; ka.strideB = p.strideB; ka.strideC = p.strideC;
   const int tiles_m = (p.M + BM - 1) / BM, tiles_n = (p.N + BN - 1) / BN;
   ka.tiles_n = tiles_n;
@@ -291,16 +300,40 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
     return rpa_fail(ctx, RPA_ERR_INVALID, "zgemm_dmma: grid too large");
   dim3 grid((unsigned)tiles, (unsigned)split, (unsigned)p.batch);
   int rc;
-  if (p.a_km && p.b_kn) rc = launch<true, true>(ctx, ka, grid);
-  else if (p.a_km && !p.b_kn) rc = launch<true, false>(ctx, ka, grid);
-  else if (!p.a_km && p.b_kn) rc = launch<false, true>(ctx, ka, grid);
-  else rc = launch<false, false>(ctx, ka, grid);
+  // the combinations the library uses: [k][m] x [k][n] conj (CHI_SUM, chi_s), [m][k] x [m][k] conj (projection, Gram,
+  // Cholesky updates), [m][k] x [k][n] conj / plain (subspace iteration, rotations, triangular solves)
+  if (p.a_km && p.b_kn && p.conj_b) rc = launch<true, true, true>(ctx, ka, grid);
+  else if (!p.a_km && !p.b_kn && p.conj_b) rc = launch<false, false, true>(ctx, ka, grid);
+  else if (!p.a_km && p.b_kn && p.conj_b) rc = launch<false, true, true>(ctx, ka, grid);
+  else if (!p.a_km && p.b_kn && !p.conj_b) rc = launch<false, true, false>(ctx, ka, grid);
+  else return rpa_fail(ctx, RPA_ERR_INVALID, "zgemm_dmma: operand layout combination not instantiated");
   if (rc) return rc;
   if (ka.atomic && p.herm) {
     dim3 mg((p.N + 255) / 256, p.N, p.batch);
     herm_mirror_kernel<<<mg, 256, 0, ctx->stream>>>(p.C, p.ldc, p.strideC, p.N);
     RPA_LAUNCH_CHECK(ctx);
   }
+  return RPA_OK;
+}
+
+namespace {
+__global__ void pair_weights_kernel(const double* __restrict__ e_v, const double* __restrict__ e_c, int nc, long long P,
+                                    const double* __restrict__ omega, double* __restrict__ out) {
+  const double w = omega ? omega[blockIdx.y] : 0.0, w2 = w * w;
+  double* o = out + blockIdx.y * P;
+  for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < P; k += (long long)gridDim.x * blockDim.x) {
+    const int v = (int)(k / nc), c = (int)(k - (long long)v * nc);
+    const double d = e_c[c] - e_v[v];
+    o[k] = 2.0 * d / (d * d + w2);
+  }
+}
+}  // namespace
+
+int pair_weights(rpa_ctx* ctx, const double* e_v, const double* e_c, int nvb, int nc, const double* omega, int n_w, double* out) {
+  const long long P = (long long)nvb * nc;
+  dim3 grid((unsigned)std::min<long long>((P + 255) / 256, 4096), omega ? n_w : 1);
+  pair_weights_kernel<<<grid, 256, 0, ctx->stream>>>(e_v, e_c, nc, P, omega, out);
+  RPA_LAUNCH_CHECK(ctx);
   return RPA_OK;
 }
 
