@@ -209,6 +209,7 @@ def main():
     l0 = rpa.rpa_launch_count(ctx)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     stage_acc = {}
+    rpa.rpa_profile_begin(ctx)          # event pairs around every launch of the hot kernel classes (device time per class)
     e0.record()
     for _ in range(args.steps):
         res = step_dev()
@@ -218,6 +219,7 @@ def main():
     barrier()
     ms = e0.elapsed_time(e1)
     launches = rpa.rpa_launch_count(ctx) - l0
+    kprof = rpa.rpa_profile_end(ctx)
     clocks = sampler.stop()
     if world > 1:
         import torch.distributed as dist
@@ -261,21 +263,54 @@ def main():
                      "frac_of_dmma_peak": (work["proj_flops"] + work["chis_flops"]) / (stage_ms["chi_freq"] * 1e-3) / 1e12 / dmma_peak},
         "energy": {"ms": stage_ms["energy"]},
     }
-    # dominant kernel of the step by device time: the DMMA contraction (a2 + a4 run the same kernel) or MTXEL
-    t_dmma = stage_ms["chi0_static"] + stage_ms["chi_freq"]
-    if t_dmma >= stage_ms["mtxel"]:
-        fl = work["chi0_flops"] + work["proj_flops"] + work["chis_flops"]
-        ach = fl / (t_dmma * 1e-3) / 1e12
-        roofline = {"kernel": "zgemm_dmma_kernel (CHI_SUM a2 + projection/chi_s a4)", "bound": "tensor", "achieved": ach,
-                    "peak": dmma_peak, "unit": "TFLOP/s", "frac": ach / dmma_peak, "traffic": None,
+    # per-kernel-class device time (CUDA events around each launch, inside the timed region) and algorithmic work
+    n_r, n3 = int(np.prod(inp.fft)), int(inp.fft[2])
+    nk = [len(np.unique(inp.g_eps[:, a])) for a in range(3)]
+    P = nv * nc
+    kwork = {   # (unit, algorithmic work per E_c)
+        "mtxel_plane": ("B", passes * P * 16.0 * (n_r + nk[0] * nk[1] * n3)),   # read one real-space function, write its kept plane frequencies
+        "mtxel_z": ("B", passes * P * 16.0 * (nk[0] * nk[1] * n3 + ng)),
+        "chi0": ("FLOP", work["chi0_flops"]), "proj": ("FLOP", work["proj_flops"]), "chis": ("FLOP", work["chis_flops"]),
+    }
+    kernels = {}
+    for k, (kms, kn) in kprof.items():
+        ent = {"ms_per_step": kms / args.steps, "launches_per_step": kn / args.steps}
+        if k in kwork and kms > 0:
+            unit, w = kwork[k]
+            rate = w / (kms / args.steps * 1e-3)
+            ent.update({"GBps": rate / 1e9, "frac_of_hbm": rate / 1e9 / hbm_peak} if unit == "B" else
+                       {"TFLOPs": rate / 1e12, "frac_of_dmma_peak": rate / 1e12 / dmma_peak})
+        kernels[k] = ent
+    traffic_tab = {}
+    try:
+        traffic_tab = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))
+    except Exception:
+        pass
+    dom = max(kwork, key=lambda k: kernels[k]["ms_per_step"])
+    kd = kernels[dom]
+    names = {"mtxel_plane": "pair_plane_fft8_kernel (MTXEL a1: pair product + pruned xy transforms)",
+             "mtxel_z": "fft_axis_kernel<false,1> (MTXEL a1: z transform + sphere gather)",
+             "chi0": "zgemm_dmma_kernel<1,1,1,3> (CHI_SUM a2)", "proj": "zgemm_dmma_kernel<0,0,1,2> (projection a4)",
+             "chis": "zgemm_dmma_kernel<1,1,1,3> batched over omega (chi_s a4)"}
+    tr = traffic_tab.get(f"{dom}:cfg{args.config}")
+    if kwork[dom][0] == "B":
+        per_launch = kwork[dom][1] / max(1.0, kd["launches_per_step"])
+        avg_s = kd["ms_per_step"] * 1e-3 / max(1.0, kd["launches_per_step"])
+        roofline = {"kernel": names[dom], "bound": "hbm", "achieved": per_launch / avg_s / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                    "frac": per_launch / avg_s / 1e9 / hbm_peak, "traffic": tr, "peak_source": hbm_src,
+                    "algorithmic_bytes_per_launch": per_launch, "avg_launch_ms": avg_s * 1e3,
+                    "bytes_model": "16 B x (N_r + nk_x nk_y N_z) per (v,c) pair in the launch (DESIGN.md 5.2)",
+                    "share_of_step": kd["ms_per_step"] / ms_per_step}
+    else:
+        per_launch = kwork[dom][1] / max(1.0, kd["launches_per_step"])
+        avg_s = kd["ms_per_step"] * 1e-3 / max(1.0, kd["launches_per_step"])
+        roofline = {"kernel": names[dom], "bound": "tensor", "achieved": per_launch / avg_s / 1e12, "peak": dmma_peak,
+                    "unit": "TFLOP/s", "frac": per_launch / avg_s / 1e12 / dmma_peak, "traffic": tr,
                     "peak_source": "FP64 mma.sync m8n8k4 register-only microbenchmark measured in this run (rpa_fp64_peak); "
                                    "MEASURED_PEAKS.json has no FP64 entry",
-                    "flops_per_launch_model": "8 flop per complex MAC; HERK counts the lower triangle only"}
-    else:
-        ach = work["mtxel_bytes"] / (stage_ms["mtxel"] * 1e-3) / 1e9
-        roofline = {"kernel": "pair_plane_kernel + fft_axis_kernel (MTXEL a1)", "bound": "hbm", "achieved": ach, "peak": hbm_peak,
-                    "unit": "GB/s", "frac": ach / hbm_peak, "traffic": None, "peak_source": hbm_src,
-                    "bytes_model": "16 B x (N_r + N_G) per (v,c) pair per pass"}
+                    "algorithmic_flops_per_launch": per_launch, "avg_launch_ms": avg_s * 1e3,
+                    "flops_model": "8 flop per complex MAC; Hermitian updates count the lower triangle only (DESIGN.md 5.1)",
+                    "share_of_step": kd["ms_per_step"] / ms_per_step}
     cpu_baseline = None
     if not args.no_cpu_baseline:
         s = oracle_sample(inp, n_eig, args.ref_pairs)
@@ -286,7 +321,7 @@ def main():
             "vs_baseline": None, "dtype": "c128 (f64)", "data": "synthetic",
             "config": {"workload": workload, "keep_m": bool(args.keep_m), "mtxel_passes": passes,
                        "l2": "no flush needed: every step streams M blocks / real-space boxes far larger than the 126 MB L2"},
-            "E_c": res["E_c"], "stages": stages, "roofline": roofline,
+            "E_c": res["E_c"], "stages": stages, "kernels": kernels, "roofline": roofline,
             "fp64_peaks_measured": {"dmma_tflops": dmma_peak, "dfma_tflops": dfma_peak},
             "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks}
     print(json.dumps(line))

@@ -119,6 +119,16 @@ int rpa_energy_host(rpa_ctx* ctx, const void* psi_v, int nv, const void* psi_c, 
  *   kind 0: mma.sync m8n8k4 f64 (DMMA), kind 1: DFMA.  Returns TFLOP/s in *tflops; runs `iters`
  *   launches of a fixed-size kernel on the context stream and synchronises.                      */
 int rpa_fp64_peak(rpa_ctx* ctx, int kind, int iters, double* tflops);
+/* Per-kernel-class device times (bench.py's roofline of the dominant kernel).  Between rpa_profile_begin and
+ * rpa_profile_end every launch of the classes below is bracketed by a pair of CUDA events on the context stream;
+ * rpa_profile_end synchronises and returns, per class, the summed device time in ms and the number of timed launches
+ * (host out, arrays of RPA_PROF_NCLASS).  Classes: the MTXEL plane kernel (product + pruned xy transforms), the MTXEL z
+ * transform + sphere gather, the wavefunction -> real-space transforms, the CHI_SUM(0) contraction, the projection
+ * GEMM, the chi_s(i omega) contraction, the whole basis stage, the whole E_c stage.                                 */
+enum { RPA_PROF_MTXEL_PLANE = 0, RPA_PROF_MTXEL_Z = 1, RPA_PROF_MTXEL_WFN = 2, RPA_PROF_CHI0 = 3, RPA_PROF_PROJ = 4,
+       RPA_PROF_CHIS = 5, RPA_PROF_BASIS = 6, RPA_PROF_ENERGY = 7, RPA_PROF_NCLASS = 8 };
+int rpa_profile_begin(rpa_ctx* ctx);
+int rpa_profile_end(rpa_ctx* ctx, double* ms, long long* launches);
 /* Number of kernels launched by this context since creation (for bench.py's gpu_launches). */
 long long rpa_launch_count(const rpa_ctx* ctx);
 

@@ -17,6 +17,7 @@ EXPORTED_SYMBOLS = [
     "rpa_create", "rpa_destroy", "rpa_last_error", "rpa_workspace_bytes", "rpa_energy_workspace_bytes",
     "rpa_set_workspace", "rpa_mtxel", "rpa_chi0_static", "rpa_subspace_basis", "rpa_chi_subspace_freq",
     "rpa_correlation_energy", "rpa_energy_device", "rpa_energy_host", "rpa_fp64_peak", "rpa_launch_count",
+    "rpa_profile_begin", "rpa_profile_end",
 ]
 
 
@@ -76,6 +77,10 @@ def load_library(build_if_missing: bool = True):
     lib.rpa_energy_host.restype = ci
     lib.rpa_fp64_peak.argtypes = [vp, ci, ci, pd]
     lib.rpa_fp64_peak.restype = ci
+    lib.rpa_profile_begin.argtypes = [vp]
+    lib.rpa_profile_begin.restype = ci
+    lib.rpa_profile_end.argtypes = [vp, pd, C.POINTER(C.c_longlong)]
+    lib.rpa_profile_end.restype = ci
     lib.rpa_launch_count.argtypes = [vp]
     lib.rpa_launch_count.restype = C.c_longlong
     _LIB = lib
@@ -247,3 +252,19 @@ def rpa_fp64_peak(ctx, kind: int, iters: int = 20) -> float:
 
 def rpa_launch_count(ctx) -> int:
     return int(load_library().rpa_launch_count(ctx.handle))
+
+
+PROFILE_CLASSES = ("mtxel_plane", "mtxel_z", "mtxel_wfn", "chi0", "proj", "chis", "basis", "energy")
+
+
+def rpa_profile_begin(ctx):
+    _check(ctx.handle, load_library().rpa_profile_begin(ctx.handle))
+
+
+def rpa_profile_end(ctx):
+    """{class: (device ms, timed launches)} for the calls since rpa_profile_begin."""
+    n = len(PROFILE_CLASSES)
+    ms = (C.c_double * n)()
+    cnt = (C.c_longlong * n)()
+    _check(ctx.handle, load_library().rpa_profile_end(ctx.handle, ms, cnt))
+    return {k: (ms[i], int(cnt[i])) for i, k in enumerate(PROFILE_CLASSES)}

@@ -49,6 +49,7 @@ int do_chi0_static(rpa_ctx* ctx, WsAlloc& ws, const cplx* M, int nvb, int nc, co
   g.conj_b = true; g.herm = true; g.accumulate = accumulate != 0; g.alpha = -1.0;
   g.rs = ctx->d_vsqrt; g.cs = ctx->d_vsqrt;
   g.wk = wk;
+  ProfScope ps(ctx, RPA_PROF_CHI0);
   return zgemm_dmma(ctx, g);
 }
 
@@ -68,6 +69,7 @@ int do_chi_freq(rpa_ctx* ctx, WsAlloc& ws, const cplx* M, int nvb, int nc, const
     g.rs = ctx->d_vsqrt; g.cs = ctx->d_vsqrt;
     g.wk = wk; g.strideW = Pall;
     g.batch = n_w; g.strideC = (long long)n_g * n_g;
+    ProfScope ps(ctx, RPA_PROF_CHIS);
     return zgemm_dmma(ctx, g);
   }
   const int vchunk = (int)chi_freq_vchunk(ctx, nvb, nc, n_eig);
@@ -82,7 +84,7 @@ int do_chi_freq(rpa_ctx* ctx, WsAlloc& ws, const cplx* M, int nvb, int nc, const
     g.B = C; g.ldb = n_g; g.b_kn = false;
     g.C = Bp; g.ldc = n_eig; g.M = P; g.N = n_eig; g.K = n_g; g.conj_b = true;
     g.wk = ctx->d_vsqrt;
-    rc = zgemm_dmma(ctx, g);
+    { ProfScope ps(ctx, RPA_PROF_PROJ); rc = zgemm_dmma(ctx, g); }
     if (rc) return rc;
     // chi_s[k] (+)= - sum_p Bp[p][:] D_p(w_k) Bp[p][:]^H                   (eq. 8)
     ZgemmParams h;
@@ -91,7 +93,7 @@ int do_chi_freq(rpa_ctx* ctx, WsAlloc& ws, const cplx* M, int nvb, int nc, const
     h.conj_b = true; h.herm = true; h.accumulate = (accumulate != 0) || v0 > 0; h.alpha = -1.0;
     h.wk = wk + (long long)v0 * nc; h.strideW = Pall;
     h.batch = n_w; h.strideC = (long long)n_eig * n_eig;
-    rc = zgemm_dmma(ctx, h);
+    { ProfScope ps(ctx, RPA_PROF_CHIS); rc = zgemm_dmma(ctx, h); }
     if (rc) return rc;
   }
   return RPA_OK;
@@ -159,6 +161,8 @@ int rpa_destroy(rpa_ctx* ctx) {
   cudaSetDevice(ctx->device);
   mtxel_plan_destroy(ctx);
   cudaFree(ctx->d_vsqrt);
+  for (auto& r : ctx->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+  for (auto e : ctx->prof_pool) cudaEventDestroy(e);
   delete ctx;
   return RPA_OK;
 }
@@ -166,6 +170,30 @@ int rpa_destroy(rpa_ctx* ctx) {
 const char* rpa_last_error(const rpa_ctx* ctx) { return ctx ? ctx->err.c_str() : g_null_err.c_str(); }
 
 long long rpa_launch_count(const rpa_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int rpa_profile_begin(rpa_ctx* ctx) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  for (auto& r : ctx->prof_recs) { ctx->prof_pool.push_back(r.a); ctx->prof_pool.push_back(r.b); }
+  ctx->prof_recs.clear();
+  ctx->prof = true;
+  return RPA_OK;
+}
+
+int rpa_profile_end(rpa_ctx* ctx, double* ms, long long* launches) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  if (!ms || !launches) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_profile_end: null argument");
+  ctx->prof = false;
+  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
+  RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  for (int c = 0; c < RPA_PROF_NCLASS; c++) { ms[c] = 0.0; launches[c] = 0; }
+  for (auto& r : ctx->prof_recs) {
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess && r.cls >= 0 && r.cls < RPA_PROF_NCLASS) { ms[r.cls] += t; launches[r.cls]++; }
+    ctx->prof_pool.push_back(r.a); ctx->prof_pool.push_back(r.b);
+  }
+  ctx->prof_recs.clear();
+  return RPA_OK;
+}
 
 size_t rpa_workspace_bytes(const rpa_ctx* ctx, int nvb, int nc, int n_eig, int n_w) {
   if (!ctx || nvb < 1 || nc < 1 || n_eig < 1 || n_w < 1) return 0;

@@ -506,6 +506,7 @@ size_t basis_workspace_bytes(const rpa_ctx* ctx, int n, int n_eig) {
 
 int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, double tol, cplx* C, double* lambda,
               int* iters_out) {
+  ProfScope prof_scope(ctx, RPA_PROF_BASIS);
   if (tol <= 0.0) tol = 1e-11;
   std::vector<int> order_h;
   std::vector<double> lam_h;

@@ -55,6 +55,7 @@ size_t energy_workspace_bytes(const rpa_ctx* ctx, int n_eig, int n_w) {
 
 int energy_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi_s, int n_eig, const double* weight, int n_w, double* e_c,
                double* per_freq) {
+  ProfScope prof_scope(ctx, RPA_PROF_ENERGY);
   cplx* W = ws.get<cplx>((size_t)n_w * n_eig * n_eig);
   double* dvec = ws.get<double>((size_t)n_w * n_eig);
   double* t = ws.get<double>(n_w + 1);

@@ -438,10 +438,13 @@ int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx*
   RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
 
   int rc;
-  if ((rc = wfn_to_realspace(ctx, psi_v, nvb, u_v))) return rc;
+  { ProfScope ps(ctx, RPA_PROF_MTXEL_WFN); rc = wfn_to_realspace(ctx, psi_v, nvb, u_v); }
+  if (rc) return rc;
   for (int c0 = 0; c0 < nc; c0 += sz.ncc) {
     const int ncc = std::min(sz.ncc, nc - c0);
-    if ((rc = wfn_to_realspace(ctx, psi_c + (long long)c0 * ctx->n_pw, ncc, u_c))) return rc;
+    { ProfScope ps(ctx, RPA_PROF_MTXEL_WFN); rc = wfn_to_realspace(ctx, psi_c + (long long)c0 * ctx->n_pw, ncc, u_c); }
+    if (rc) return rc;
+    ProfScope* pp = new ProfScope(ctx, RPA_PROF_MTXEL_PLANE);
     switch (n8) {
       case 24: rc = launch_fft8<24>(ctx, u_v, u_c, nvb, ncc, N3, mp, T); break;
       case 40: rc = launch_fft8<40>(ctx, u_v, u_c, nvb, ncc, N3, mp, T); break;
@@ -454,11 +457,13 @@ int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx*
         RPA_LAUNCH_CHECK(ctx);
         rc = RPA_OK;
     }
+    delete pp;
     if (rc) return rc;
     ZScatter zs;
     zs.kpos3 = mp->ax[2].d_kpos; zs.nk3 = nk3; zs.inv_map = mp->d_inv_map; zs.M = M;
     zs.ncc = ncc; zs.nc = nc; zs.c0 = c0; zs.n_g = ctx->n_g; zs.scale = 1.0 / (double)n_r;
-    if ((rc = launch_axis<false, 1>(ctx, T, mp->ax[2].fwd(), (long long)nvb * ncc * J, J, zs))) return rc;
+    { ProfScope ps(ctx, RPA_PROF_MTXEL_Z); rc = launch_axis<false, 1>(ctx, T, mp->ax[2].fwd(), (long long)nvb * ncc * J, J, zs); }
+    if (rc) return rc;
   }
   return RPA_OK;
 }

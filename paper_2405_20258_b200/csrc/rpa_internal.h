@@ -33,8 +33,11 @@ struct rpa_ctx {
   char* ws = nullptr;
   size_t ws_bytes = 0;
 
-  cudaEvent_t ev[12];
-  bool ev_ok = false;
+  // per-kernel-class device timers (rpa_profile_begin / rpa_profile_end): event pairs around the launches of a class
+  bool prof = false;
+  struct ProfRec { int cls; cudaEvent_t a, b; };
+  std::vector<ProfRec> prof_recs;
+  std::vector<cudaEvent_t> prof_pool;
 };
 
 int rpa_fail(rpa_ctx* ctx, int code, const char* fmt, ...);
@@ -53,6 +56,27 @@ int rpa_fail(rpa_ctx* ctx, int code, const char* fmt, ...);
       return rpa_fail(ctx, RPA_ERR_CUDA, "kernel launch failed: %s (%s:%d)", cudaGetErrorString(e__), \
                       __FILE__, __LINE__);                                               \
   } while (0)
+
+// Times the launches enqueued during its lifetime under class `cls` (RPA_PROF_* of rpa_b200.h) when profiling is on.
+struct ProfScope {
+  rpa_ctx* ctx; bool on; rpa_ctx::ProfRec rec;
+  static cudaEvent_t get(rpa_ctx* c) {
+    cudaEvent_t e;
+    if (!c->prof_pool.empty()) { e = c->prof_pool.back(); c->prof_pool.pop_back(); }
+    else cudaEventCreate(&e);
+    return e;
+  }
+  ProfScope(rpa_ctx* c, int cls) : ctx(c), on(c->prof) {
+    if (!on) return;
+    rec.cls = cls; rec.a = get(c); rec.b = get(c);
+    cudaEventRecord(rec.a, c->stream);
+  }
+  ~ProfScope() {
+    if (!on) return;
+    cudaEventRecord(rec.b, ctx->stream);
+    ctx->prof_recs.push_back(rec);
+  }
+};
 
 // bump allocator over the caller's workspace (256-byte aligned)
 struct WsAlloc {
