@@ -145,7 +145,9 @@ def main():
     ap.add_argument("--n-v", type=int, default=None, help="override the number of valence bands (scaled-down twin)")
     ap.add_argument("--n-c", type=int, default=None)
     ap.add_argument("--n-eig", type=int, default=None)
-    ap.add_argument("--keep-m", type=int, default=0, help="1: keep M resident, skip the second MTXEL pass if it fits")
+    ap.add_argument("--keep-m", type=int, default=1,
+                    help="1 (default): keep all M blocks resident in HBM and skip the second MTXEL pass when they fit in 85 %% of the "
+                         "free device memory (the single-block case of PAPER.md:158); 0: always recompute")
     ap.add_argument("--ref-pairs", type=int, default=600, help="pairs in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -175,8 +177,15 @@ def main():
     dev = f"cuda:{local}"
     ctx = rpa.rpa_create(inp.cell, inp.fft, inp.g_eps, inp.vcoul, inp.g_wfn, device=local)
     need = rpa.rpa_energy_workspace_bytes(ctx, nv, nc, nvb, n_eig, n_w)
-    if args.keep_m:
-        need += nv * nc * ng * 16
+    m_all = nv * nc * ng * 16
+    free_b, _ = torch.cuda.mem_get_info(local)
+    inputs_b = sum(getattr(inp, k).nbytes for k in ("psi_v", "psi_c"))
+    keep_m = bool(args.keep_m) and nvb < nv and need + m_all + inputs_b <= 0.85 * free_b
+    if keep_m:
+        need += m_all
+    uc_all = nc * int(np.prod(inp.fft)) * 16 + 4096     # real-space conduction functions kept across valence blocks
+    if args.keep_m and nvb < nv and need + uc_all + inputs_b <= 0.85 * free_b:
+        need += uc_all
     ws = torch.empty(need, dtype=torch.uint8, device=dev)
     rpa.rpa_set_workspace(ctx, ws)
     d = {k: torch.from_numpy(getattr(inp, k)).to(dev) for k in ("psi_v", "psi_c", "e_v", "e_c", "omega", "weight")}
@@ -184,11 +193,11 @@ def main():
 
     def step_dev():
         return rpa.rpa_energy_device(ctx, d["psi_v"], d["psi_c"], d["e_v"], d["e_c"], nvb, n_eig, 0.0, d["omega"], d["weight"],
-                                     keep_m=bool(args.keep_m))
+                                     keep_m=keep_m)
 
     def step_host():
         return rpa.rpa_energy_host(ctx, h["psi_v"], h["psi_c"], h["e_v"], h["e_c"], nvb, n_eig, 0.0, h["omega"], h["weight"],
-                                   keep_m=bool(args.keep_m))
+                                   keep_m=keep_m)
 
     def barrier():
         if world > 1:
@@ -250,7 +259,7 @@ def main():
         pass
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     hbm_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
-    passes = 1 if (args.keep_m or nvb >= nv) else 2
+    passes = 1 if (keep_m or nvb >= nv) else 2
     work = algorithmic_work(inp, n_eig, passes)
     stages = {
         "mtxel": {"ms": stage_ms["mtxel"], "GBps": work["mtxel_bytes"] / (stage_ms["mtxel"] * 1e-3) / 1e9,
@@ -319,7 +328,7 @@ def main():
     line = {"metric": METRIC, "value": ms_per_step * 1e-3, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": n_warm, "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "strong",
             "vs_baseline": None, "dtype": "c128 (f64)", "data": "synthetic",
-            "config": {"workload": workload, "keep_m": bool(args.keep_m), "mtxel_passes": passes,
+            "config": {"workload": workload, "keep_m": keep_m, "mtxel_passes": passes,
                        "l2": "no flush needed: every step streams M blocks / real-space boxes far larger than the 126 MB L2"},
             "E_c": res["E_c"], "stages": stages, "kernels": kernels, "roofline": roofline,
             "fp64_peaks_measured": {"dmma_tflops": dmma_peak, "dfma_tflops": dfma_peak},

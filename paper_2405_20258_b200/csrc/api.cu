@@ -314,6 +314,15 @@ int rpa_energy_device(rpa_ctx* ctx, const void* psi_v_, int nv, const void* psi_
   if (!ws.ok || ws.off + stage_need > ctx->ws_bytes)
     return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_energy: workspace too small (need %zu bytes, have %zu)", ws.off + stage_need,
                     ctx->ws_bytes);
+  // several MTXEL calls on the same conduction bands: keep their real-space functions too if there is room
+  const int n_mtxel = keep_all ? nblocks : 2 * nblocks;
+  const size_t uc_bytes = ws_round((size_t)nc * ctx->n_r * sizeof(cplx));
+  ctx->uc_cache = nullptr; ctx->uc_cache_filled = false;
+  if (keep_m && n_mtxel > 1 && ws.off + uc_bytes + stage_need <= ctx->ws_bytes) {
+    ctx->uc_cache = ws.get<cplx>((size_t)nc * ctx->n_r);
+    ctx->uc_cache_src = psi_c; ctx->uc_cache_nc = nc;
+  }
+  struct CacheGuard { rpa_ctx* c; ~CacheGuard() { c->uc_cache = nullptr; c->uc_cache_filled = false; } } cache_guard{ctx};
   char* scratch = ctx->ws + ws.off;
   const size_t scratch_bytes = ctx->ws_bytes - ws.off;
 

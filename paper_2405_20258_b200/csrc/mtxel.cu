@@ -442,7 +442,12 @@ int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx*
   if (rc) return rc;
   for (int c0 = 0; c0 < nc; c0 += sz.ncc) {
     const int ncc = std::min(sz.ncc, nc - c0);
-    { ProfScope ps(ctx, RPA_PROF_MTXEL_WFN); rc = wfn_to_realspace(ctx, psi_c + (long long)c0 * ctx->n_pw, ncc, u_c); }
+    const bool cached = ctx->uc_cache && ctx->uc_cache_src == psi_c && ctx->uc_cache_nc == nc;
+    if (cached) u_c = ctx->uc_cache + (long long)c0 * n_r;
+    if (!cached || !ctx->uc_cache_filled) {
+      ProfScope ps(ctx, RPA_PROF_MTXEL_WFN);
+      rc = wfn_to_realspace(ctx, psi_c + (long long)c0 * ctx->n_pw, ncc, u_c);
+    }
     if (rc) return rc;
     ProfScope* pp = new ProfScope(ctx, RPA_PROF_MTXEL_PLANE);
     switch (n8) {
@@ -465,5 +470,6 @@ int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx*
     { ProfScope ps(ctx, RPA_PROF_MTXEL_Z); rc = launch_axis<false, 1>(ctx, T, mp->ax[2].fwd(), (long long)nvb * ncc * J, J, zs); }
     if (rc) return rc;
   }
+  if (ctx->uc_cache && ctx->uc_cache_src == psi_c && ctx->uc_cache_nc == nc) ctx->uc_cache_filled = true;
   return RPA_OK;
 }

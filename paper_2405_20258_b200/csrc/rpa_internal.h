@@ -33,6 +33,10 @@ struct rpa_ctx {
   char* ws = nullptr;
   size_t ws_bytes = 0;
 
+  // real-space conduction functions u_c kept across the valence blocks of one rpa_energy_* call when HBM allows
+  // (set by the driver in api.cu, used by mtxel_run): [uc_cache_nc][n_r], valid for coefficient array uc_cache_src
+  cplx* uc_cache = nullptr; const cplx* uc_cache_src = nullptr; int uc_cache_nc = 0; bool uc_cache_filled = false;
+
   // per-kernel-class device timers (rpa_profile_begin / rpa_profile_end): event pairs around the launches of a class
   bool prof = false;
   struct ProfRec { int cls; cudaEvent_t a, b; };

@@ -267,8 +267,9 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
     const long long slots = 2LL * ctx->sm_count;
     const long long base = tiles * p.batch;
     split = 1;
-    const int max_split = n_kt / 8;  // at least 8 k-tiles (128 k) per split
-    if (max_split > 1 && base < 8 * slots) {
+    int max_split = n_kt / 8;  // at least 8 k-tiles (128 k) per split
+    if (base >= 8 * slots) max_split = std::min(max_split, 4);   // many waves already: only trim the last partial wave
+    if (max_split > 1 && base < 64 * slots) {
       double best = 0.0;
       for (int s = 1; s <= max_split && s <= 64; s++) {
         const long long ctas = base * s;
