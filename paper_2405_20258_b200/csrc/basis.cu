@@ -277,6 +277,7 @@ __global__ void __launch_bounds__(256) pair_rotations_kernel(const cplx* __restr
       atomicMax((unsigned long long*)off_max, (unsigned long long)__double_as_longlong(off));
     }
   }
+  const int lane = tid & 31, wrp = tid >> 5;
   for (int r = 0; r < JP - 1; r++) {
     if (tid < JB) {
       int i, j;
@@ -297,28 +298,50 @@ __global__ void __launch_bounds__(256) pair_rotations_kernel(const cplx* __restr
       rp_[tid] = i; rq_[tid] = j; rc_[tid] = c; rs_[tid] = s; rx_[tid] = ex; ry_[tid] = ey;
     }
     __syncthreads();
-    // rows i, j of W and U:  x_i' = c x_i - s e^{i theta} x_j ;  x_j' = s x_i + c e^{i theta} x_j
-    for (int idx = tid; idx < 2 * JB * JP; idx += 256) {
-      const int half = idx / (JB * JP), rem = idx - half * (JB * JP);
-      const int k = rem / JP, col = rem - k * JP;
-      cplx* X = half ? U : W;
-      const int i = rp_[k], j = rq_[k];
-      const double c = rc_[k], s = rs_[k], ex = rx_[k], ey = ry_[k];
-      const cplx xi = X[i * JLD + col], xj = X[j * JLD + col];
-      const cplx ej = make_double2(ex * xj.x - ey * xj.y, ex * xj.y + ey * xj.x);   // e^{i theta} x_j
-      X[i * JLD + col] = make_double2(c * xi.x - s * ej.x, c * xi.y - s * ej.y);
-      X[j * JLD + col] = make_double2(s * xi.x + c * ej.x, s * xi.y + c * ej.y);
-    }
-    __syncthreads();
-    // columns i, j of W:  y_i' = c y_i - s e^{-i theta} y_j ;  y_j' = s y_i + c e^{-i theta} y_j
-    for (int idx = tid; idx < JB * JP; idx += 256) {
-      const int k = idx / JP, row = idx - k * JP;
-      const int i = rp_[k], j = rq_[k];
-      const double c = rc_[k], s = rs_[k], ex = rx_[k], ey = ry_[k];
-      const cplx yi = W[row * JLD + i], yj = W[row * JLD + j];
-      const cplx ej = make_double2(ex * yj.x + ey * yj.y, ex * yj.y - ey * yj.x);   // e^{-i theta} y_j
-      W[row * JLD + i] = make_double2(c * yi.x - s * ej.x, c * yi.y - s * ej.y);
-      W[row * JLD + j] = make_double2(s * yi.x + c * ej.x, s * yi.y + c * ej.y);
+    // W <- R W R^H on 2 x 2 blocks: block (k, l) = rows {i_k, j_k} x columns {i_l, j_l} is read and written by one thread
+    // only, so the row and the column rotation are applied together and in place.
+    //   rows:    x_i' = c x_i - s e^{i theta} x_j ;  x_j' = s x_i + c e^{i theta} x_j          (rotation of pair k)
+    //   columns: y_i' = c y_i - s e^{-i theta} y_j ; y_j' = s y_i + c e^{-i theta} y_j         (rotation of pair l)
+    {
+      const int pl = rp_[lane], ql = rq_[lane];
+      const double cl = rc_[lane], sl = rs_[lane], xl = rx_[lane], yl = ry_[lane];
+#pragma unroll
+      for (int m = 0; m < JB / 8; m++) {
+        const int k = wrp + 8 * m;
+        const double ck = rc_[k], sk = rs_[k];
+        if (sk == 0.0 && sl == 0.0) continue;
+        const int pk = rp_[k], qk = rq_[k];
+        const double xk = rx_[k], yk = ry_[k];
+        cplx w00 = W[pk * JLD + pl], w01 = W[pk * JLD + ql], w10 = W[qk * JLD + pl], w11 = W[qk * JLD + ql];
+        // rows
+        cplx e0 = make_double2(xk * w10.x - yk * w10.y, xk * w10.y + yk * w10.x);   // e^{i theta_k} w10
+        cplx e1 = make_double2(xk * w11.x - yk * w11.y, xk * w11.y + yk * w11.x);
+        cplx r00 = make_double2(ck * w00.x - sk * e0.x, ck * w00.y - sk * e0.y);
+        cplx r10 = make_double2(sk * w00.x + ck * e0.x, sk * w00.y + ck * e0.y);
+        cplx r01 = make_double2(ck * w01.x - sk * e1.x, ck * w01.y - sk * e1.y);
+        cplx r11 = make_double2(sk * w01.x + ck * e1.x, sk * w01.y + ck * e1.y);
+        // columns
+        cplx f0 = make_double2(xl * r01.x + yl * r01.y, xl * r01.y - yl * r01.x);   // e^{-i theta_l} r01
+        cplx f1 = make_double2(xl * r11.x + yl * r11.y, xl * r11.y - yl * r11.x);
+        W[pk * JLD + pl] = make_double2(cl * r00.x - sl * f0.x, cl * r00.y - sl * f0.y);
+        W[pk * JLD + ql] = make_double2(sl * r00.x + cl * f0.x, sl * r00.y + cl * f0.y);
+        W[qk * JLD + pl] = make_double2(cl * r10.x - sl * f1.x, cl * r10.y - sl * f1.y);
+        W[qk * JLD + ql] = make_double2(sl * r10.x + cl * f1.x, sl * r10.y + cl * f1.y);
+      }
+      // U <- R U (rows only)
+      const int col = tid & (JP - 1), k0 = tid >> 6;
+#pragma unroll
+      for (int m = 0; m < JB / 4; m++) {
+        const int k = k0 + 4 * m;
+        const double ck = rc_[k], sk = rs_[k];
+        if (sk == 0.0) continue;
+        const int pk = rp_[k], qk = rq_[k];
+        const double xk = rx_[k], yk = ry_[k];
+        const cplx ui = U[pk * JLD + col], uj = U[qk * JLD + col];
+        const cplx ej = make_double2(xk * uj.x - yk * uj.y, xk * uj.y + yk * uj.x);
+        U[pk * JLD + col] = make_double2(ck * ui.x - sk * ej.x, ck * ui.y - sk * ej.y);
+        U[qk * JLD + col] = make_double2(sk * ui.x + ck * ej.x, sk * ui.y + ck * ej.y);
+      }
     }
     __syncthreads();
   }
