@@ -175,16 +175,25 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl")
     dev = f"cuda:{local}"
+    if world > 1:
+        # strong scaling: the conduction bands (hence the (v,c) pairs) are sharded over the ranks, one all-reduce per pass
+        c0, c1 = rpa.shard_range(nc, world, rank)
+        inp.psi_c, inp.e_c = np.ascontiguousarray(inp.psi_c[c0:c1]), np.ascontiguousarray(inp.e_c[c0:c1])
+        nc = c1 - c0
+        comm = rpa.Comm()
     ctx = rpa.rpa_create(inp.cell, inp.fft, inp.g_eps, inp.vcoul, inp.g_wfn, device=local)
     need = rpa.rpa_energy_workspace_bytes(ctx, nv, nc, nvb, n_eig, n_w)
     m_all = nv * nc * ng * 16
     free_b, _ = torch.cuda.mem_get_info(local)
     inputs_b = sum(getattr(inp, k).nbytes for k in ("psi_v", "psi_c"))
     keep_m = bool(args.keep_m) and nvb < nv and need + m_all + inputs_b <= 0.85 * free_b
-    if keep_m:
+    if world > 1:   # the sharded driver keeps its M blocks in torch tensors: the workspace is stage scratch only
+        keep_m = bool(args.keep_m) and need + m_all + inputs_b <= 0.85 * free_b
+        need = rpa.rpa_workspace_bytes(ctx, nvb, nc, n_eig, n_w)
+    elif keep_m:
         need += m_all
     uc_all = nc * int(np.prod(inp.fft)) * 16 + 4096     # real-space conduction functions kept across valence blocks
-    if args.keep_m and nvb < nv and need + uc_all + inputs_b <= 0.85 * free_b:
+    if world == 1 and args.keep_m and nvb < nv and need + uc_all + inputs_b <= 0.85 * free_b:
         need += uc_all
     ws = torch.empty(need, dtype=torch.uint8, device=dev)
     rpa.rpa_set_workspace(ctx, ws)
@@ -192,10 +201,17 @@ def main():
     h = {k: torch.from_numpy(getattr(inp, k)).pin_memory() for k in ("psi_v", "psi_c", "e_v", "e_c", "omega", "weight")}
 
     def step_dev():
+        if world > 1:
+            return rpa.rpa_energy_sharded(ctx, d["psi_v"], d["psi_c"], d["e_v"], d["e_c"], nvb, n_eig, 0.0, d["omega"], d["weight"],
+                                          comm=comm, keep_m=keep_m)
         return rpa.rpa_energy_device(ctx, d["psi_v"], d["psi_c"], d["e_v"], d["e_c"], nvb, n_eig, 0.0, d["omega"], d["weight"],
                                      keep_m=keep_m)
 
     def step_host():
+        if world > 1:   # this rank's inputs from pinned host memory, then the sharded path; E_c read back inside
+            t = {k: h[k].to(dev, non_blocking=True) for k in h}
+            return rpa.rpa_energy_sharded(ctx, t["psi_v"], t["psi_c"], t["e_v"], t["e_c"], nvb, n_eig, 0.0, t["omega"], t["weight"],
+                                          comm=comm, keep_m=keep_m)
         return rpa.rpa_energy_host(ctx, h["psi_v"], h["psi_c"], h["e_v"], h["e_c"], nvb, n_eig, 0.0, h["omega"], h["weight"],
                                    keep_m=keep_m)
 
@@ -321,7 +337,7 @@ def main():
                     "flops_model": "8 flop per complex MAC; Hermitian updates count the lower triangle only (DESIGN.md 5.1)",
                     "share_of_step": kd["ms_per_step"] / ms_per_step}
     cpu_baseline = None
-    if not args.no_cpu_baseline:
+    if not args.no_cpu_baseline and world == 1:
         s = oracle_sample(inp, n_eig, args.ref_pairs)
         cpu_baseline = {"value": s["t_full_est_s"], "unit": UNIT, "cores": cpu_threads(), "kind": "oracle", "sample": s["sample"],
                         "t_sample_s": s["t_sample_s"]}
@@ -329,6 +345,7 @@ def main():
             "warmup": n_warm, "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "strong",
             "vs_baseline": None, "dtype": "c128 (f64)", "data": "synthetic",
             "config": {"workload": workload, "keep_m": keep_m, "mtxel_passes": passes,
+                       "parallelism": f"conduction bands sharded over {world} ranks, one all-reduce per pass" if world > 1 else "1 GPU",
                        "l2": "no flush needed: every step streams M blocks / real-space boxes far larger than the 126 MB L2"},
             "E_c": res["E_c"], "stages": stages, "kernels": kernels, "roofline": roofline,
             "fp64_peaks_measured": {"dmma_tflops": dmma_peak, "dfma_tflops": dfma_peak},

@@ -7,7 +7,9 @@ from .binding import (RpaContext, RpaError, load_library, library_path, EXPORTED
                       rpa_correlation_energy, rpa_energy_device, rpa_energy_host, rpa_fp64_peak, rpa_launch_count,
                       rpa_profile_begin, rpa_profile_end, PROFILE_CLASSES)
 
-__all__ = ["RpaContext", "RpaError", "load_library", "library_path", "EXPORTED_SYMBOLS",
+from .sharded import shard_range, Comm, rpa_energy_sharded
+
+__all__ = ["shard_range", "Comm", "rpa_energy_sharded", "RpaContext", "RpaError", "load_library", "library_path", "EXPORTED_SYMBOLS",
            "rpa_create", "rpa_destroy", "rpa_workspace_bytes", "rpa_energy_workspace_bytes", "rpa_set_workspace",
            "rpa_mtxel", "rpa_chi0_static", "rpa_subspace_basis", "rpa_chi_subspace_freq",
            "rpa_correlation_energy", "rpa_energy_device", "rpa_energy_host", "rpa_fp64_peak", "rpa_launch_count",

@@ -108,10 +108,11 @@ def _dev(t, dtype=None):
 class RpaContext:
     """Owns an rpa_ctx* and the workspace tensor lent to it."""
 
-    def __init__(self, handle, device):
+    def __init__(self, handle, device, n_g=None, n_pw=None):
         self.handle = handle
         self.device = device
         self.workspace = None
+        self.n_g, self.n_pw = n_g, n_pw
 
     def close(self):
         if self.handle:
@@ -144,7 +145,7 @@ def rpa_create(cell, fft, g_eps, vcoul, g_wfn, device: int = 0, stream=None) -> 
                         vcoul.ctypes.data_as(C.POINTER(C.c_double)), g_wfn.shape[0],
                         g_wfn.ctypes.data_as(C.POINTER(C.c_int32)), device, C.c_void_p(stream))
     _check(None, rc)
-    return RpaContext(h, device)
+    return RpaContext(h, device, n_g=int(g_eps.shape[0]), n_pw=int(g_wfn.shape[0]))
 
 
 def rpa_destroy(ctx: RpaContext):
