@@ -389,3 +389,59 @@ def test_medium_twin_against_golden():
     mu_ref = np.array(g["chi_s_eigs_first_freq"])
     assert np.abs(mu - mu_ref).max() <= 1e-10 * np.abs(mu_ref).max()
     assert g["E_c_full"] < g["E_c"] < 0
+
+
+def test_medium_config_full_size_sampled_and_properties():
+    """configs[2] at FULL size (256 x 6000 bands: 1.5e6 pairs, ~15 s of B200 time) in the launch configuration bench.py
+    times (rpa_energy_device, valence blocks of 32, M kept resident).  The oracle cannot run this size inside a test, so:
+    sampled M rows against the oracle computed pair by pair; properties that hold at any size (P4, P6, P7, P13,
+    E_c < 0, t_k < 0 and increasing with omega); and agreement of the driver with an independent accumulation order
+    through the stage calls (valence blocks of 64)."""
+    import paper_2405_20258_b200 as rpa
+    import torch
+    inp = make_inputs(2, qr_device="cuda")
+    nv, nc, ng, n_eig, n_w = 256, 6000, inp.n_g, inp.cfg.n_eig, len(inp.omega)
+    ctx = rpa.rpa_create(inp.cell, inp.fft, inp.g_eps, inp.vcoul, inp.g_wfn)
+    try:
+        need = rpa.rpa_energy_workspace_bytes(ctx, nv, nc, 32, n_eig, n_w) + nv * nc * ng * 16
+        ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+        rpa.rpa_set_workspace(ctx, ws)
+        psi_v, psi_c, e_v, e_c = dev(inp.psi_v), dev(inp.psi_c), dev(inp.e_v), dev(inp.e_c)
+        omega, weight = dev(inp.omega), dev(inp.weight)
+        r = rpa.rpa_energy_device(ctx, psi_v, psi_c, e_v, e_c, 32, n_eig, 0.0, omega, weight, keep_m=True)
+        assert r["E_c"] < 0 and np.all(r["t"] < 0) and np.all(np.diff(r["t"]) > 0)
+        assert np.all(np.diff(r["lam"]) >= 0) and r["lam"][-1] < 0
+        del ws
+        # sampled pairs: M through the C-ABI against the oracle's naive DFT
+        vs, cs = [0, 131, 255], [0, 2999, 5999]
+        M = torch.empty((3, 3, ng), dtype=torch.complex128, device="cuda")
+        ws = torch.empty(rpa.rpa_workspace_bytes(ctx, 64, nc, n_eig, n_w), dtype=torch.uint8, device="cuda")
+        rpa.rpa_set_workspace(ctx, ws)
+        rpa.rpa_mtxel(ctx, psi_v[vs].contiguous(), psi_c[cs].contiguous(), M)
+        Mref = orc.mtxel(inp.psi_v[vs], inp.psi_c[cs], inp.g_wfn, inp.g_eps, inp.fft)
+        assert maxnorm_rel(M.cpu().numpy(), Mref) <= 1e-12
+        g0 = int(np.where((inp.g_eps == 0).all(axis=1))[0][0])
+        assert np.abs(M.cpu().numpy()[:, :, g0]).max() < 1e-13                      # P4
+        # independent accumulation order through the stage calls
+        chi0 = torch.zeros((ng, ng), dtype=torch.complex128, device="cuda")
+        Mb = torch.empty((64, nc, ng), dtype=torch.complex128, device="cuda")
+        for b in range(0, nv, 64):
+            rpa.rpa_mtxel(ctx, psi_v[b:b + 64].contiguous(), psi_c, Mb)
+            rpa.rpa_chi0_static(ctx, Mb, e_v[b:b + 64].contiguous(), e_c, b > 0, chi0)
+        assert float((chi0 - chi0.conj().T).abs().max()) == 0.0                       # R20
+        Cm = torch.empty((n_eig, ng), dtype=torch.complex128, device="cuda")
+        lam = torch.empty(n_eig, dtype=torch.float64, device="cuda")
+        rpa.rpa_subspace_basis(ctx, chi0, n_eig, 0.0, Cm, lam)
+        assert eig_rel(lam.cpu().numpy(), r["lam"]) <= TOL_LAM
+        res = chi0 @ Cm.T - Cm.T * lam[None, :]                                       # P13 (torch = plumbing for the check)
+        assert float(res.abs().max()) <= 1e-10 * abs(r["lam"][0])
+        assert float((Cm.conj() @ Cm.T - torch.eye(n_eig, dtype=torch.complex128, device="cuda")).abs().max()) <= 1e-12
+        om0 = torch.zeros(1, dtype=torch.float64, device="cuda")                      # P7: chi_s(0) = diag(lambda)
+        chi_s0 = torch.zeros((1, n_eig, n_eig), dtype=torch.complex128, device="cuda")
+        for b in range(0, nv, 64):
+            rpa.rpa_mtxel(ctx, psi_v[b:b + 64].contiguous(), psi_c, Mb)
+            rpa.rpa_chi_subspace_freq(ctx, Mb, e_v[b:b + 64].contiguous(), e_c, Cm, n_eig, om0, b > 0, chi_s0)
+        dif = chi_s0[0] - torch.diag(lam).to(torch.complex128)
+        assert float(dif.abs().max()) <= 1e-10 * abs(r["lam"][0])
+    finally:
+        rpa.rpa_destroy(ctx)
