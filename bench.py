@@ -193,8 +193,8 @@ def main():
     elif keep_m:
         need += m_all
     uc_all = nc * int(np.prod(inp.fft)) * 16 + 4096     # real-space conduction functions kept across valence blocks
-    if world == 1 and args.keep_m and nvb < nv and need + uc_all + inputs_b <= 0.85 * free_b:
-        need += uc_all
+    if world == 1 and args.keep_m and nvb < nv:           # ... as many of them as fit in 85 % of the free memory
+        need += max(0, min(uc_all, int(0.85 * free_b) - need - inputs_b))
     ws = torch.empty(need, dtype=torch.uint8, device=dev)
     rpa.rpa_set_workspace(ctx, ws)
     d = {k: torch.from_numpy(getattr(inp, k)).to(dev) for k in ("psi_v", "psi_c", "e_v", "e_c", "omega", "weight")}

@@ -316,11 +316,15 @@ int rpa_energy_device(rpa_ctx* ctx, const void* psi_v_, int nv, const void* psi_
                     ctx->ws_bytes);
   // several MTXEL calls on the same conduction bands: keep their real-space functions too if there is room
   const int n_mtxel = keep_all ? nblocks : 2 * nblocks;
-  const size_t uc_bytes = ws_round((size_t)nc * ctx->n_r * sizeof(cplx));
-  ctx->uc_cache = nullptr; ctx->uc_cache_filled = false;
-  if (keep_m && n_mtxel > 1 && ws.off + uc_bytes + stage_need <= ctx->ws_bytes) {
-    ctx->uc_cache = ws.get<cplx>((size_t)nc * ctx->n_r);
-    ctx->uc_cache_src = psi_c; ctx->uc_cache_nc = nc;
+  const size_t per_band = (size_t)ctx->n_r * sizeof(cplx);
+  ctx->uc_cache = nullptr; ctx->uc_cache_filled = false; ctx->uc_cache_rows = 0;
+  if (keep_m && n_mtxel > 1 && ws.off + stage_need + 256 < ctx->ws_bytes) {
+    const size_t room = ctx->ws_bytes - ws.off - stage_need - 256;
+    const int rows = (int)std::min<size_t>((size_t)nc, room / per_band);   // as many bands as fit: the rest is recomputed
+    if (rows >= 64 || rows == nc) {
+      ctx->uc_cache = ws.get<cplx>((size_t)rows * ctx->n_r);
+      ctx->uc_cache_src = psi_c; ctx->uc_cache_nc = nc; ctx->uc_cache_rows = rows;
+    }
   }
   struct CacheGuard { rpa_ctx* c; ~CacheGuard() { c->uc_cache = nullptr; c->uc_cache_filled = false; } } cache_guard{ctx};
   char* scratch = ctx->ws + ws.off;

@@ -440,10 +440,14 @@ int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx*
   int rc;
   { ProfScope ps(ctx, RPA_PROF_MTXEL_WFN); rc = wfn_to_realspace(ctx, psi_v, nvb, u_v); }
   if (rc) return rc;
-  for (int c0 = 0; c0 < nc; c0 += sz.ncc) {
-    const int ncc = std::min(sz.ncc, nc - c0);
-    const bool cached = ctx->uc_cache && ctx->uc_cache_src == psi_c && ctx->uc_cache_nc == nc;
-    if (cached) u_c = ctx->uc_cache + (long long)c0 * n_r;
+  cplx* const u_c_scratch = u_c;
+  const bool have_cache = ctx->uc_cache && ctx->uc_cache_src == psi_c && ctx->uc_cache_nc == nc;
+  const int n_cached = have_cache ? ctx->uc_cache_rows : 0;   // the first n_cached conduction bands live in the cache
+  for (int c0 = 0, ncc = 0; c0 < nc; c0 += ncc) {
+    ncc = std::min(sz.ncc, nc - c0);
+    if (c0 < n_cached && c0 + ncc > n_cached) ncc = n_cached - c0;   // a chunk is either all cached or all scratch
+    const bool cached = c0 < n_cached;
+    u_c = cached ? ctx->uc_cache + (long long)c0 * n_r : u_c_scratch;
     if (!cached || !ctx->uc_cache_filled) {
       ProfScope ps(ctx, RPA_PROF_MTXEL_WFN);
       rc = wfn_to_realspace(ctx, psi_c + (long long)c0 * ctx->n_pw, ncc, u_c);

@@ -34,8 +34,9 @@ struct rpa_ctx {
   size_t ws_bytes = 0;
 
   // real-space conduction functions u_c kept across the valence blocks of one rpa_energy_* call when HBM allows
-  // (set by the driver in api.cu, used by mtxel_run): [uc_cache_nc][n_r], valid for coefficient array uc_cache_src
-  cplx* uc_cache = nullptr; const cplx* uc_cache_src = nullptr; int uc_cache_nc = 0; bool uc_cache_filled = false;
+  // (set by the driver in api.cu, used by mtxel_run): the first uc_cache_rows of the uc_cache_nc bands of coefficient
+  // array uc_cache_src, [uc_cache_rows][n_r]
+  cplx* uc_cache = nullptr; const cplx* uc_cache_src = nullptr; int uc_cache_nc = 0, uc_cache_rows = 0; bool uc_cache_filled = false;
 
   // per-kernel-class device timers (rpa_profile_begin / rpa_profile_end): event pairs around the launches of a class
   bool prof = false;
