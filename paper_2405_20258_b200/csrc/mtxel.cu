@@ -369,11 +369,19 @@ int wfn_to_realspace(rpa_ctx* ctx, const cplx* psi, int nb, cplx* u) {
 template <int N>
 int launch_fft8(rpa_ctx* ctx, const cplx* u_v, const cplx* u_c, int nvb, int ncc, int N3, const MtxelPlan* mp, cplx* T) {
   const int nk1 = mp->ax[0].nk, nk2 = mp->ax[1].nk;
-  const size_t smem = fft8::smem_bytes<N>(nk1, nk2);
-  auto kern = fft8::Geo<N>::MAXREG > 0 ? fft8::pair_plane_fft8_kernel_r<N> : fft8::pair_plane_fft8_kernel_b<N>;
+  // ring variant (no block barrier in the band loop) where one CTA fits per SM anyway; RPA_FFT8_RING=0/1 overrides
+  static const char* ring_env = getenv("RPA_FFT8_RING");
+  const size_t smem_ring = fft8::smem_bytes_ring<N>(nk2);
+  const bool ring_ok = smem_ring <= 227 * 1024 && (nk2 + fft8::Geo<N>::RW - 1) / fft8::Geo<N>::RW <= fft8::Geo<N>::NWARP;
+  const bool ring = ring_ok && (ring_env ? ring_env[0] == '1' : N >= 48);
+  const size_t smem = ring ? smem_ring : fft8::smem_bytes<N>(nk1, nk2);
+  auto kern = ring ? fft8::pair_plane_fft8_kernel_ring<N>
+                   : (fft8::Geo<N>::MAXREG > 0 ? fft8::pair_plane_fft8_kernel_r<N> : fft8::pair_plane_fft8_kernel_b<N>);
   static bool attr = false;
   if (!attr) {
-    RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_ring<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_r<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_b<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     attr = true;
     if (getenv("RPA_VERBOSE")) {
       cudaFuncAttributes fa;

@@ -211,6 +211,173 @@ __device__ __forceinline__ void pair_plane_fft8_body(const cplx* __restrict__ u_
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Ring variant of the same kernel (used where only ONE CTA fits per SM: N = 48, 64).  There is no block barrier in the
+// band loop: the column buffer is a ring of RING_D bands guarded by mbarriers (full[b]: all warps have written their rows
+// of the band into cb[b]; empty[b]: the x transforms of that band are done and cb[b] may be overwritten).  The x
+// transforms of band v are dealt, in batches of RW kept columns, to ncb warps that rotate with v, and a warp takes that
+// duty one band late -- so a warp with column duty falls behind by one duty and catches up while the others carry the
+// next bands, instead of every warp idling at a barrier while ncb of them transform columns.
+constexpr int RING_D = 3;
+
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+  asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  unsigned ok;
+  do {
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+                 : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+  } while (!ok);
+}
+
+template <int N>
+__device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict__ u_v, const cplx* __restrict__ u_c, int nvb, int ncc,
+                                                          int N3, const cplx* __restrict__ tw, const int* __restrict__ kfreq1,
+                                                          const int* __restrict__ kfreq2, int nk1, int nk2, cplx* __restrict__ T) {
+  using GE = Geo<N>;
+  constexpr int R2 = GE::R2, RW = GE::RW, NWARP = GE::NWARP, G = GE::G, PS = GE::PS, PW = GE::PW, PC = GE::PC, D = RING_D;
+  constexpr int NTHR = NWARP * 32;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx* sc = reinterpret_cast<cplx*>(smem_raw);   // [N][PS]  u_c plane
+  cplx* wk = sc + N * PS;                         // [N][PW]  pass-A output of the rows (warp-private rows)
+  cplx* cb0 = wk + N * PW;                        // D x [nk2][PC] kept y-frequencies, x contiguous
+  unsigned long long* slot2 = reinterpret_cast<unsigned long long*>(cb0 + D * nk2 * PC);
+  unsigned long long* slot1 = slot2 + 8;
+  unsigned long long* full = slot1 + 8;           // [D]
+  unsigned long long* empty = full + D;           // [D]
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int z = blockIdx.x / ncc, c = blockIdx.x - z * ncc;
+  constexpr int plane = N * N;
+  const long long n_r = (long long)plane * N3;
+  const cplx* ucp = u_c + (long long)c * n_r + (long long)z * plane;
+  for (int idx = tid; idx < plane; idx += NTHR) {
+    int x = idx / N, y = idx - x * N;
+    sc[x * PS + y] = ucp[idx];
+  }
+  const int ncb = (nk2 + RW - 1) / RW;            // column batches per band (host guarantees ncb <= NWARP)
+  if (tid < 16) {
+    const int* kf = tid < 8 ? kfreq2 : kfreq1;
+    const int nk = tid < 8 ? nk2 : nk1, s = tid & 7;
+    unsigned long long m = ~0ull;
+    for (int i = 0; i < nk; i++) {
+      const int k = kf[i];
+      if ((k & 7) == s) { const int sh = 8 * (k >> 3); m = (m & ~(0xffull << sh)) | ((unsigned long long)i << sh); }
+    }
+    (tid < 8 ? slot2 : slot1)[s] = m;
+  }
+  if (tid == 32) {
+    for (int b = 0; b < D; b++) { mbar_init(full + b, NWARP); mbar_init(empty + b, ncb); }
+  }
+  const int ls = lane / R2, j = lane - ls * R2;
+  const bool lane_on = lane < RW * R2;
+  const int r0 = warp * RW, row = r0 + ls;
+  const bool row_on = lane_on && row < N;
+  const int nrow = min(RW, N - r0);
+  cplx twj[8];
+#pragma unroll
+  for (int s = 1; s < 8; s++) twj[s] = tw[(j * s) % N];
+  const cplx* uvp = u_v + (long long)z * plane + (long long)row * N + j;
+  cplx nxt[8];
+  if (row_on) {
+#pragma unroll
+    for (int q = 0; q < 8; q++) nxt[q] = uvp[q * R2];
+  }
+  __syncthreads();
+  const long long J = (long long)nk1 * nk2;
+
+  auto cols = [&](int band) {   // this warp's share of the x transforms of `band`, if it has one
+    int k = warp - (int)(((long long)band * ncb) % NWARP);
+    if (k < 0) k += NWARP;
+    if (k >= ncb) return;
+    const int b = band % D;
+    mbar_wait(full + b, (band / D) & 1);
+    cplx* cb = cb0 + b * nk2 * PC;
+    const int l0 = k * RW, nl = min(RW, nk2 - l0);
+    const bool col_on = lane_on && ls < nl;
+    cplx x[8];
+    cplx* line = cb + (l0 + ls) * PC;
+    if (col_on) {
+#pragma unroll
+      for (int q = 0; q < 8; q++) x[q] = line[j + q * R2];
+      fftsm::bfly8<false>(x);
+    }
+    __syncwarp();
+    if (col_on) {
+      line[j] = x[0];
+#pragma unroll
+      for (int s = 1; s < 8; s++) line[s * G + j] = fftsm::cmul(x[s], twj[s]);
+    }
+    __syncwarp();
+    cplx* dstT = T + (((long long)band * ncc + c) * N3 + z) * J;
+    for (int t = lane; t < nl * 8; t += 32) {
+      const int l = l0 + (t >> 3), s = t & 7;
+      const cplx* grp = cb + l * PC + s * G;
+      cplx zz[R2];
+#pragma unroll
+      for (int q = 0; q < R2; q++) zz[q] = grp[q];
+      dft_small<R2>(zz);
+      const unsigned long long sl = slot1[s];
+      cplx* dst = dstT + (long long)l * nk1;
+#pragma unroll
+      for (int s2 = 0; s2 < R2; s2++) {
+        const int i1 = (int)((sl >> (8 * s2)) & 0xff);
+        if (i1 != 0xff) dst[i1] = zz[s2];
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(empty + b);
+  };
+
+  for (int it = 0; it < nvb; it++) {
+    const int b = it % D;
+    if (it >= D) mbar_wait(empty + b, ((it / D) - 1) & 1);   // the x transforms of band it - D have left cb[b]
+    cplx* cb = cb0 + b * nk2 * PC;
+    if (row_on) {
+      cplx x[8];
+#pragma unroll
+      for (int q = 0; q < 8; q++) {
+        cplx a = nxt[q], bb = sc[row * PS + j + q * R2];
+        x[q] = make_double2(a.x * bb.x + a.y * bb.y, a.x * bb.y - a.y * bb.x);   // conj(u_v) u_c
+      }
+      if (it + 1 < nvb) {
+        const cplx* nx = uvp + (long long)(it + 1) * n_r;
+#pragma unroll
+        for (int q = 0; q < 8; q++) nxt[q] = nx[q * R2];
+      }
+      fftsm::bfly8<false>(x);
+      cplx* line = wk + row * PW + j;
+      line[0] = x[0];
+#pragma unroll
+      for (int s = 1; s < 8; s++) line[s * G] = fftsm::cmul(x[s], twj[s]);
+    }
+    __syncwarp();
+    for (int t = lane; t < nrow * 8; t += 32) {
+      const int l = t >> 3, s = t & 7;
+      const cplx* grp = wk + (r0 + l) * PW + s * G;
+      cplx zz[R2];
+#pragma unroll
+      for (int q = 0; q < R2; q++) zz[q] = grp[q];
+      dft_small<R2>(zz);
+      const unsigned long long sl = slot2[s];
+      cplx* dst = cb + r0 + l;
+#pragma unroll
+      for (int s2 = 0; s2 < R2; s2++) {
+        const int i2 = (int)((sl >> (8 * s2)) & 0xff);
+        if (i2 != 0xff) dst[i2 * PC] = zz[s2];
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(full + b);
+    if (it >= 1) cols(it - 1);
+  }
+  cols(nvb - 1);
+}
+
 #define RPA_FFT8_ARGS                                                                                              \
   const cplx *__restrict__ u_v, const cplx *__restrict__ u_c, int nvb, int ncc, int N3, const cplx *__restrict__ tw, \
       const int *__restrict__ kfreq1, const int *__restrict__ kfreq2, int nk1, int nk2, cplx *__restrict__ T
@@ -222,6 +389,10 @@ template <int N>
 __global__ void __launch_bounds__(Geo<N>::NWARP * 32) pair_plane_fft8_kernel_b(RPA_FFT8_ARGS) {
   pair_plane_fft8_body<N>(u_v, u_c, nvb, ncc, N3, tw, kfreq1, kfreq2, nk1, nk2, T);
 }
+template <int N>
+__global__ void __launch_bounds__(Geo<N>::NWARP * 32) pair_plane_fft8_kernel_ring(RPA_FFT8_ARGS) {
+  pair_plane_fft8_ring_body<N>(u_v, u_c, nvb, ncc, N3, tw, kfreq1, kfreq2, nk1, nk2, T);
+}
 #undef RPA_FFT8_ARGS
 
 template <int N>
@@ -230,4 +401,12 @@ size_t smem_bytes(int nk1, int nk2) {
   return ((size_t)N * Geo<N>::PS + (size_t)N * Geo<N>::PW + (size_t)2 * Geo<N>::VB * nk2 * Geo<N>::PC) * sizeof(cplx) + 16 * sizeof(unsigned long long);
 }
 
+}  // namespace fft8
+
+namespace fft8 {
+template <int N>
+size_t smem_bytes_ring(int nk2) {
+  return ((size_t)N * Geo<N>::PS + (size_t)N * Geo<N>::PW + (size_t)RING_D * nk2 * Geo<N>::PC) * sizeof(cplx) +
+         (16 + 2 * RING_D) * sizeof(unsigned long long);
+}
 }  // namespace fft8
