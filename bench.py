@@ -77,7 +77,7 @@ def oracle_sample(inp, n_eig, budget_pairs):
     of the full-workload time (pair stages scaled by pairs_full / pairs_sample, two MTXEL passes)."""
     from oracle import rpa_oracle as orc
     nv, nc = inp.psi_v.shape[0], inp.psi_c.shape[0]
-    sv = max(1, min(nv, 2))
+    sv = max(1, min(nv, max(2, budget_pairs // nc)))
     sc = max(1, min(nc, budget_pairs // sv))
     t0 = time.perf_counter()
     M = orc.mtxel(inp.psi_v[:sv], inp.psi_c[:sc], inp.g_wfn, inp.g_eps, inp.fft)
@@ -148,7 +148,7 @@ def main():
     ap.add_argument("--keep-m", type=int, default=1,
                     help="1 (default): keep all M blocks resident in HBM and skip the second MTXEL pass when they fit in 85 %% of the "
                          "free device memory (the single-block case of PAPER.md:158); 0: always recompute")
-    ap.add_argument("--ref-pairs", type=int, default=600, help="pairs in the oracle's bounded sample")
+    ap.add_argument("--ref-pairs", type=int, default=6000, help="pairs in the oracle's bounded sample (about 10 s of CPU)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -205,7 +205,7 @@ def main():
             return rpa.rpa_energy_sharded(ctx, d["psi_v"], d["psi_c"], d["e_v"], d["e_c"], nvb, n_eig, 0.0, d["omega"], d["weight"],
                                           comm=comm, keep_m=keep_m)
         return rpa.rpa_energy_device(ctx, d["psi_v"], d["psi_c"], d["e_v"], d["e_c"], nvb, n_eig, 0.0, d["omega"], d["weight"],
-                                     keep_m=keep_m)
+                                     keep_m=bool(args.keep_m))   # the library keeps what fits in the workspace it was lent
 
     def step_host():
         if world > 1:   # this rank's inputs from pinned host memory, then the sharded path; E_c read back inside
@@ -213,7 +213,7 @@ def main():
             return rpa.rpa_energy_sharded(ctx, t["psi_v"], t["psi_c"], t["e_v"], t["e_c"], nvb, n_eig, 0.0, t["omega"], t["weight"],
                                           comm=comm, keep_m=keep_m)
         return rpa.rpa_energy_host(ctx, h["psi_v"], h["psi_c"], h["e_v"], h["e_c"], nvb, n_eig, 0.0, h["omega"], h["weight"],
-                                   keep_m=keep_m)
+                                   keep_m=bool(args.keep_m))
 
     def barrier():
         if world > 1:

@@ -91,12 +91,31 @@ int rpa_chi_subspace_freq(rpa_ctx* ctx, const void* M, int nvb, int nc, const do
                           const double* e_c, const void* C, int n_eig, const double* omega, int n_w,
                           int accumulate, void* chi_s);
 
+/* (next-4) Partial occupations, PAPER.md:29, :48-67 eq. 4, :71 eq. 5; reading R21 of DESIGN.md.  The same two
+ * contractions with the pair weight  D_vc(i omega) = max(f_v - f_c, 0) 2 Delta/(Delta^2 + omega^2),  Delta = e_c - e_v:
+ * the "valence" set holds every band with f > 0 and the "conduction" set every band with f < 1, so a partially occupied
+ * band sits in both (the four classes of eq. 4); max(., 0) counts each unordered pair once and gives the pair of a band
+ * with itself weight 0.  f_v dev [nvb], f_c dev [nc], occupations in [0, 1]; f_v = 1, f_c = 0 reproduces
+ * rpa_chi0_static / rpa_chi_subspace_freq.  A pair with Delta = 0 and omega = 0 gets weight 0.                          */
+int rpa_chi0_static_occ(rpa_ctx* ctx, const void* M, int nvb, int nc, const double* e_v, const double* e_c,
+                        const double* f_v, const double* f_c, int accumulate, void* chi0);
+int rpa_chi_subspace_freq_occ(rpa_ctx* ctx, const void* M, int nvb, int nc, const double* e_v, const double* e_c,
+                              const double* f_v, const double* f_c, const void* C, int n_eig, const double* omega,
+                              int n_w, int accumulate, void* chi_s);
+
 /* (a5) E_c, PAPER.md:35 eq. 1, :160, :174; reading R10.
  *   per k: L L^H = 1 - chi_s[k];  t_k = 2 sum_i ln L_ii + Re Tr chi_s[k];  E_c = (1/2 pi) sum_k W_k t_k.
  *   weight dev [n_w] (quadrature weight incl. Jacobian).  e_c host out; per_freq host out [n_w],
  *   optional.  chi_s is not modified.  Synchronises.                                             */
 int rpa_correlation_energy(rpa_ctx* ctx, const void* chi_s, int n_eig, const double* weight, int n_w,
                            double* e_c, double* per_freq);
+
+/* (next-3) eps_s^-1(i omega_k) = (1 - chi_s(i omega_k))^-1 in the subspace, from the same Cholesky factor as E_c -- the
+ * by-product the paper keeps for later GW.  chi_s dev [n_w][n_eig][n_eig] (not modified); eps_inv dev out
+ * [n_w][n_eig][n_eig], Hermitian, both triangles.  Needs rpa_epsilon_inverse_workspace_bytes of workspace.  Synchronises;
+ * RPA_ERR_NOT_POSDEF as for rpa_correlation_energy.                                                                   */
+size_t rpa_epsilon_inverse_workspace_bytes(const rpa_ctx* ctx, int n_eig, int n_w);
+int rpa_epsilon_inverse(rpa_ctx* ctx, const void* chi_s, int n_eig, int n_w, void* eps_inv);
 
 /* Whole path (PAPER.md:139-158 NV-block two-pass loop): for each valence block of nvb bands
  * {a1, a2}; a3; for each block {a1, a4}; a5.  All inputs dev (rpa_energy_device) or host

@@ -113,13 +113,21 @@ def mtxel_convolution(psi_v, psi_c, g_wfn, g_eps) -> np.ndarray:
 # --------------------------------------------------------------------------
 # Step a2 -- CHI_SUM (eq. 6 with :71 eq. 5; north_star step 2)
 # --------------------------------------------------------------------------
-def pair_weights(e_v: np.ndarray, e_c: np.ndarray, omega: float) -> np.ndarray:
-    """D_vc(i omega) = 2 Delta/(Delta^2 + omega^2), Delta = e_c - e_v (reading R6), shape [nv, nc]."""
+def pair_weights(e_v: np.ndarray, e_c: np.ndarray, omega: float, f_v=None, f_c=None) -> np.ndarray:
+    """D_vc(i omega) = 2 Delta/(Delta^2 + omega^2), Delta = e_c - e_v (reading R6), shape [nv, nc].
+
+    With occupations (eq. 4-5, reading R21): times max(f_v - f_c, 0), so that a partially occupied band,
+    which sits in both band sets, meets every other band once and itself with weight 0; a pair with Delta = omega = 0
+    has weight 0."""
     delta = e_c[None, :] - e_v[:, None]
-    return 2.0 * delta / (delta * delta + omega * omega)
+    den = delta * delta + omega * omega
+    d = np.where(den > 0.0, 2.0 * delta / np.where(den > 0.0, den, 1.0), 0.0)
+    if f_v is not None:
+        d = d * np.maximum(np.asarray(f_v)[:, None] - np.asarray(f_c)[None, :], 0.0)
+    return d
 
 
-def chi0(M: np.ndarray, e_v, e_c, vcoul, omega: float = 0.0) -> np.ndarray:
+def chi0(M: np.ndarray, e_v, e_c, vcoul, omega: float = 0.0, f_v=None, f_c=None) -> np.ndarray:
     """chi~0(i omega)[G,G'] = - sum_vc a_vc(G) D_vc(i omega) conj(a_vc(G')), a = v^1/2 M.
 
     PAPER.md:75 eq. 6 (sum over valence / conduction pairs), :71 eq. 5 with
@@ -127,7 +135,7 @@ def chi0(M: np.ndarray, e_v, e_c, vcoul, omega: float = 0.0) -> np.ndarray:
     symmetrised as in north_star step 2.  The pair sum is one matrix product."""
     nv, nc, ng = M.shape
     a = (M * np.sqrt(vcoul)[None, None, :]).reshape(nv * nc, ng)
-    d = pair_weights(np.asarray(e_v), np.asarray(e_c), omega).reshape(nv * nc)
+    d = pair_weights(np.asarray(e_v), np.asarray(e_c), omega, f_v, f_c).reshape(nv * nc)
     return -(a.T * d[None, :]) @ np.conj(a)
 
 
@@ -164,7 +172,7 @@ def subspace_basis(chi0_static: np.ndarray, n_eig: int):
 # --------------------------------------------------------------------------
 # Step a4 -- projected chi_s(i omega) (PAPER.md:84 eq. 7, :88 eq. 8; north_star step 4)
 # --------------------------------------------------------------------------
-def chi_subspace_freq(M, e_v, e_c, vcoul, C: np.ndarray, omegas) -> np.ndarray:
+def chi_subspace_freq(M, e_v, e_c, vcoul, C: np.ndarray, omegas, f_v=None, f_c=None) -> np.ndarray:
     """chi_s(i w_k) = - sum_vc B_vc D_vc(i w_k) B_vc^H,  B_vc = C^H v^1/2 M_vc.
 
     PAPER.md:84 eq. 7 (M_s = M C_s) and :88 eq. 8 (chi_s = M_s^dagger Delta M_s).
@@ -175,7 +183,7 @@ def chi_subspace_freq(M, e_v, e_c, vcoul, C: np.ndarray, omegas) -> np.ndarray:
     b = a @ np.conj(C).T                                          # [P, n_eig]
     out = np.empty((len(omegas), C.shape[0], C.shape[0]), dtype=np.complex128)
     for k, w in enumerate(omegas):
-        d = pair_weights(np.asarray(e_v), np.asarray(e_c), float(w)).reshape(nv * nc)
+        d = pair_weights(np.asarray(e_v), np.asarray(e_c), float(w), f_v, f_c).reshape(nv * nc)
         out[k] = -(b.T * d[None, :]) @ np.conj(b)
     return out
 
@@ -209,6 +217,13 @@ def cholesky_trace_log_term(chi: np.ndarray) -> float:
         for i in range(j + 1, n):
             L[i, j] = (a[i, j] - np.sum(L[i, :j] * np.conj(L[j, :j]))) / L[j, j]
     return float(2.0 * np.sum(np.log(np.diag(L).real)) + np.trace(chi).real)
+
+
+def epsilon_inverse(chis: np.ndarray) -> np.ndarray:
+    """eps_s^-1(i w_k) = (1 - chi_s(i w_k))^-1 for every frequency (the factorisation of eps "also gives
+    eps^-1"), by the library's general inverse.  [n_w, n, n] -> [n_w, n, n]."""
+    n = chis.shape[-1]
+    return np.array([np.linalg.inv(np.eye(n) - 0.5 * (c + c.conj().T)) for c in chis])
 
 
 # --------------------------------------------------------------------------

@@ -5,7 +5,9 @@ from .binding import (RpaContext, RpaError, load_library, library_path, EXPORTED
                       rpa_create, rpa_destroy, rpa_workspace_bytes, rpa_energy_workspace_bytes, rpa_set_workspace,
                       rpa_mtxel, rpa_chi0_static, rpa_subspace_basis, rpa_chi_subspace_freq,
                       rpa_correlation_energy, rpa_energy_device, rpa_energy_host, rpa_fp64_peak, rpa_launch_count,
-                      rpa_profile_begin, rpa_profile_end, PROFILE_CLASSES)
+                      rpa_profile_begin, rpa_profile_end, PROFILE_CLASSES,
+                      rpa_chi0_static_occ, rpa_chi_subspace_freq_occ,
+                      rpa_epsilon_inverse, rpa_epsilon_inverse_workspace_bytes)
 
 from .sharded import shard_range, Comm, rpa_energy_sharded
 
@@ -13,4 +15,6 @@ __all__ = ["shard_range", "Comm", "rpa_energy_sharded", "RpaContext", "RpaError"
            "rpa_create", "rpa_destroy", "rpa_workspace_bytes", "rpa_energy_workspace_bytes", "rpa_set_workspace",
            "rpa_mtxel", "rpa_chi0_static", "rpa_subspace_basis", "rpa_chi_subspace_freq",
            "rpa_correlation_energy", "rpa_energy_device", "rpa_energy_host", "rpa_fp64_peak", "rpa_launch_count",
-           "rpa_profile_begin", "rpa_profile_end", "PROFILE_CLASSES"]
+           "rpa_profile_begin", "rpa_profile_end", "PROFILE_CLASSES",
+           "rpa_chi0_static_occ", "rpa_chi_subspace_freq_occ",
+           "rpa_epsilon_inverse", "rpa_epsilon_inverse_workspace_bytes"]

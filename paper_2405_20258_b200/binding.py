@@ -17,7 +17,8 @@ EXPORTED_SYMBOLS = [
     "rpa_create", "rpa_destroy", "rpa_last_error", "rpa_workspace_bytes", "rpa_energy_workspace_bytes",
     "rpa_set_workspace", "rpa_mtxel", "rpa_chi0_static", "rpa_subspace_basis", "rpa_chi_subspace_freq",
     "rpa_correlation_energy", "rpa_energy_device", "rpa_energy_host", "rpa_fp64_peak", "rpa_launch_count",
-    "rpa_profile_begin", "rpa_profile_end",
+    "rpa_profile_begin", "rpa_profile_end", "rpa_chi0_static_occ", "rpa_chi_subspace_freq_occ",
+    "rpa_epsilon_inverse", "rpa_epsilon_inverse_workspace_bytes",
 ]
 
 
@@ -68,6 +69,14 @@ def load_library(build_if_missing: bool = True):
     lib.rpa_subspace_basis.restype = ci
     lib.rpa_chi_subspace_freq.argtypes = [vp, vp, ci, ci, vp, vp, vp, ci, vp, ci, ci, vp]
     lib.rpa_chi_subspace_freq.restype = ci
+    lib.rpa_chi0_static_occ.argtypes = [vp, vp, ci, ci, vp, vp, vp, vp, ci, vp]
+    lib.rpa_chi0_static_occ.restype = ci
+    lib.rpa_chi_subspace_freq_occ.argtypes = [vp, vp, ci, ci, vp, vp, vp, vp, vp, ci, vp, ci, ci, vp]
+    lib.rpa_chi_subspace_freq_occ.restype = ci
+    lib.rpa_epsilon_inverse.argtypes = [vp, vp, ci, ci, vp]
+    lib.rpa_epsilon_inverse.restype = ci
+    lib.rpa_epsilon_inverse_workspace_bytes.argtypes = [vp, ci, ci]
+    lib.rpa_epsilon_inverse_workspace_bytes.restype = C.c_size_t
     lib.rpa_correlation_energy.argtypes = [vp, vp, ci, vp, ci, pd, pd]
     lib.rpa_correlation_energy.restype = ci
     energy_args = [vp, vp, ci, vp, ci, vp, vp, ci, ci, cd, vp, vp, ci, ci, pd, pd, pd, pd]
@@ -199,6 +208,37 @@ def rpa_chi_subspace_freq(ctx, M, e_v, e_c, Cmat, n_eig, omega, accumulate, chi_
         _dev(e_c, torch.float64), _dev(Cmat, torch.complex128) if Cmat is not None else None, n_eig,
         _dev(omega, torch.float64), omega.shape[0], int(bool(accumulate)), _dev(chi_s, torch.complex128)))
     return chi_s
+
+
+def rpa_chi0_static_occ(ctx, M, e_v, e_c, f_v, f_c, accumulate, chi0):
+    import torch
+    f64, c128 = torch.float64, torch.complex128
+    _check(ctx.handle, load_library().rpa_chi0_static_occ(ctx.handle, _dev(M, c128), e_v.shape[0], e_c.shape[0], _dev(e_v, f64),
+                                                          _dev(e_c, f64), _dev(f_v, f64), _dev(f_c, f64), int(bool(accumulate)),
+                                                          _dev(chi0, c128)))
+    return chi0
+
+
+def rpa_chi_subspace_freq_occ(ctx, M, e_v, e_c, f_v, f_c, Cmat, n_eig, omega, accumulate, chi_s):
+    import torch
+    f64, c128 = torch.float64, torch.complex128
+    _check(ctx.handle, load_library().rpa_chi_subspace_freq_occ(
+        ctx.handle, _dev(M, c128), e_v.shape[0], e_c.shape[0], _dev(e_v, f64), _dev(e_c, f64), _dev(f_v, f64), _dev(f_c, f64),
+        _dev(Cmat, c128) if Cmat is not None else None, n_eig, _dev(omega, f64), omega.shape[0], int(bool(accumulate)),
+        _dev(chi_s, c128)))
+    return chi_s
+
+
+def rpa_epsilon_inverse_workspace_bytes(ctx, n_eig, n_w) -> int:
+    return int(load_library().rpa_epsilon_inverse_workspace_bytes(ctx.handle, n_eig, n_w))
+
+
+def rpa_epsilon_inverse(ctx, chi_s, eps_inv):
+    import torch
+    n_w, n_eig = chi_s.shape[0], chi_s.shape[1]
+    _check(ctx.handle, load_library().rpa_epsilon_inverse(ctx.handle, _dev(chi_s, torch.complex128), n_eig, n_w,
+                                                          _dev(eps_inv, torch.complex128)))
+    return eps_inv
 
 
 def rpa_correlation_energy(ctx, chi_s, n_eig, weight):

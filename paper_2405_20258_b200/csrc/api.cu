@@ -38,10 +38,10 @@ size_t chi_freq_workspace(const rpa_ctx* ctx, int nvb, int nc, int n_eig, int n_
 size_t chi0_static_workspace(int nvb, int nc) { return ws_round((size_t)nvb * nc * sizeof(double)); }
 
 int do_chi0_static(rpa_ctx* ctx, WsAlloc& ws, const cplx* M, int nvb, int nc, const double* e_v, const double* e_c,
-                   int accumulate, cplx* chi0) {
+                   int accumulate, cplx* chi0, const double* f_v = nullptr, const double* f_c = nullptr) {
   double* wk = ws.get<double>((size_t)nvb * nc);
   if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_chi0_static: workspace too small (need %zu bytes)", ws.off);
-  int rc = pair_weights(ctx, e_v, e_c, nvb, nc, nullptr, 1, wk);   // D_vc(0) = 2/Delta_vc  (eq. 5)
+  int rc = pair_weights(ctx, e_v, e_c, nvb, nc, nullptr, 1, wk, f_v, f_c);   // D_vc(0) = 2/Delta_vc  (eq. 5)
   if (rc) return rc;
   ZgemmParams g;
   g.A = M; g.lda = ctx->n_g; g.a_km = true; g.B = M; g.ldb = ctx->n_g; g.b_kn = true;
@@ -54,12 +54,13 @@ int do_chi0_static(rpa_ctx* ctx, WsAlloc& ws, const cplx* M, int nvb, int nc, co
 }
 
 int do_chi_freq(rpa_ctx* ctx, WsAlloc& ws, const cplx* M, int nvb, int nc, const double* e_v, const double* e_c, const cplx* C,
-                int n_eig, const double* omega, int n_w, int accumulate, cplx* chi_s) {
+                int n_eig, const double* omega, int n_w, int accumulate, cplx* chi_s, const double* f_v = nullptr,
+                const double* f_c = nullptr) {
   const int n_g = ctx->n_g;
   const long long Pall = (long long)nvb * nc;
   double* wk = ws.get<double>((size_t)n_w * Pall);   // D_vc(i omega_k) for the whole block, [k][v * nc + c]
   if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_chi_subspace_freq: workspace too small (need %zu bytes)", ws.off);
-  int rc = pair_weights(ctx, e_v, e_c, nvb, nc, omega, n_w, wk);
+  int rc = pair_weights(ctx, e_v, e_c, nvb, nc, omega, n_w, wk, f_v, f_c);
   if (rc) return rc;
   if (!C) {  // full basis: chi~0(i w_k) directly from M
     ZgemmParams g;
@@ -254,6 +255,32 @@ int rpa_chi_subspace_freq(rpa_ctx* ctx, const void* M, int nvb, int nc, const do
   return do_chi_freq(ctx, ws, (const cplx*)M, nvb, nc, e_v, e_c, (const cplx*)C, n_eig, omega, n_w, accumulate, (cplx*)chi_s);
 }
 
+int rpa_chi0_static_occ(rpa_ctx* ctx, const void* M, int nvb, int nc, const double* e_v, const double* e_c, const double* f_v,
+                        const double* f_c, int accumulate, void* chi0) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  if (!M || !e_v || !e_c || !f_v || !f_c || !chi0 || nvb < 1 || nc < 1)
+    return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_chi0_static_occ: invalid argument");
+  if ((long long)nvb * nc > 2147483647LL) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_chi0_static_occ: too many pairs");
+  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
+  WsAlloc ws(ctx->ws, ctx->ws_bytes);
+  return do_chi0_static(ctx, ws, (const cplx*)M, nvb, nc, e_v, e_c, accumulate, (cplx*)chi0, f_v, f_c);
+}
+
+int rpa_chi_subspace_freq_occ(rpa_ctx* ctx, const void* M, int nvb, int nc, const double* e_v, const double* e_c, const double* f_v,
+                              const double* f_c, const void* C, int n_eig, const double* omega, int n_w, int accumulate,
+                              void* chi_s) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  if (!M || !e_v || !e_c || !f_v || !f_c || !omega || !chi_s || nvb < 1 || nc < 1 || n_w < 1)
+    return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_chi_subspace_freq_occ: invalid argument");
+  if (n_eig < 1 || n_eig > ctx->n_g || (!C && n_eig != ctx->n_g))
+    return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_chi_subspace_freq_occ: n_eig = %d invalid (n_g = %d)", n_eig, ctx->n_g);
+  if ((long long)nvb * nc > 2147483647LL) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_chi_subspace_freq_occ: too many pairs");
+  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
+  WsAlloc ws(ctx->ws, ctx->ws_bytes);
+  return do_chi_freq(ctx, ws, (const cplx*)M, nvb, nc, e_v, e_c, (const cplx*)C, n_eig, omega, n_w, accumulate, (cplx*)chi_s, f_v,
+                     f_c);
+}
+
 int rpa_correlation_energy(rpa_ctx* ctx, const void* chi_s, int n_eig, const double* weight, int n_w, double* e_c,
                            double* per_freq) {
   if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
@@ -261,6 +288,19 @@ int rpa_correlation_energy(rpa_ctx* ctx, const void* chi_s, int n_eig, const dou
   RPA_CUDA(ctx, cudaSetDevice(ctx->device));
   WsAlloc ws(ctx->ws, ctx->ws_bytes);
   return energy_run(ctx, ws, (const cplx*)chi_s, n_eig, weight, n_w, e_c, per_freq);
+}
+
+size_t rpa_epsilon_inverse_workspace_bytes(const rpa_ctx* ctx, int n_eig, int n_w) {
+  if (!ctx || n_eig < 1 || n_w < 1) return 0;
+  return epsinv_workspace_bytes(ctx, n_eig, n_w) + 4096;
+}
+
+int rpa_epsilon_inverse(rpa_ctx* ctx, const void* chi_s, int n_eig, int n_w, void* eps_inv) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  if (!chi_s || !eps_inv || n_eig < 1 || n_w < 1) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_epsilon_inverse: invalid argument");
+  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
+  WsAlloc ws(ctx->ws, ctx->ws_bytes);
+  return epsinv_run(ctx, ws, (const cplx*)chi_s, n_eig, n_w, (cplx*)eps_inv);
 }
 
 int rpa_fp64_peak(rpa_ctx* ctx, int kind, int iters, double* tflops) {

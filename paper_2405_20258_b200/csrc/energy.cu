@@ -46,6 +46,18 @@ __global__ void quadrature_kernel(const double* __restrict__ t, const double* __
   }
 }
 
+// X[k] = identity (n x n) for every matrix of the batch
+__global__ void identity_kernel(cplx* __restrict__ X, int n, long long total) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+    const long long r = i % ((long long)n * n);
+    X[i] = make_double2((r / n) == (r % n) ? 1.0 : 0.0, 0.0);
+  }
+}
+__global__ void conj_kernel(cplx* __restrict__ X, long long total) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x)
+    X[i].y = -X[i].y;
+}
+
 }  // namespace
 
 size_t energy_workspace_bytes(const rpa_ctx* ctx, int n_eig, int n_w) {
@@ -81,5 +93,43 @@ int energy_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi_s, int n_eig, const do
   *e_c = th[n_w];
   if (per_freq)
     for (int k = 0; k < n_w; k++) per_freq[k] = th[k];
+  return RPA_OK;
+}
+
+// (next-3) eps_s^-1(i w_k) = (1 - chi_s(i w_k))^-1 from the same Cholesky factor as E_c (the factorisation
+// "also gives eps^-1", kept for GW):  1 - chi_s = L L^H  =>  eps^-1 = L^-H L^-1 = X^H X with X = L^-1.
+size_t epsinv_workspace_bytes(const rpa_ctx* ctx, int n_eig, int n_w) {
+  (void)ctx;
+  return 2 * ws_round((size_t)n_w * n_eig * n_eig * sizeof(cplx)) + ws_round((size_t)n_w * n_eig * sizeof(double)) + ws_round((size_t)(n_w + 1) * sizeof(int)) + 256;
+}
+
+int epsinv_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi_s, int n, int n_w, cplx* eps_inv) {
+  const long long nn = (long long)n * n;
+  cplx* W = ws.get<cplx>((size_t)n_w * nn);
+  cplx* X = ws.get<cplx>((size_t)n_w * nn);
+  double* dvec = ws.get<double>((size_t)n_w * n);
+  int* info = ws.get<int>(n_w + 1);
+  if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_epsilon_inverse: workspace too small (need %zu bytes)", ws.off);
+  negate_kernel<<<ctx->sm_count * 8, 256, 0, ctx->stream>>>(chi_s, n_w * nn, W);
+  RPA_LAUNCH_CHECK(ctx);
+  int rc = zpotrf_batched(ctx, W, n, n, n_w, nn, info, 1, dvec);
+  if (rc) return rc;
+  identity_kernel<<<ctx->sm_count * 8, 256, 0, ctx->stream>>>(X, n, n_w * nn);
+  RPA_LAUNCH_CHECK(ctx);
+  for (int k = 0; k < n_w; k++)
+    if ((rc = ztrsm_left_lower(ctx, W + k * nn, n, n, X + k * nn, n, n))) return rc;
+  ZgemmParams g;   // R[m][n'] = sum_k X[k][m] conj(X[k][n']) = conj((X^H X)[m][n'])
+  g.A = X; g.lda = n; g.a_km = true; g.B = X; g.ldb = n; g.b_kn = true; g.C = eps_inv; g.ldc = n;
+  g.M = n; g.N = n; g.K = n; g.conj_b = true; g.herm = true;
+  g.batch = n_w; g.strideA = nn; g.strideB = nn; g.strideC = nn;
+  if ((rc = zgemm_dmma(ctx, g))) return rc;
+  conj_kernel<<<ctx->sm_count * 8, 256, 0, ctx->stream>>>(eps_inv, n_w * nn);
+  RPA_LAUNCH_CHECK(ctx);
+  std::vector<int> ih(n_w);
+  RPA_CUDA(ctx, cudaMemcpyAsync(ih.data(), info, n_w * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+  RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  for (int k = 0; k < n_w; k++)
+    if (ih[k] != 0)
+      return rpa_fail(ctx, RPA_ERR_NOT_POSDEF, "1 - chi_s(i w_%d) is not positive definite (pivot %d)", k, ih[k]);
   return RPA_OK;
 }

@@ -123,7 +123,8 @@ struct ZgemmParams {
 int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p);
 // out[k][v * nc + c] = 2 D/(D^2 + omega_k^2), D = e_c[c] - e_v[v]  (eq. 5 in the reading R6); omega == nullptr: one
 // row with omega = 0
-int pair_weights(rpa_ctx* ctx, const double* e_v, const double* e_c, int nvb, int nc, const double* omega, int n_w, double* out);
+int pair_weights(rpa_ctx* ctx, const double* e_v, const double* e_c, int nvb, int nc, const double* omega, int n_w, double* out,
+                 const double* f_v = nullptr, const double* f_c = nullptr);   // f given: times max(f_v - f_c, 0)
 int fp64_peak_kernel(rpa_ctx* ctx, int kind, int iters, double* tflops);
 
 // mtxel.cu
@@ -141,6 +142,9 @@ int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, dou
 size_t energy_workspace_bytes(const rpa_ctx* ctx, int n_eig, int n_w);
 int energy_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi_s, int n_eig, const double* weight, int n_w, double* e_c,
                double* per_freq);
+
+size_t epsinv_workspace_bytes(const rpa_ctx* ctx, int n_eig, int n_w);
+int epsinv_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi_s, int n_eig, int n_w, cplx* eps_inv);
 
 // chol.cu
 int zpotrf_batched(rpa_ctx* ctx, cplx* A, int n, long long lda, int batch, long long stride, int* d_info, int shift = 0,

@@ -319,21 +319,26 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
 
 namespace {
 __global__ void pair_weights_kernel(const double* __restrict__ e_v, const double* __restrict__ e_c, int nc, long long P,
-                                    const double* __restrict__ omega, double* __restrict__ out) {
+                                    const double* __restrict__ omega, const double* __restrict__ f_v,
+                                    const double* __restrict__ f_c, double* __restrict__ out) {
   const double w = omega ? omega[blockIdx.y] : 0.0, w2 = w * w;
   double* o = out + blockIdx.y * P;
   for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < P; k += (long long)gridDim.x * blockDim.x) {
     const int v = (int)(k / nc), c = (int)(k - (long long)v * nc);
     const double d = e_c[c] - e_v[v];
-    o[k] = 2.0 * d / (d * d + w2);
+    const double den = d * d + w2;
+    double x = den > 0.0 ? 2.0 * d / den : 0.0;
+    if (f_v) x *= fmax(f_v[v] - f_c[c], 0.0);   // partial occupations (reading R21): every unordered pair once, f_v > f_c
+    o[k] = x;
   }
 }
 }  // namespace
 
-int pair_weights(rpa_ctx* ctx, const double* e_v, const double* e_c, int nvb, int nc, const double* omega, int n_w, double* out) {
+int pair_weights(rpa_ctx* ctx, const double* e_v, const double* e_c, int nvb, int nc, const double* omega, int n_w, double* out,
+                 const double* f_v, const double* f_c) {
   const long long P = (long long)nvb * nc;
   dim3 grid((unsigned)std::min<long long>((P + 255) / 256, 4096), omega ? n_w : 1);
-  pair_weights_kernel<<<grid, 256, 0, ctx->stream>>>(e_v, e_c, nc, P, omega, out);
+  pair_weights_kernel<<<grid, 256, 0, ctx->stream>>>(e_v, e_c, nc, P, omega, f_v, f_c, out);
   RPA_LAUNCH_CHECK(ctx);
   return RPA_OK;
 }

@@ -277,3 +277,49 @@ def test_tiny_config_subspace_error_is_the_methods_own_approximation():
     assert r["E_c_full"] < r["E_c"] < 0
     rel = (r["E_c"] - r["E_c_full"]) / abs(r["E_c_full"])
     assert 0.03 < rel < 0.10
+
+
+# ------------------------------------------------------------------ partial occupations (NEXT-4, reading R21)
+def test_partial_occupations_closed_form_reduction_and_single_counting():
+    """Pins for the occupation-weighted pair weight (eq. 4-5): (a) the single-pair closed form with
+    b = 2 Delta (f_v - f_c) |v^1/2 M|^2; (b) f_v = 1, f_c = 0 is the integer-occupation result; (c) a partially occupied
+    band listed in both band sets meets itself with weight 0 and every other band once (by hand on a 3-band case)."""
+    ng = 5
+    m = RNG.standard_normal(ng) + 1j * RNG.standard_normal(ng)
+    v = RNG.uniform(0.5, 2.0, ng)
+    s = float(np.sum(v * np.abs(m) ** 2))
+    delta, fv, fc = 0.4, 0.85, 0.25
+    omega, weight = quadrature(200, 0.5)
+    M = m.reshape(1, 1, ng)
+    chis = np.array([orc.chi0(M, np.array([-delta]), np.array([0.0]), v, w, np.array([fv]), np.array([fc])) for w in omega])
+    e, _ = orc.correlation_energy(chis, weight)
+    ref = closed_form_pair(delta, 2.0 * delta * (fv - fc) * s)
+    assert abs(e - ref) <= 2e-11 * abs(ref)
+    # (b)
+    Mr = RNG.standard_normal((2, 3, ng)) + 1j * RNG.standard_normal((2, 3, ng))
+    e_v, e_c = np.array([-0.5, -0.2]), np.array([0.1, 0.6, 1.5])
+    a = orc.chi0(Mr, e_v, e_c, v, 0.3)
+    b = orc.chi0(Mr, e_v, e_c, v, 0.3, np.ones(2), np.zeros(3))
+    assert np.array_equal(a, b)
+    # (c) bands: 0 occupied (f = 1), 1 partial (f = 0.4), 2 empty (f = 0); valence set {0, 1}, conduction set {1, 2}
+    e = np.array([-0.5, 0.0, 0.7])
+    f = np.array([1.0, 0.4, 0.0])
+    d = orc.pair_weights(e[[0, 1]], e[[1, 2]], 0.2, f[[0, 1]], f[[1, 2]])
+    by_hand = np.array([[0.6 * 2 * 0.5 / (0.25 + 0.04), 1.0 * 2 * 1.2 / (1.44 + 0.04)],
+                        [0.0, 0.4 * 2 * 0.7 / (0.49 + 0.04)]])
+    assert np.allclose(d, by_hand, rtol=1e-15, atol=0)
+    assert orc.pair_weights(e[[1]], e[[1]], 0.0, f[[1]], f[[1]])[0, 0] == 0.0      # Delta = omega = 0
+
+
+def test_epsilon_inverse_pins():
+    """eps^-1 (NEXT-3): defining identity (1 - chi) eps^-1 = 1, the diagonal case 1/(1 - mu), and Hermiticity."""
+    n = 9
+    a = RNG.standard_normal((n, 4)) + 1j * RNG.standard_normal((n, 4))
+    chi = -(a @ a.conj().T)                                   # Hermitian negative-semidefinite like chi_s
+    mu = -RNG.uniform(0.0, 2.0, n)
+    chis = np.array([chi, np.diag(mu).astype(complex)])
+    inv = orc.epsilon_inverse(chis)
+    assert np.abs((np.eye(n) - chi) @ inv[0] - np.eye(n)).max() <= 1e-13
+    assert np.abs(inv[0] - inv[0].conj().T).max() <= 1e-14
+    assert np.allclose(np.diag(inv[1]).real, 1.0 / (1.0 - mu), rtol=1e-15)
+    assert np.abs(inv[1] - np.diag(np.diag(inv[1]))).max() == 0.0
