@@ -155,21 +155,34 @@ template <bool INV, int MODE>
 __global__ void fft_axis_kernel(cplx* __restrict__ data, Plan pl, long long n_lines, int inner, int TL, ZScatter zs) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx* s = reinterpret_cast<cplx*>(smem_raw);
+  __shared__ long long s_base[64];   // per line of the tile (TL <= 64): element offset of its first element ...
+  __shared__ long long s_row[64];    // ... MODE 1: offset of the M row of its pair
+  __shared__ int s_j[64];            // ... MODE 1: its kept (k_x, k_y) column
   const int n = pl.n, pitch = n | 1;
   const int tid = threadIdx.x, nthr = blockDim.x;
   const long long line0 = (long long)blockIdx.x * TL;
   const int nl = (int)min((long long)TL, n_lines - line0);
+  if (tid < nl) {   // the 64-bit divisions are done once per line, not once per element
+    const long long line = line0 + tid, o = line / inner;
+    const int i = (int)(line - o * inner);
+    s_base[tid] = inner == 1 ? line * n : o * n * inner + i;
+    if (MODE == 1) {
+      const long long v = o / zs.ncc;
+      const int cl = (int)(o - v * zs.ncc);
+      s_row[tid] = (v * zs.nc + zs.c0 + cl) * zs.n_g;
+      s_j[tid] = i;
+    }
+  }
+  __syncthreads();
   if (inner == 1) {
     for (int idx = tid; idx < nl * n; idx += nthr) {
       int l = idx / n, e = idx - l * n;
-      s[l * pitch + e] = data[(line0 + l) * n + e];
+      s[l * pitch + e] = data[s_base[l] + e];
     }
   } else {
     for (int idx = tid; idx < nl * n; idx += nthr) {
       int e = idx / nl, l = idx - e * nl;
-      long long line = line0 + l, o = line / inner;
-      int i = (int)(line - o * inner);
-      s[l * pitch + e] = data[(o * n + e) * inner + i];
+      s[l * pitch + e] = data[s_base[l] + (long long)e * inner];
     }
   }
   __syncthreads();
@@ -178,26 +191,21 @@ __global__ void fft_axis_kernel(cplx* __restrict__ data, Plan pl, long long n_li
     if (inner == 1) {
       for (int idx = tid; idx < nl * n; idx += nthr) {
         int l = idx / n, e = idx - l * n;
-        data[(line0 + l) * n + e] = s[l * pitch + pl.perm[e]];
+        data[s_base[l] + e] = s[l * pitch + pl.perm[e]];
       }
     } else {
       for (int idx = tid; idx < nl * n; idx += nthr) {
         int e = idx / nl, l = idx - e * nl;
-        long long line = line0 + l, o = line / inner;
-        int i = (int)(line - o * inner);
-        data[(o * n + e) * inner + i] = s[l * pitch + pl.perm[e]];
+        data[s_base[l] + (long long)e * inner] = s[l * pitch + pl.perm[e]];
       }
     }
   } else {
     for (int idx = tid; idx < nl * zs.nk3; idx += nthr) {
       int l = idx / zs.nk3, i3 = idx - l * zs.nk3;
-      long long line = line0 + l, pair = line / inner;
-      int j = (int)(line - pair * inner);
-      int g = zs.inv_map[j * zs.nk3 + i3];
+      int g = zs.inv_map[s_j[l] * zs.nk3 + i3];
       if (g >= 0) {
-        long long v = pair / zs.ncc; int cl = (int)(pair - v * zs.ncc);
         cplx x = s[l * pitch + zs.kpos3[i3]];
-        zs.M[(v * zs.nc + zs.c0 + cl) * zs.n_g + g] = make_double2(x.x * zs.scale, x.y * zs.scale);
+        zs.M[s_row[l] + g] = make_double2(x.x * zs.scale, x.y * zs.scale);
       }
     }
   }
