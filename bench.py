@@ -297,6 +297,9 @@ def main():
         "mtxel_z": ("B", passes * P * 16.0 * (nk[0] * nk[1] * n3 + ng)),
         "chi0": ("FLOP", work["chi0_flops"]), "proj": ("FLOP", work["proj_flops"]), "chis": ("FLOP", work["chis_flops"]),
     }
+    jn, jsweeps, jkind = rpa.rpa_basis_info(ctx)
+    if jn > 0:   # direct Jacobi of chi~0(0): vector form = FP64 ALU work, block form = DMMA GEMM work
+        kwork["basis"] = ("FLOP", jsweeps * 32.0 * jn ** 3) if jkind == 1 else ("ALU", jsweeps * 0.5 * jn * (jn - 1) * 44.0 * jn)
     kernels = {}
     for k, (kms, kn) in kprof.items():
         ent = {"ms_per_step": kms / args.steps, "launches_per_step": kn / args.steps}
@@ -304,6 +307,7 @@ def main():
             unit, w = kwork[k]
             rate = w / (kms / args.steps * 1e-3)
             ent.update({"GBps": rate / 1e9, "frac_of_hbm": rate / 1e9 / hbm_peak} if unit == "B" else
+                       {"TFLOPs": rate / 1e12, "frac_of_dfma_peak": rate / 1e12 / dfma_peak} if unit == "ALU" else
                        {"TFLOPs": rate / 1e12, "frac_of_dmma_peak": rate / 1e12 / dmma_peak})
         kernels[k] = ent
     traffic_tab = {}
@@ -316,7 +320,9 @@ def main():
     names = {"mtxel_plane": "pair_plane_fft8_kernel (MTXEL a1: pair product + pruned xy transforms)",
              "mtxel_z": "fft_axis_kernel<false,1> (MTXEL a1: z transform + sphere gather)",
              "chi0": "zgemm_dmma_kernel<1,1,1,3> (CHI_SUM a2)", "proj": "zgemm_dmma_kernel<0,0,1,2> (projection a4)",
-             "chis": "zgemm_dmma_kernel<1,1,1,3> batched over omega (chi_s a4)"}
+             "chis": "zgemm_dmma_kernel<1,1,1,3> batched over omega (chi_s a4)",
+             "basis": "jacobi_persistent_kernel (a3: one-sided Jacobi of chi~0(0), all sweeps in one cooperative launch)" if jkind == 0
+             else "block Jacobi of chi~0(0) (a3: batched zgemm_dmma Gram + pair_rotations_kernel + batched zgemm_dmma update)"}
     tr = traffic_tab.get(f"{dom}:cfg{args.config}")
     if kwork[dom][0] == "B":
         per_launch = kwork[dom][1] / max(1.0, kd["launches_per_step"])
@@ -325,6 +331,15 @@ def main():
                     "frac": per_launch / avg_s / 1e9 / hbm_peak, "traffic": tr, "peak_source": hbm_src,
                     "algorithmic_bytes_per_launch": per_launch, "avg_launch_ms": avg_s * 1e3,
                     "bytes_model": "16 B x (N_r + nk_x nk_y N_z) per (v,c) pair in the launch (DESIGN.md 5.2)",
+                    "share_of_step": kd["ms_per_step"] / ms_per_step}
+    elif kwork[dom][0] == "ALU":
+        avg_s = kd["ms_per_step"] * 1e-3
+        roofline = {"kernel": names[dom], "bound": "alu", "achieved": kwork[dom][1] / avg_s / 1e12, "peak": dfma_peak, "unit": "TFLOP/s",
+                    "frac": kwork[dom][1] / avg_s / 1e12 / dfma_peak, "traffic": tr,
+                    "peak_source": "FP64 FMA register-only microbenchmark measured in this run (rpa_fp64_peak kind 1)",
+                    "algorithmic_flops_per_launch": kwork[dom][1], "avg_launch_ms": avg_s * 1e3,
+                    "flops_model": f"{jsweeps} sweeps x n(n-1)/2 pairs x 44 n FLOP (16 n for the three dot products, 28 n for the "
+                                   f"rotation), n = {jn}; the kernel is bound by the grid-wide barrier per round, not by the ALUs",
                     "share_of_step": kd["ms_per_step"] / ms_per_step}
     else:
         per_launch = kwork[dom][1] / max(1.0, kd["launches_per_step"])

@@ -148,6 +148,10 @@ enum { RPA_PROF_MTXEL_PLANE = 0, RPA_PROF_MTXEL_Z = 1, RPA_PROF_MTXEL_WFN = 2, R
        RPA_PROF_CHIS = 5, RPA_PROF_BASIS = 6, RPA_PROF_ENERGY = 7, RPA_PROF_NCLASS = 8 };
 int rpa_profile_begin(rpa_ctx* ctx);
 int rpa_profile_end(rpa_ctx* ctx, double* ms, long long* launches);
+/* The last Jacobi eigen-decomposition run by the basis stage (for bench.py's work model): matrix size, sweeps done,
+ * kind 0 = vector one-sided Jacobi (44 n FLOP per rotated pair, n(n-1)/2 pairs per sweep), 1 = block Jacobi (32 n^3
+ * GEMM FLOP per sweep).  Host out.                                                                                 */
+int rpa_basis_info(const rpa_ctx* ctx, int* n, int* sweeps, int* kind);
 /* Number of kernels launched by this context since creation (for bench.py's gpu_launches). */
 long long rpa_launch_count(const rpa_ctx* ctx);
 

@@ -18,7 +18,7 @@ EXPORTED_SYMBOLS = [
     "rpa_set_workspace", "rpa_mtxel", "rpa_chi0_static", "rpa_subspace_basis", "rpa_chi_subspace_freq",
     "rpa_correlation_energy", "rpa_energy_device", "rpa_energy_host", "rpa_fp64_peak", "rpa_launch_count",
     "rpa_profile_begin", "rpa_profile_end", "rpa_chi0_static_occ", "rpa_chi_subspace_freq_occ",
-    "rpa_epsilon_inverse", "rpa_epsilon_inverse_workspace_bytes",
+    "rpa_epsilon_inverse", "rpa_epsilon_inverse_workspace_bytes", "rpa_basis_info",
 ]
 
 
@@ -90,6 +90,8 @@ def load_library(build_if_missing: bool = True):
     lib.rpa_profile_begin.restype = ci
     lib.rpa_profile_end.argtypes = [vp, pd, C.POINTER(C.c_longlong)]
     lib.rpa_profile_end.restype = ci
+    lib.rpa_basis_info.argtypes = [vp, pi, pi, pi]
+    lib.rpa_basis_info.restype = ci
     lib.rpa_launch_count.argtypes = [vp]
     lib.rpa_launch_count.restype = C.c_longlong
     _LIB = lib
@@ -309,3 +311,10 @@ def rpa_profile_end(ctx):
     cnt = (C.c_longlong * n)()
     _check(ctx.handle, load_library().rpa_profile_end(ctx.handle, ms, cnt))
     return {k: (ms[i], int(cnt[i])) for i, k in enumerate(PROFILE_CLASSES)}
+
+
+def rpa_basis_info(ctx):
+    """(n, sweeps, kind) of the last Jacobi eigen-decomposition of the basis stage (kind 0 vector, 1 block)."""
+    n, sw, kind = C.c_int(0), C.c_int(0), C.c_int(0)
+    _check(ctx.handle, load_library().rpa_basis_info(ctx.handle, C.byref(n), C.byref(sw), C.byref(kind)))
+    return n.value, sw.value, kind.value

@@ -172,6 +172,12 @@ const char* rpa_last_error(const rpa_ctx* ctx) { return ctx ? ctx->err.c_str() :
 
 long long rpa_launch_count(const rpa_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
+int rpa_basis_info(const rpa_ctx* ctx, int* n, int* sweeps, int* kind) {
+  if (!ctx || !n || !sweeps || !kind) return RPA_ERR_INVALID;
+  *n = ctx->jac_n; *sweeps = ctx->jac_sweeps; *kind = ctx->jac_kind;
+  return RPA_OK;
+}
+
 int rpa_profile_begin(rpa_ctx* ctx) {
   if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
   for (auto& r : ctx->prof_recs) { ctx->prof_pool.push_back(r.a); ctx->prof_pool.push_back(r.b); }

@@ -38,6 +38,9 @@ struct rpa_ctx {
   // array uc_cache_src, [uc_cache_rows][n_r]
   cplx* uc_cache = nullptr; const cplx* uc_cache_src = nullptr; int uc_cache_nc = 0, uc_cache_rows = 0; bool uc_cache_filled = false;
 
+  // last direct Jacobi eigen-decomposition of the basis stage: matrix size, sweeps, 0 = vector iteration / 1 = block
+  int jac_n = 0, jac_sweeps = 0, jac_kind = 0;
+
   // per-kernel-class device timers (rpa_profile_begin / rpa_profile_end): event pairs around the launches of a class
   bool prof = false;
   struct ProfRec { int cls; cudaEvent_t a, b; };
