@@ -15,6 +15,7 @@
 
 #include "fft_smem.cuh"
 #include "pair_plane_fft8.cuh"
+#include "z_fft8.cuh"
 #include "rpa_internal.h"
 
 using fftsm::Plan;
@@ -28,6 +29,7 @@ struct AxisPlan {
   int nk = 0;            // number of distinct epsilon-sphere Miller indices on this axis
   int* d_kpos = nullptr; // [nk] position (after the in-place passes) of each kept frequency
   int* d_kfreq = nullptr; // [nk] the kept frequencies themselves, in 0..n-1
+  int max_res8 = 0;       // largest number of kept frequencies in one residue class mod 8
   Plan fwd() const { Plan p; p.n = n; p.n_pass = n_pass; for (int i = 0; i < n_pass; i++) p.radix[i] = radix[i]; p.tw = d_tw_fwd; p.perm = d_perm; return p; }
   Plan inv() const { Plan p = fwd(); p.tw = d_tw_inv; return p; }
 };
@@ -88,6 +90,7 @@ int mtxel_plan_create(rpa_ctx* ctx, const int32_t* g_eps, const int32_t* g_wfn) 
     std::vector<int> kpos(ap.nk);
     std::vector<int> kfreq(ap.nk);
     for (int i = 0; i < ap.nk; i++) { kfreq[i] = ((kidx[a][i] % n) + n) % n; kpos[i] = perm[kfreq[i]]; }
+    { int cnt[8] = {0}; for (int i = 0; i < ap.nk; i++) ap.max_res8 = std::max(ap.max_res8, ++cnt[kfreq[i] & 7]); }
     int rc;
     if ((rc = upload(ctx, (void**)&ap.d_tw_fwd, twf.data(), n * sizeof(cplx)))) return rc;
     if ((rc = upload(ctx, (void**)&ap.d_tw_inv, twi.data(), n * sizeof(cplx)))) return rc;
@@ -487,7 +490,37 @@ int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx*
     ZScatter zs;
     zs.kpos3 = mp->ax[2].d_kpos; zs.nk3 = nk3; zs.inv_map = mp->d_inv_map; zs.M = M;
     zs.ncc = ncc; zs.nc = nc; zs.c0 = c0; zs.n_g = ctx->n_g; zs.scale = 1.0 / (double)n_r;
-    { ProfScope ps(ctx, RPA_PROF_MTXEL_Z); rc = launch_axis<false, 1>(ctx, T, mp->ax[2].fwd(), (long long)nvb * ncc * J, J, zs); }
+    {
+      ProfScope ps(ctx, RPA_PROF_MTXEL_Z);
+      const long long n_lines = (long long)nvb * ncc * J;
+      const bool z8 = !ctx->force_generic_fft && (N3 == 40 || N3 == 120 || N3 == 160) && mp->ax[2].max_res8 <= zfft8::MAXO &&
+                      (n_lines + 31) / 32 <= 2147483647LL;
+      if (z8) {
+        zfft8::Args za;
+        za.T = T; za.n_lines = n_lines; za.J = J; za.tw = mp->ax[2].d_tw_fwd; za.kfreq3 = mp->ax[2].d_kfreq; za.nk3 = nk3;
+        za.inv_map = mp->d_inv_map; za.M = M; za.ncc = ncc; za.nc = nc; za.c0 = c0; za.n_g = ctx->n_g; za.scale = zs.scale;
+        static bool zattr = false;
+        static int per_sm[3] = {0, 0, 0};   // resident CTAs per SM of the three instantiations (persistent grid)
+        if (!zattr) {
+          RPA_CUDA(ctx, cudaFuncSetAttribute(zfft8::z_fft8_scatter_kernel<40>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zfft8::smem_bytes<40>()));
+          RPA_CUDA(ctx, cudaFuncSetAttribute(zfft8::z_fft8_scatter_kernel<120>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zfft8::smem_bytes<120>()));
+          RPA_CUDA(ctx, cudaFuncSetAttribute(zfft8::z_fft8_scatter_kernel<160>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zfft8::smem_bytes<160>()));
+          cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[0], zfft8::z_fft8_scatter_kernel<40>, 32 * 5, zfft8::smem_bytes<40>());
+          cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[1], zfft8::z_fft8_scatter_kernel<120>, 32 * 15, zfft8::smem_bytes<120>());
+          cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[2], zfft8::z_fft8_scatter_kernel<160>, 32 * 20, zfft8::smem_bytes<160>());
+          zattr = true;
+        }
+        const int occ = std::max(1, per_sm[N3 == 40 ? 0 : (N3 == 120 ? 1 : 2)]);
+        const unsigned zb = (unsigned)std::min<long long>((n_lines + 31) / 32, (long long)ctx->sm_count * occ);
+        if (N3 == 40) zfft8::z_fft8_scatter_kernel<40><<<zb, 32 * 5, zfft8::smem_bytes<40>(), ctx->stream>>>(za);
+        else if (N3 == 120) zfft8::z_fft8_scatter_kernel<120><<<zb, 32 * 15, zfft8::smem_bytes<120>(), ctx->stream>>>(za);
+        else zfft8::z_fft8_scatter_kernel<160><<<zb, 32 * 20, zfft8::smem_bytes<160>(), ctx->stream>>>(za);
+        RPA_LAUNCH_CHECK(ctx);
+        rc = RPA_OK;
+      } else {
+        rc = launch_axis<false, 1>(ctx, T, mp->ax[2].fwd(), n_lines, J, zs);
+      }
+    }
     if (rc) return rc;
   }
   if (ctx->uc_cache && ctx->uc_cache_src == psi_c && ctx->uc_cache_nc == nc) ctx->uc_cache_filled = true;
