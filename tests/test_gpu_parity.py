@@ -568,3 +568,48 @@ def test_large_twin_against_golden():
         assert eig_rel(r["lam"], np.array(g["lam"])) <= TOL_LAM
     finally:
         rpa.rpa_destroy(ctx)
+
+
+def test_phase_invariance_and_degenerate_sizes():
+    """P12 on the GPU path: psi_n -> e^{i theta_n} psi_n leaves chi~0 and E_c unchanged (fixes the conjugation conventions
+    of R7 end to end); and the degenerate sizes of every stage call: one valence band, one conduction band, N_eig = 1,
+    one frequency."""
+    import paper_2405_20258_b200 as rpa
+    import torch
+    rng = np.random.default_rng(12)
+    inp = make_inputs(0, n_v=3, n_c=17)
+    n_eig = 9
+    ctx = make_ctx(inp, 3, 17, n_eig, len(inp.omega))
+    try:
+        a = run_stages(ctx, inp, n_eig)
+        ph_v = np.exp(2j * np.pi * rng.uniform(size=3))[:, None]
+        ph_c = np.exp(2j * np.pi * rng.uniform(size=17))[:, None]
+        inp2 = dataclasses.replace(inp, psi_v=inp.psi_v * ph_v, psi_c=inp.psi_c * ph_c)
+        b = run_stages(ctx, inp2, n_eig)
+        assert maxnorm_rel(b["chi0"], a["chi0"]) <= 1e-13
+        assert abs(b["E_c"] - a["E_c"]) <= 1e-12 * abs(a["E_c"])
+        assert eig_rel(b["lam"], a["lam"]) <= 1e-11
+        # one pair, one basis vector, one frequency
+        M = torch.empty((1, 1, inp.n_g), dtype=torch.complex128, device="cuda")
+        rpa.rpa_mtxel(ctx, dev(inp.psi_v[:1]), dev(inp.psi_c[:1]), M)
+        Mref = orc.mtxel(inp.psi_v[:1], inp.psi_c[:1], inp.g_wfn, inp.g_eps, inp.fft)
+        assert maxnorm_rel(M.cpu().numpy(), Mref) <= 1e-12
+        chi = torch.empty((inp.n_g, inp.n_g), dtype=torch.complex128, device="cuda")
+        rpa.rpa_chi0_static(ctx, M, dev(inp.e_v[:1]), dev(inp.e_c[:1]), False, chi)
+        ref = orc.chi0(Mref, inp.e_v[:1], inp.e_c[:1], inp.vcoul)
+        assert maxnorm_rel(chi.cpu().numpy(), ref) <= 1e-13
+        Cm = torch.empty((1, inp.n_g), dtype=torch.complex128, device="cuda")
+        lam = torch.empty(1, dtype=torch.float64, device="cuda")
+        rpa.rpa_subspace_basis(ctx, chi, 1, 0.0, Cm, lam)
+        lref, _ = orc.subspace_basis(ref, 1)
+        assert abs(lam.item() - lref[0]) <= TOL_LAM * abs(lref[0])
+        om = dev(np.array([0.3]))
+        chis = torch.empty((1, 1, 1), dtype=torch.complex128, device="cuda")
+        rpa.rpa_chi_subspace_freq(ctx, M, dev(inp.e_v[:1]), dev(inp.e_c[:1]), Cm, 1, om, False, chis)
+        e, t = rpa.rpa_correlation_energy(ctx, chis, 1, dev(np.array([2.0])))
+        mu = chis.cpu().numpy()[0, 0, 0].real                    # rank-one chi: mu = D(0.3)/D(0) * lambda
+        d03 = orc.pair_weights(inp.e_v[:1], inp.e_c[:1], 0.3)[0, 0] / orc.pair_weights(inp.e_v[:1], inp.e_c[:1], 0.0)[0, 0]
+        assert abs(mu - d03 * lref[0]) <= 1e-12 * abs(lref[0])
+        assert abs(e - 2.0 * (np.log1p(-mu) + mu) / (2 * np.pi)) <= 1e-12 * abs(e)
+    finally:
+        rpa.rpa_destroy(ctx)
