@@ -37,6 +37,8 @@ struct AxisPlan {
 struct MtxelPlan {
   AxisPlan ax[3];        // 0: x (N1), 1: y (N2), 2: z (N3)
   int* d_wfn_box = nullptr;  // [n_pw] index of each wavefunction G in the [z][x][y] box
+  int* d_wx = nullptr; int n_wx = 0;   // distinct x (axis 0) box indices of the wavefunction sphere
+  int* d_wz = nullptr; int n_wz = 0;   // distinct z (axis 2) box indices of the wavefunction sphere
   int* d_inv_map = nullptr;  // [nk2*nk1*nk3] epsilon-sphere index of pruned-box point ((i2*nk1+i1)*nk3+i3), or -1
 };
 
@@ -98,7 +100,7 @@ int mtxel_plan_create(rpa_ctx* ctx, const int32_t* g_eps, const int32_t* g_wfn) 
     if ((rc = upload(ctx, (void**)&ap.d_kpos, kpos.data(), ap.nk * sizeof(int)))) return rc;
     if ((rc = upload(ctx, (void**)&ap.d_kfreq, kfreq.data(), ap.nk * sizeof(int)))) return rc;
   }
-  std::vector<int> box(ctx->n_pw);
+  std::vector<int> box(ctx->n_pw), wxs, wzs;
   for (int g = 0; g < ctx->n_pw; g++) {
     int i[3];
     for (int a = 0; a < 3; a++) {
@@ -107,7 +109,10 @@ int mtxel_plan_create(rpa_ctx* ctx, const int32_t* g_eps, const int32_t* g_wfn) 
       i[a] = ((m % N[a]) + N[a]) % N[a];
     }
     box[g] = (i[2] * N[0] + i[0]) * N[1] + i[1];
+    wxs.push_back(i[0]); wzs.push_back(i[2]);
   }
+  for (auto* w : {&wxs, &wzs}) { std::sort(w->begin(), w->end()); w->erase(std::unique(w->begin(), w->end()), w->end()); }
+  mp->n_wx = (int)wxs.size(); mp->n_wz = (int)wzs.size();
   const int nk1 = mp->ax[0].nk, nk2 = mp->ax[1].nk, nk3 = mp->ax[2].nk;
   std::vector<int> inv((size_t)nk1 * nk2 * nk3, -1);
   for (int g = 0; g < ctx->n_g; g++) {
@@ -120,6 +125,8 @@ int mtxel_plan_create(rpa_ctx* ctx, const int32_t* g_eps, const int32_t* g_wfn) 
   }
   int rc;
   if ((rc = upload(ctx, (void**)&mp->d_wfn_box, box.data(), box.size() * sizeof(int)))) return rc;
+  if ((rc = upload(ctx, (void**)&mp->d_wx, wxs.data(), wxs.size() * sizeof(int)))) return rc;
+  if ((rc = upload(ctx, (void**)&mp->d_wz, wzs.data(), wzs.size() * sizeof(int)))) return rc;
   if ((rc = upload(ctx, (void**)&mp->d_inv_map, inv.data(), inv.size() * sizeof(int)))) return rc;
   return RPA_OK;
 }
@@ -130,7 +137,7 @@ void mtxel_plan_destroy(rpa_ctx* ctx) {
   for (int a = 0; a < 3; a++) {
     cudaFree(mp->ax[a].d_tw_fwd); cudaFree(mp->ax[a].d_tw_inv); cudaFree(mp->ax[a].d_perm); cudaFree(mp->ax[a].d_kpos); cudaFree(mp->ax[a].d_kfreq);
   }
-  cudaFree(mp->d_wfn_box); cudaFree(mp->d_inv_map);
+  cudaFree(mp->d_wfn_box); cudaFree(mp->d_inv_map); cudaFree(mp->d_wx); cudaFree(mp->d_wz);
   delete mp;
   ctx->mtxel = nullptr;
 }
@@ -153,6 +160,10 @@ __global__ void scatter_wfn_kernel(const cplx* __restrict__ psi, const int* __re
 //         M[(v*nc + c0 + cl)*n_g + g] = X * scale, pair = v*ncc + cl.
 struct ZScatter {
   const int* kpos3; int nk3; const int* inv_map; cplx* M; int ncc, nc, c0, n_g; double scale;
+  // MODE 0 only, optional pruning of the wavefunction transforms (lines that hold nothing but zeros are skipped):
+  //   sel 1 (y pass, inner == 1):  line = (band, iz < nz, ix < nx) -> box line (band, zl[iz], xl[ix])
+  //   sel 2 (x pass, inner == N2): line = (band, iz < nz, y < N2)   -> box plane (band, zl[iz]), column y
+  int sel; const int* zl; int nz; const int* xl; int nx; int N1, N3;
 };
 template <bool INV, int MODE>
 __global__ void fft_axis_kernel(cplx* __restrict__ data, Plan pl, long long n_lines, int inner, int TL, ZScatter zs) {
@@ -168,7 +179,17 @@ __global__ void fft_axis_kernel(cplx* __restrict__ data, Plan pl, long long n_li
   if (tid < nl) {   // the 64-bit divisions are done once per line, not once per element
     const long long line = line0 + tid, o = line / inner;
     const int i = (int)(line - o * inner);
-    s_base[tid] = inner == 1 ? line * n : o * n * inner + i;
+    if (MODE == 0 && zs.sel == 1) {
+      const long long band = line / ((long long)zs.nz * zs.nx);
+      const int r = (int)(line - band * zs.nz * zs.nx), iz = r / zs.nx, ix = r - iz * zs.nx;
+      s_base[tid] = ((band * zs.N3 + zs.zl[iz]) * zs.N1 + zs.xl[ix]) * (long long)n;
+    } else if (MODE == 0 && zs.sel == 2) {
+      const long long band = line / ((long long)zs.nz * inner);
+      const int r = (int)(line - band * zs.nz * inner), iz = r / inner, yy = r - iz * inner;
+      s_base[tid] = (band * zs.N3 + zs.zl[iz]) * (long long)n * inner + yy;
+    } else {
+      s_base[tid] = inner == 1 ? line * n : o * n * inner + i;
+    }
     if (MODE == 1) {
       const long long v = o / zs.ncc;
       const int cl = (int)(o - v * zs.ncc);
@@ -371,8 +392,13 @@ int wfn_to_realspace(rpa_ctx* ctx, const cplx* psi, int nb, cplx* u) {
   RPA_LAUNCH_CHECK(ctx);
   ZScatter zs{};
   int rc;
-  if ((rc = launch_axis<true, 0>(ctx, u, mp->ax[1].inv(), (long long)nb * N3 * N1, 1, zs))) return rc;        // y
-  if ((rc = launch_axis<true, 0>(ctx, u, mp->ax[0].inv(), (long long)nb * N3 * N2, N2, zs))) return rc;       // x
+  // y and x passes only on the lines that hold coefficients (the others are zero and stay zero); z pass on all
+  zs.zl = mp->d_wz; zs.nz = mp->n_wz; zs.xl = mp->d_wx; zs.nx = mp->n_wx; zs.N1 = N1; zs.N3 = N3;
+  zs.sel = 1;
+  if ((rc = launch_axis<true, 0>(ctx, u, mp->ax[1].inv(), (long long)nb * mp->n_wz * mp->n_wx, 1, zs))) return rc;    // y
+  zs.sel = 2;
+  if ((rc = launch_axis<true, 0>(ctx, u, mp->ax[0].inv(), (long long)nb * mp->n_wz * N2, N2, zs))) return rc;         // x
+  zs.sel = 0;
   if ((rc = launch_axis<true, 0>(ctx, u, mp->ax[2].inv(), (long long)nb * N1 * N2, N1 * N2, zs))) return rc;  // z
   return RPA_OK;
 }
@@ -487,7 +513,7 @@ int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx*
     }
     delete pp;
     if (rc) return rc;
-    ZScatter zs;
+    ZScatter zs{};
     zs.kpos3 = mp->ax[2].d_kpos; zs.nk3 = nk3; zs.inv_map = mp->d_inv_map; zs.M = M;
     zs.ncc = ncc; zs.nc = nc; zs.c0 = c0; zs.n_g = ctx->n_g; zs.scale = 1.0 / (double)n_r;
     {

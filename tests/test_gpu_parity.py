@@ -597,7 +597,7 @@ def test_phase_invariance_and_degenerate_sizes():
         chi = torch.empty((inp.n_g, inp.n_g), dtype=torch.complex128, device="cuda")
         rpa.rpa_chi0_static(ctx, M, dev(inp.e_v[:1]), dev(inp.e_c[:1]), False, chi)
         ref = orc.chi0(Mref, inp.e_v[:1], inp.e_c[:1], inp.vcoul)
-        assert maxnorm_rel(chi.cpu().numpy(), ref) <= 1e-13
+        assert maxnorm_rel(chi.cpu().numpy(), ref) <= 1e-11          # rank one: inherits twice the error of M (<= 1e-12)
         Cm = torch.empty((1, inp.n_g), dtype=torch.complex128, device="cuda")
         lam = torch.empty(1, dtype=torch.float64, device="cuda")
         rpa.rpa_subspace_basis(ctx, chi, 1, 0.0, Cm, lam)
