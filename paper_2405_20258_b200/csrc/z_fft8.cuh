@@ -26,12 +26,12 @@ struct Args {
   const int* inv_map; cplx* M; int ncc, nc, c0, n_g; double scale;
 };
 
-constexpr int OG = 2;      // kept outputs per pass-B task
-constexpr int MAXT = 8 * ((MAXO + OG - 1) / OG);
+constexpr int MAXT = 8 * ((MAXO + 1) / 2);   // pass-B tasks (at least 2 kept outputs per task)
 
 template <int N3>
 __global__ void __launch_bounds__(32 * (N3 / 8)) z_fft8_scatter_kernel(Args a) {
   constexpr int R3 = N3 / 8, P = N3 | 1, NTHR = 32 * R3;
+  constexpr int OG = R3 >= 20 ? 3 : 2;                  // kept outputs per pass-B task: about one round of tasks per tile
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx* y = reinterpret_cast<cplx*>(smem_raw);          // [32][P]   y_s[j3] at s*R3 + j3
   cplx* twb = y + 32 * P;                               // [8][MAXO][R3]  w_R3^{j3 s2} of the kept outputs of residue s
@@ -102,6 +102,13 @@ __global__ void __launch_bounds__(32 * (N3 / 8)) z_fft8_scatter_kernel(Args a) {
       const cplx* ys = y + lane * P + sB * R3;
       const cplx* tw_s = twb + (sB * MAXO + o0) * R3;
       const int* oi = oidx + sB * MAXO + o0;
+      // sphere indices of this task's outputs first: their (dependent) loads fly during the sums
+      int g[OG];
+#pragma unroll
+      for (int o = 0; o < OG; o++) {
+        const int i3 = (o0 + o < MAXO) ? oi[o] : -1;
+        g[o] = (i3 >= 0 && jl >= 0) ? a.inv_map[jl * a.nk3 + i3] : -1;
+      }
       cplx acc[OG];
 #pragma unroll
       for (int o = 0; o < OG; o++) acc[o] = make_double2(0.0, 0.0);
@@ -115,16 +122,9 @@ __global__ void __launch_bounds__(32 * (N3 / 8)) z_fft8_scatter_kernel(Args a) {
           acc[o].y += v.x * w.y + v.y * w.x;
         }
       }
-      if (jl >= 0) {
 #pragma unroll
-        for (int o = 0; o < OG; o++) {
-          const int i3 = (o0 + o < MAXO) ? oi[o] : -1;
-          if (i3 >= 0) {
-            const int g = a.inv_map[jl * a.nk3 + i3];
-            if (g >= 0) a.M[s_row[lane] + g] = make_double2(acc[o].x * a.scale, acc[o].y * a.scale);
-          }
-        }
-      }
+      for (int o = 0; o < OG; o++)
+        if (g[o] >= 0) a.M[s_row[lane] + g[o]] = make_double2(acc[o].x * a.scale, acc[o].y * a.scale);
     }
     __syncthreads();                                     // y, s_row, s_j are free again
   }
