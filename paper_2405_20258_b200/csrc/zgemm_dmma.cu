@@ -121,6 +121,10 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
     }
   };
 
+  // In a diagonal tile of a Hermitian update the warp (wm, wn) = (0, 1) owns rows 0..31 x columns 32..63: all above the
+  // diagonal, mirrored from the lower triangle in the epilogue.  It keeps loading and synchronising but issues no DMMA,
+  // which leaves the FP64 pipe to the other CTA resident on the SM.
+  const bool upper_only = p.herm && tm == tn && wm == 0 && wn == 1;
   double cre[4][4][2], cim[4][4][2];
 #pragma unroll
   for (int i = 0; i < 4; i++)
@@ -142,6 +146,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
       cp_async_commit();
     }
     const int st = it % STAGES;
+    if (upper_only) continue;   // this warp's 32 x 32 block lies strictly above the diagonal of a Hermitian tile: never stored
     const cplx* a_s = sA + st * TA;
     const cplx* b_s = sB + st * TB;
     const double* w_s = sW + st * BK;
