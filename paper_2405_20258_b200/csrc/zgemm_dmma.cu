@@ -125,6 +125,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
   // diagonal, mirrored from the lower triangle in the epilogue.  It keeps loading and synchronising but issues no DMMA,
   // which leaves the FP64 pipe to the other CTA resident on the SM.
   const bool upper_only = p.herm && tm == tn && wm == 0 && wn == 1;
+  const bool diag_warp = p.herm && tm == tn && wm == wn;   // its own diagonal block: fragments with j > i are above the diagonal
   double cre[4][4][2], cim[4][4][2];
 #pragma unroll
   for (int i = 0; i < 4; i++)
@@ -173,6 +174,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
       for (int i = 0; i < 4; i++)
 #pragma unroll
         for (int j = 0; j < 4; j++) {
+          if (diag_warp && j > i) continue;   // 8 x 8 fragment strictly above the diagonal: never stored
           dmma(cre[i][j][0], cre[i][j][1], ar[i], br[j]);
           dmma(cim[i][j][0], cim[i][j][1], ai[i], br[j]);
         }
@@ -180,6 +182,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
       for (int i = 0; i < 4; i++)
 #pragma unroll
         for (int j = 0; j < 4; j++) {
+          if (diag_warp && j > i) continue;
           dmma(cre[i][j][0], cre[i][j][1], CONJ_B ? ai[i] : -ai[i], bi[j]);
           dmma(cim[i][j][0], cim[i][j][1], CONJ_B ? -ar[i] : ar[i], bi[j]);
         }
