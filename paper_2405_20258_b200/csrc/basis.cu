@@ -286,14 +286,16 @@ __global__ void __launch_bounds__(256) pair_rotations_kernel(const cplx* __restr
       if (i > j) { int t = i; i = j; j = t; }
       const double alpha = W[i * JLD + i].x, beta = W[j * JLD + j].x;
       const cplx w = W[i * JLD + j];
-      const double gabs = sqrt(w.x * w.x + w.y * w.y);
+      const double g2 = w.x * w.x + w.y * w.y, ab = alpha * beta;
       double c = 1.0, s = 0.0, ex = 1.0, ey = 0.0;
-      const double den = sqrt(alpha * beta);
-      if (!(alpha <= null2 && beta <= null2) && den > 0.0 && gabs > rot_tol * den) {
-        const double zeta = (beta - alpha) / (2.0 * gabs);
-        const double t = (zeta >= 0.0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
-        c = 1.0 / sqrt(1.0 + t * t); s = c * t;
-        ex = w.x / gabs; ey = w.y / gabs;          // e^{i theta} = W_ij / |W_ij|
+      // rotation parameters with reciprocal square roots only (this chain is the critical path of a round)
+      if (!(alpha <= null2 && beta <= null2) && ab > 0.0 && g2 > rot_tol * rot_tol * ab) {
+        const double rg = rsqrt(g2);                               // 1 / |W_ij|
+        const double zeta = (beta - alpha) * 0.5 * rg;
+        const double z1 = 1.0 + zeta * zeta;
+        const double t = (zeta >= 0.0 ? 1.0 : -1.0) * __drcp_rn(fabs(zeta) + z1 * rsqrt(z1));
+        c = rsqrt(1.0 + t * t); s = c * t;
+        ex = w.x * rg; ey = w.y * rg;                              // e^{i theta} = W_ij / |W_ij|
       }
       rp_[tid] = i; rq_[tid] = j; rc_[tid] = c; rs_[tid] = s; rx_[tid] = ex; ry_[tid] = ey;
     }
