@@ -484,6 +484,11 @@ int jacobi_eigh(rpa_ctx* ctx, const cplx* src, long long ld, int n, bool src_is_
       converged = off <= stop;
     }
     if (verbose) fprintf(stderr, "[rpa] jacobi n=%d with_v=%d stash=%d persistent=%d sweeps=%d\n", n, (int)with_v, (int)stash, (int)persistent, sweep);
+    if (verbose && persistent && !block) {
+      double offh[64];
+      cudaMemcpy(offh, jw.off, sizeof(offh), cudaMemcpyDeviceToHost);
+      for (int k = 0; k < sweep && k < 64; k++) fprintf(stderr, "[rpa]   sweep %d off %.3e\n", k, offh[k]);
+    }
     ctx->jac_n = n; ctx->jac_sweeps = sweep; ctx->jac_kind = block ? 1 : 0;
     if (!converged) return rpa_fail(ctx, RPA_ERR_NO_CONVERGENCE, "one-sided Jacobi did not converge in 60 sweeps (n = %d)", n);
     rayleigh_kernel<<<n_rows, 256, 0, ctx->stream>>>(jw.A, jw.V, n, with_v ? 1 : 0, jw.lam, jw.scale);
