@@ -530,7 +530,7 @@ size_t basis_workspace_bytes(const rpa_ctx* ctx, int n, int n_eig) {
   auto jac = [](size_t m) {   // A, V (padded to whole blocks) and the Gram / rotation matrices of the block iteration
     return 2 * ws_round((m + JB) * m * sizeof(cplx)) + 2 * ws_round(((m + JB) / JP + 1) * JP * JP * sizeof(cplx));
   };
-  if (use_direct(n, n_eig)) return jac(n) + small;
+  if (use_direct(n, n_eig)) return jac(n) + small + tridiag_workspace_bytes(n, n_eig) + ws_round((size_t)n_eig * n_eig * sizeof(cplx));
   const size_t p = block_size(n, n_eig);
   return 3 * ws_round(p * n * sizeof(cplx)) + 2 * ws_round(p * p * sizeof(cplx)) + jac(p) + small;
 }
@@ -558,6 +558,36 @@ int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, dou
     jw.Wb = ws.get<cplx>((size_t)((n + JB) / JP + 1) * JP * JP);
     jw.Ub = ws.get<cplx>((size_t)((n + JB) / JP + 1) * JP * JP);
     if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_subspace_basis: workspace too small (need %zu bytes)", ws.off);
+    if (n >= 32 && n < jacobi_block_min() && 4 * n_eig <= 3 * n && !getenv("RPA_NO_TRIDIAG")) {
+      // small matrix, part of the spectrum: tridiagonalisation + bisection + inverse iteration (tridiag_eig.cu), then a
+      // CholeskyQR2 clean-up of the n_eig vectors; any failure (e.g. a numerically singular Gram matrix because wanted
+      // eigenvalues coincide) falls through to the Jacobi iteration below
+      WsAlloc wt = ws;
+      cplx* S = wt.get<cplx>((size_t)n_eig * n_eig);
+      rc = tridiag_eigh_lowest(ctx, wt, chi0, n, n, n_eig, jw.A, jw.V, C, lambda);
+      if (rc == RPA_ERR_WORKSPACE) return rc;
+      bool ok = rc == RPA_OK && wt.ok;
+      for (int pass = 0; pass < 2 && ok; pass++) {
+        ZgemmParams g;
+        g.A = C; g.lda = n; g.a_km = false; g.B = C; g.ldb = n; g.b_kn = false; g.C = S; g.ldc = n_eig;
+        g.M = n_eig; g.N = n_eig; g.K = n; g.conj_b = true; g.herm = true;
+        if ((rc = zgemm_dmma(ctx, g))) return rc;
+        if ((rc = zpotrf_batched(ctx, S, n_eig, n_eig, 1, 0, d_info))) return rc;
+        int info_h = 0;
+        RPA_CUDA(ctx, cudaMemcpyAsync(&info_h, d_info, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+        RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        if (info_h != 0) { ok = false; break; }
+        if ((rc = ztrsm_left_lower(ctx, S, n_eig, n_eig, C, n, n))) return rc;
+      }
+      if (getenv("RPA_VERBOSE")) fprintf(stderr, "[rpa] tridiagonal eigensolver n=%d n_eig=%d %s\n", n, n_eig, ok ? "ok" : "failed -> Jacobi");
+      if (ok) {
+        ctx->jac_n = n; ctx->jac_sweeps = 0; ctx->jac_kind = 2;
+        RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        if (iters_out) *iters_out = 0;
+        return RPA_OK;
+      }
+      (void)cudaGetLastError();
+    }
     if ((rc = jacobi_eigh(ctx, chi0, n, n, false, n_eig, n_eig < n, jw, order_h, lam_h))) return rc;
     if ((rc = jacobi_vectors(ctx, jw, n, n_eig, C, n))) return rc;
     std::vector<double> ls(n_eig);

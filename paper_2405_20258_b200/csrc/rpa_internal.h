@@ -141,6 +141,11 @@ size_t basis_workspace_bytes(const rpa_ctx* ctx, int n, int n_eig);
 int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, double tol, cplx* C, double* lambda,
               int* iters_out);
 
+// tridiag_eig.cu
+size_t tridiag_workspace_bytes(int n, int n_eig);
+int tridiag_eigh_lowest(rpa_ctx* ctx, WsAlloc& ws, const cplx* H, long long ld, int n, int n_eig, cplx* Abuf, cplx* Vbuf, cplx* C,
+                        double* lambda);
+
 // energy.cu
 size_t energy_workspace_bytes(const rpa_ctx* ctx, int n_eig, int n_w);
 int energy_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi_s, int n_eig, const double* weight, int n_w, double* e_c,

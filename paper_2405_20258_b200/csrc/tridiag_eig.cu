@@ -1,0 +1,302 @@
+// Lowest eigenpairs of a small Hermitian matrix by the classical dense route, all on the device:
+//   (1) Householder tridiagonalisation  H = Q T Q^H  (unblocked, LAPACK zhetd2 'L' arithmetic) in ONE cooperative launch,
+//   (2) the n_eig smallest eigenvalues of the real symmetric tridiagonal T by bisection on the Sturm count,
+//   (3) their eigenvectors by inverse iteration (tridiagonal LU with partial pivoting),
+//   (4) back-transformation  c_i = Q z_i  (reflectors applied in reverse order),
+// followed, in basis.cu, by a CholeskyQR2 clean-up.  Used by the basis stage (a3) for n < 1024, where a
+// Jacobi sweep costs ~n dependent grid-wide rounds; here the only grid-wide dependencies are the 2 (n - 1) of step (1).
+#include <algorithm>
+#include <cooperative_groups.h>
+
+#include "rpa_internal.h"
+
+namespace cg = cooperative_groups;
+
+namespace {
+
+__device__ __forceinline__ double wsum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+// block-wide sums of NV doubles (256 threads), result in every thread
+template <int NV>
+__device__ __forceinline__ void bsum(double (&v)[NV], double* sh /* [NV][8] */) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int k = 0; k < NV; k++) { v[k] = wsum(v[k]); if (lane == 0) sh[k * 8 + warp] = v[k]; }
+  __syncthreads();
+#pragma unroll
+  for (int k = 0; k < NV; k++) { double s = 0.0; for (int w = 0; w < 8; w++) s += sh[k * 8 + w]; v[k] = s; }
+  __syncthreads();
+}
+__device__ __forceinline__ cplx cmulf(cplx a, cplx b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+
+// (1) A: n x n Hermitian, row-major, both triangles (destroyed).  Vh[k][:] = reflector v_k (v_k[j] = 0 for j <= k,
+// v_k[k+1] = 1), tau[k]; T = tridiag(e, d, e).  256 threads per CTA, one warp per matrix row in the two O(m^2) phases.
+__global__ void __launch_bounds__(256) hetrd_kernel(cplx* __restrict__ A, int n, cplx* __restrict__ Vh, cplx* __restrict__ tau,
+                                                    double* __restrict__ d, double* __restrict__ e, cplx* __restrict__ p) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx* v = reinterpret_cast<cplx*>(smem_raw);   // [n]
+  cplx* w = v + n;                               // [n]
+  __shared__ double sh[4 * 8];
+  cg::grid_group grid = cg::this_grid();
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int gw = blockIdx.x * 8 + warp, nw = gridDim.x * 8;
+  for (int k = 0; k + 1 < n; k++) {
+    // ---- reflector of column k (every CTA, redundantly): x_i = A[i][k] = conj(A[k][i]), i > k
+    const cplx* rowk = A + (long long)k * n;
+    double s[1] = {0.0};
+    for (int i = k + 2 + tid; i < n; i += 256) { const cplx x = __ldcg(rowk + i); s[0] += x.x * x.x + x.y * x.y; }
+    bsum<1>(s, sh);
+    const cplx a0 = __ldcg(rowk + k + 1);
+    const double alr = a0.x, ali = -a0.y, xn2 = s[0];
+    cplx t = make_double2(0.0, 0.0), sc = make_double2(0.0, 0.0);
+    double beta = alr;
+    if (xn2 > 0.0 || ali != 0.0) {
+      const double nrm = sqrt(alr * alr + ali * ali + xn2);
+      beta = alr >= 0.0 ? -nrm : nrm;
+      t = make_double2((beta - alr) / beta, -ali / beta);
+      const double dr = alr - beta, di = ali, den = dr * dr + di * di;     // 1 / (alpha - beta)
+      sc = make_double2(dr / den, -di / den);
+    }
+    for (int i = tid; i < n; i += 256) {
+      cplx vi = make_double2(0.0, 0.0);
+      if (i == k + 1) vi = make_double2(1.0, 0.0);
+      else if (i > k + 1) { const cplx x = __ldcg(rowk + i); vi = cmulf(make_double2(x.x, -x.y), sc); }
+      v[i] = vi;
+    }
+    __syncthreads();
+    if (blockIdx.x == 0) {
+      for (int i = tid; i < n; i += 256) Vh[(long long)k * n + i] = v[i];
+      if (tid == 0) { tau[k] = t; e[k] = beta; d[k] = __ldcg(rowk + k).x; }
+    }
+    // ---- p = tau * A22 v  (warp per row)
+    for (int i = k + 1 + gw; i < n; i += nw) {
+      const cplx* ri = A + (long long)i * n;
+      double pr = 0.0, pi = 0.0;
+      for (int j = k + 1 + lane; j < n; j += 32) { const cplx a = __ldcg(ri + j), b = v[j]; pr += a.x * b.x - a.y * b.y; pi += a.x * b.y + a.y * b.x; }
+      pr = wsum(pr); pi = wsum(pi);
+      if (lane == 0) p[i] = cmulf(t, make_double2(pr, pi));
+    }
+    grid.sync();
+    // ---- w = p - (tau/2) (p^H v) v  (every CTA, redundantly)
+    double q[2] = {0.0, 0.0};
+    for (int i = k + 1 + tid; i < n; i += 256) { const cplx x = __ldcg(p + i), b = v[i]; q[0] += x.x * b.x + x.y * b.y; q[1] += x.x * b.y - x.y * b.x; }
+    bsum<2>(q, sh);
+    const cplx al2 = cmulf(make_double2(-0.5 * t.x, -0.5 * t.y), make_double2(q[0], q[1]));
+    for (int i = k + 1 + tid; i < n; i += 256) { const cplx x = __ldcg(p + i), av = cmulf(al2, v[i]); w[i] = make_double2(x.x + av.x, x.y + av.y); }
+    __syncthreads();
+    // ---- A22 -= v w^H + w v^H  (warp per row)
+    if (t.x != 0.0 || t.y != 0.0) {
+      for (int i = k + 1 + gw; i < n; i += nw) {
+        cplx* ri = A + (long long)i * n;
+        const cplx vi = v[i], wi = w[i];
+        for (int j = k + 1 + lane; j < n; j += 32) {
+          const cplx vj = v[j], wj = w[j];
+          cplx a = __ldcg(ri + j);
+          a.x -= vi.x * wj.x + vi.y * wj.y + wi.x * vj.x + wi.y * vj.y;      // v_i conj(w_j) + w_i conj(v_j)
+          a.y -= vi.y * wj.x - vi.x * wj.y + wi.y * vj.x - wi.x * vj.y;
+          __stcg(ri + j, a);
+        }
+      }
+    }
+    grid.sync();
+  }
+  if (blockIdx.x == 0 && tid == 0) { d[n - 1] = __ldcg(A + (long long)(n - 1) * n + (n - 1)).x; e[n - 1] = 0.0; }
+}
+
+}  // namespace
+
+namespace {
+
+// (2) lam[i] = i-th smallest eigenvalue of T, i < n_eig: bisection on the Sturm count (one thread per eigenvalue)
+__global__ void __launch_bounds__(128) bisect_kernel(const double* __restrict__ d, const double* __restrict__ e, int n, int n_eig,
+                                                     double* __restrict__ lam, double* __restrict__ tnorm) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double* sd = reinterpret_cast<double*>(smem_raw);   // [n]
+  double* se2 = sd + n;                               // [n] e_j^2
+  __shared__ double s_gl, s_gu, s_piv;
+  for (int j = threadIdx.x; j < n; j += blockDim.x) { sd[j] = d[j]; const double x = j + 1 < n ? e[j] : 0.0; se2[j] = x * x; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double gl = sd[0], gu = sd[0], emax = 0.0;
+    for (int j = 0; j < n; j++) {
+      const double r = (j > 0 ? sqrt(se2[j - 1]) : 0.0) + (j + 1 < n ? sqrt(se2[j]) : 0.0);
+      gl = fmin(gl, sd[j] - r); gu = fmax(gu, sd[j] + r); emax = fmax(emax, se2[j]);
+    }
+    const double tn = fmax(fabs(gl), fabs(gu));
+    s_gl = gl - 2.2e-16 * tn * n - 1e-300; s_gu = gu + 2.2e-16 * tn * n + 1e-300;
+    s_piv = 2.3e-308 * fmax(1.0, emax);
+    if (blockIdx.x == 0) tnorm[0] = tn;
+  }
+  __syncthreads();
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n_eig) return;
+  double lo = s_gl, hi = s_gu;
+  const double piv = s_piv;
+  for (int it = 0; it < 200; it++) {
+    const double mid = 0.5 * (lo + hi);
+    if (hi - lo <= 2.0 * 2.2e-16 * fmax(fabs(lo), fabs(hi)) + 2.0 * piv || mid <= lo || mid >= hi) break;
+    double q = sd[0] - mid;
+    int c = q < 0.0;
+    for (int j = 1; j < n; j++) {
+      if (fabs(q) < piv) q = -piv;
+      q = sd[j] - mid - se2[j - 1] / q;
+      c += q < 0.0;
+    }
+    if (c >= idx + 1) hi = mid; else lo = mid;
+  }
+  lam[idx] = 0.5 * (lo + hi);
+}
+
+// (3) z_i = eigenvector of T for lam[i] by inverse iteration; ws layout [6][n][n_eig] (thread index fastest)
+__global__ void __launch_bounds__(128) invit_kernel(const double* __restrict__ d, const double* __restrict__ e, int n, int n_eig,
+                                                    const double* __restrict__ lam, const double* __restrict__ tnorm,
+                                                    double* __restrict__ ws, cplx* __restrict__ Z) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n_eig) return;
+  const long long S = n_eig;
+  double* dl = ws + idx;                   // multipliers          dl[j] at dl[j * S]
+  double* dd = dl + (long long)n * S;      // U diagonal
+  double* du = dd + (long long)n * S;      // U first superdiagonal
+  double* du2 = du + (long long)n * S;     // U second superdiagonal
+  double* pv = du2 + (long long)n * S;     // 1.0 if rows j, j+1 were swapped
+  double* x = pv + (long long)n * S;       // the iterate
+  const double tn = fmax(tnorm[0], 1e-300), eps = 2.2e-16;
+  // a tiny index-dependent shift keeps (numerically) equal eigenvalues from giving identical vectors
+  const double sigma = lam[idx] + eps * tn * (double)((idx % 7) - 3);
+  for (int j = 0; j < n; j++) { dd[j * S] = d[j] - sigma; du[j * S] = j + 1 < n ? e[j] : 0.0; dl[j * S] = j + 1 < n ? e[j] : 0.0; du2[j * S] = 0.0; }
+  // LU with partial pivoting (dgttrf)
+  for (int j = 0; j + 1 < n; j++) {
+    const double dj = dd[j * S], lj = dl[j * S];
+    if (fabs(dj) >= fabs(lj)) {
+      double piv = dj;
+      if (piv == 0.0) { piv = eps * tn; dd[j * S] = piv; }
+      const double f = lj / piv;
+      dl[j * S] = f; pv[j * S] = 0.0;
+      dd[(j + 1) * S] -= f * du[j * S];
+    } else {
+      const double f = dj / lj;
+      dd[j * S] = lj; dl[j * S] = f; pv[j * S] = 1.0;
+      const double t = du[j * S];
+      du[j * S] = dd[(j + 1) * S];
+      dd[(j + 1) * S] = t - f * dd[(j + 1) * S];
+      if (j + 2 < n) { du2[j * S] = du[(j + 1) * S]; du[(j + 1) * S] = -f * du[(j + 1) * S]; }
+    }
+  }
+  if (dd[(n - 1) * S] == 0.0) dd[(n - 1) * S] = eps * tn;
+  // start vector: deterministic pseudo-random signs
+  for (int j = 0; j < n; j++) {
+    unsigned h = (unsigned)(j * 2654435761u) ^ (unsigned)(idx * 40503u + 12345u);
+    h ^= h >> 15; h *= 2246822519u; h ^= h >> 13;
+    x[j * S] = 0.5 + (double)(h & 0xffff) * (1.0 / 65536.0);
+  }
+  for (int iter = 0; iter < 4; iter++) {
+    // forward (L with the row interchanges)
+    for (int j = 0; j + 1 < n; j++) {
+      if (pv[j * S] == 0.0) x[(j + 1) * S] -= dl[j * S] * x[j * S];
+      else { const double t = x[j * S]; x[j * S] = x[(j + 1) * S]; x[(j + 1) * S] = t - dl[j * S] * x[j * S]; }
+    }
+    // back substitution (U)
+    x[(n - 1) * S] /= dd[(n - 1) * S];
+    if (n > 1) x[(n - 2) * S] = (x[(n - 2) * S] - du[(n - 2) * S] * x[(n - 1) * S]) / dd[(n - 2) * S];
+    for (int j = n - 3; j >= 0; j--) x[j * S] = (x[j * S] - du[j * S] * x[(j + 1) * S] - du2[j * S] * x[(j + 2) * S]) / dd[j * S];
+    // normalise (max norm first: the solve amplifies by ~1/eps)
+    double mx = 0.0;
+    for (int j = 0; j < n; j++) mx = fmax(mx, fabs(x[j * S]));
+    const double r = mx > 0.0 ? 1.0 / mx : 1.0;
+    double s2 = 0.0;
+    for (int j = 0; j < n; j++) { const double t = x[j * S] * r; x[j * S] = t; s2 += t * t; }
+    const double r2 = s2 > 0.0 ? 1.0 / sqrt(s2) : 1.0;
+    for (int j = 0; j < n; j++) x[j * S] *= r2;
+  }
+  for (int j = 0; j < n; j++) Z[(long long)idx * n + j] = make_double2(x[j * S], 0.0);
+}
+
+// (4) rows of Z <- Q z:  y <- H_0 H_1 ... H_{n-2} y,  H_k = I - tau_k v_k v_k^H.  NV vectors per CTA, kept in shared memory.
+constexpr int BT_NV = 4;
+__global__ void __launch_bounds__(256) backtransform_kernel(const cplx* __restrict__ Vh, const cplx* __restrict__ tau, int n, int n_eig,
+                                                            cplx* __restrict__ Z) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx* y = reinterpret_cast<cplx*>(smem_raw);   // [BT_NV][n]
+  __shared__ double sh[2 * BT_NV * 8];
+  const int tid = threadIdx.x, v0 = blockIdx.x * BT_NV, nv = min(BT_NV, n_eig - v0);
+  for (int idx = tid; idx < BT_NV * n; idx += 256) {
+    const int u = idx / n, j = idx - u * n;
+    y[idx] = u < nv ? Z[(long long)(v0 + u) * n + j] : make_double2(0.0, 0.0);
+  }
+  __syncthreads();
+  for (int k = n - 2; k >= 0; k--) {
+    const cplx t = tau[k];
+    if (t.x == 0.0 && t.y == 0.0) continue;
+    const cplx* vk = Vh + (long long)k * n;
+    double s[2 * BT_NV];
+#pragma unroll
+    for (int u = 0; u < 2 * BT_NV; u++) s[u] = 0.0;
+    for (int j = k + 1 + tid; j < n; j += 256) {
+      const cplx v = vk[j];
+#pragma unroll
+      for (int u = 0; u < BT_NV; u++) { const cplx yy = y[u * n + j]; s[2 * u] += v.x * yy.x + v.y * yy.y; s[2 * u + 1] += v.x * yy.y - v.y * yy.x; }
+    }
+    bsum<2 * BT_NV>(s, sh);
+    for (int j = k + 1 + tid; j < n; j += 256) {
+      const cplx v = vk[j];
+#pragma unroll
+      for (int u = 0; u < BT_NV; u++) {
+        const cplx f = cmulf(t, make_double2(s[2 * u], s[2 * u + 1]));     // tau (v^H y)
+        const cplx g = cmulf(f, v);
+        y[u * n + j].x -= g.x; y[u * n + j].y -= g.y;
+      }
+    }
+    __syncthreads();
+  }
+  for (int idx = tid; idx < nv * n; idx += 256) {
+    const int u = idx / n, j = idx - u * n;
+    Z[(long long)(v0 + u) * n + j] = y[idx];
+  }
+}
+
+}  // namespace
+
+size_t tridiag_workspace_bytes(int n, int n_eig) {
+  return ws_round((size_t)n * sizeof(cplx)) * 2 + ws_round((size_t)n * sizeof(double)) * 2 + ws_round((size_t)6 * n * n_eig * sizeof(double)) + 1024;
+}
+
+// H (n x n Hermitian, row-major, leading dimension ld, not modified) -> C [n_eig][n] (rows = eigenvectors of the n_eig
+// smallest eigenvalues, unit norm up to rounding, NOT yet re-orthogonalised), lambda dev [n_eig] ascending.
+// Abuf, Vbuf: n x n scratch each.  Returns RPA_OK, or a negative code (the caller may fall back to Jacobi).
+int tridiag_eigh_lowest(rpa_ctx* ctx, WsAlloc& ws, const cplx* H, long long ld, int n, int n_eig, cplx* Abuf, cplx* Vbuf, cplx* C,
+                        double* lambda) {
+  cplx* tau = ws.get<cplx>(n);
+  cplx* p = ws.get<cplx>(n);
+  double* d = ws.get<double>(n);
+  double* e = ws.get<double>(n);
+  double* iws = ws.get<double>((size_t)6 * n * n_eig);
+  double* tnorm = ws.get<double>(8);
+  if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_subspace_basis: workspace too small (need %zu bytes)", ws.off);
+  RPA_CUDA(ctx, cudaMemcpy2DAsync(Abuf, (size_t)n * sizeof(cplx), H, (size_t)ld * sizeof(cplx), (size_t)n * sizeof(cplx), n,
+                                  cudaMemcpyDeviceToDevice, ctx->stream));
+  int coop = 0, per_sm = 0;
+  cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device);
+  const size_t smem1 = (size_t)2 * n * sizeof(cplx);
+  if (!coop || smem1 > 96 * 1024) return RPA_ERR_INVALID;
+  const void* fn = (const void*)hetrd_kernel;
+  RPA_CUDA(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 256, smem1) != cudaSuccess || per_sm < 1) return RPA_ERR_INVALID;
+  const int grid = std::min(ctx->sm_count * std::min(per_sm, 2), (n + 7) / 8);
+  cplx* A_ = Abuf; int n_ = n; cplx* V_ = Vbuf; cplx* tau_ = tau; double* d_ = d; double* e_ = e; cplx* p_ = p;
+  void* args[] = {&A_, &n_, &V_, &tau_, &d_, &e_, &p_};
+  RPA_CUDA(ctx, cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(256), args, smem1, ctx->stream));
+  ctx->launches++;
+  const int nb = (n_eig + 127) / 128;
+  bisect_kernel<<<nb, 128, (size_t)2 * n * sizeof(double), ctx->stream>>>(d, e, n, n_eig, lambda, tnorm);
+  RPA_LAUNCH_CHECK(ctx);
+  invit_kernel<<<nb, 128, 0, ctx->stream>>>(d, e, n, n_eig, lambda, tnorm, iws, C);
+  RPA_LAUNCH_CHECK(ctx);
+  const size_t smem4 = (size_t)BT_NV * n * sizeof(cplx);
+  RPA_CUDA(ctx, cudaFuncSetAttribute(backtransform_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+  backtransform_kernel<<<(n_eig + BT_NV - 1) / BT_NV, 256, smem4, ctx->stream>>>(Vbuf, tau, n, n_eig, C);
+  RPA_LAUNCH_CHECK(ctx);
+  return RPA_OK;
+}
