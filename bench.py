@@ -299,7 +299,12 @@ def main():
     }
     jn, jsweeps, jkind = rpa.rpa_basis_info(ctx)
     if jn > 0:   # direct Jacobi of chi~0(0): vector form = FP64 ALU work, block form = DMMA GEMM work
-        kwork["basis"] = ("FLOP", jsweeps * 32.0 * jn ** 3) if jkind == 1 else ("ALU", jsweeps * 0.5 * jn * (jn - 1) * 44.0 * jn)
+        if jkind == 1:
+            kwork["basis"] = ("FLOP", jsweeps * 32.0 * jn ** 3)
+        elif jkind == 2:   # tridiagonalisation (16/3 n^3 real FLOP for a complex Hermitian matrix) + back-transformation (8 n^2 n_eig)
+            kwork["basis"] = ("ALU", 16.0 / 3.0 * jn ** 3 + 8.0 * jn * jn * n_eig)
+        else:
+            kwork["basis"] = ("ALU", jsweeps * 0.5 * jn * (jn - 1) * 44.0 * jn)
     kernels = {}
     for k, (kms, kn) in kprof.items():
         ent = {"ms_per_step": kms / args.steps, "launches_per_step": kn / args.steps}
@@ -322,6 +327,7 @@ def main():
              "chi0": "zgemm_dmma_kernel<1,1,1,3> (CHI_SUM a2)", "proj": "zgemm_dmma_kernel<0,0,1,2> (projection a4)",
              "chis": "zgemm_dmma_kernel<1,1,1,3> batched over omega (chi_s a4)",
              "basis": "jacobi_persistent_kernel (a3: one-sided Jacobi of chi~0(0), all sweeps in one cooperative launch)" if jkind == 0
+             else "hetrd_kernel + bisect/invit/backtransform kernels (a3: tridiagonalisation route for the lowest N_eig eigenpairs)" if jkind == 2
              else "block Jacobi of chi~0(0) (a3: batched zgemm_dmma Gram + pair_rotations_kernel + batched zgemm_dmma update)"}
     tr = traffic_tab.get(f"{dom}:cfg{args.config}")
     if kwork[dom][0] == "B":
@@ -338,8 +344,10 @@ def main():
                     "frac": kwork[dom][1] / avg_s / 1e12 / dfma_peak, "traffic": tr,
                     "peak_source": "FP64 FMA register-only microbenchmark measured in this run (rpa_fp64_peak kind 1)",
                     "algorithmic_flops_per_launch": kwork[dom][1], "avg_launch_ms": avg_s * 1e3,
-                    "flops_model": f"{jsweeps} sweeps x n(n-1)/2 pairs x 44 n FLOP (16 n for the three dot products, 28 n for the "
-                                   f"rotation), n = {jn}; the kernel is bound by the grid-wide barrier per round, not by the ALUs",
+                    "flops_model": (f"16/3 n^3 + 8 n^2 N_eig FLOP, n = {jn}; bound by the two grid-wide barriers per Householder step"
+                                    if jkind == 2 else
+                                    f"{jsweeps} sweeps x n(n-1)/2 pairs x 44 n FLOP (16 n for the three dot products, 28 n for the "
+                                    f"rotation), n = {jn}; the kernel is bound by the grid-wide barrier per round, not by the ALUs"),
                     "share_of_step": kd["ms_per_step"] / ms_per_step}
     else:
         per_launch = kwork[dom][1] / max(1.0, kd["launches_per_step"])

@@ -567,7 +567,7 @@ int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, dou
       rc = tridiag_eigh_lowest(ctx, wt, chi0, n, n, n_eig, jw.A, jw.V, C, lambda);
       if (rc == RPA_ERR_WORKSPACE) return rc;
       bool ok = rc == RPA_OK && wt.ok;
-      for (int pass = 0; pass < 2 && ok; pass++) {
+      for (int pass = 0; pass < 1 && ok; pass++) {   // the vectors arrive orthogonal to ~eps / gap: one CholeskyQR pass restores eps
         ZgemmParams g;
         g.A = C; g.lda = n; g.a_km = false; g.B = C; g.ldb = n; g.b_kn = false; g.C = S; g.ldc = n_eig;
         g.M = n_eig; g.N = n_eig; g.K = n; g.conj_b = true; g.herm = true;

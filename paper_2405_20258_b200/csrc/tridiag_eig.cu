@@ -111,7 +111,7 @@ __global__ void __launch_bounds__(256) hetrd_kernel(cplx* __restrict__ A, int n,
 namespace {
 
 // (2) lam[i] = i-th smallest eigenvalue of T, i < n_eig: bisection on the Sturm count (one thread per eigenvalue)
-__global__ void __launch_bounds__(128) bisect_kernel(const double* __restrict__ d, const double* __restrict__ e, int n, int n_eig,
+__global__ void __launch_bounds__(256) bisect_kernel(const double* __restrict__ d, const double* __restrict__ e, int n, int n_eig,
                                                      double* __restrict__ lam, double* __restrict__ tnorm) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double* sd = reinterpret_cast<double*>(smem_raw);   // [n]
@@ -131,33 +131,43 @@ __global__ void __launch_bounds__(128) bisect_kernel(const double* __restrict__ 
     if (blockIdx.x == 0) tnorm[0] = tn;
   }
   __syncthreads();
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  // one warp per eigenvalue: 32 trial points per step (the interval shrinks 33-fold per Sturm sweep)
+  const int lane = threadIdx.x & 31;
+  const int idx = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (idx >= n_eig) return;
   double lo = s_gl, hi = s_gu;
   const double piv = s_piv;
-  for (int it = 0; it < 200; it++) {
-    const double mid = 0.5 * (lo + hi);
-    if (hi - lo <= 2.0 * 2.2e-16 * fmax(fabs(lo), fabs(hi)) + 2.0 * piv || mid <= lo || mid >= hi) break;
-    double q = sd[0] - mid;
+  for (int it = 0; it < 40; it++) {
+    const double h = (hi - lo) / 33.0;
+    if (hi - lo <= 2.0 * 2.2e-16 * fmax(fabs(lo), fabs(hi)) + 2.0 * piv || !(h > 0.0)) break;
+    const double x = lo + h * (lane + 1);
+    double q = sd[0] - x;
     int c = q < 0.0;
     for (int j = 1; j < n; j++) {
       if (fabs(q) < piv) q = -piv;
-      q = sd[j] - mid - se2[j - 1] / q;
+      q = sd[j] - x - se2[j - 1] / q;
       c += q < 0.0;
     }
-    if (c >= idx + 1) hi = mid; else lo = mid;
+    const unsigned m = __ballot_sync(0xffffffffu, c >= idx + 1);   // counts are monotone in x: a suffix of lanes
+    const int first = m ? __ffs(m) - 1 : 32;
+    const double nlo = first == 0 ? lo : lo + h * first, nhi = first == 32 ? hi : lo + h * (first + 1);
+    lo = nlo; hi = nhi;
   }
-  lam[idx] = 0.5 * (lo + hi);
+  if (lane == 0) lam[idx] = 0.5 * (lo + hi);
 }
 
-// (3) z_i = eigenvector of T for lam[i] by inverse iteration; ws layout [6][n][n_eig] (thread index fastest)
-__global__ void __launch_bounds__(128) invit_kernel(const double* __restrict__ d, const double* __restrict__ e, int n, int n_eig,
-                                                    const double* __restrict__ lam, const double* __restrict__ tnorm,
-                                                    double* __restrict__ ws, cplx* __restrict__ Z) {
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= n_eig) return;
-  const long long S = n_eig;
-  double* dl = ws + idx;                   // multipliers          dl[j] at dl[j * S]
+// (3) z_i = eigenvector of T for lam[i] by inverse iteration.  The solves are sequential in j, so what matters is the
+// latency of a step: IV_NT eigenvectors per CTA (one lane each), their LU factors in shared memory, layout [6][n][IV_NT].
+constexpr int IV_NT = 4;
+__global__ void __launch_bounds__(32) invit_kernel(const double* __restrict__ d, const double* __restrict__ e, int n, int n_eig,
+                                                   const double* __restrict__ lam, const double* __restrict__ tnorm,
+                                                   cplx* __restrict__ Z) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double* ws = reinterpret_cast<double*>(smem_raw);
+  const int idx = blockIdx.x * IV_NT + threadIdx.x;
+  if (threadIdx.x >= IV_NT || idx >= n_eig) return;
+  const int S = IV_NT;
+  double* dl = ws + threadIdx.x;           // multipliers          dl[j] at dl[j * S]
   double* dd = dl + (long long)n * S;      // U diagonal
   double* du = dd + (long long)n * S;      // U first superdiagonal
   double* du2 = du + (long long)n * S;     // U second superdiagonal
@@ -192,7 +202,7 @@ __global__ void __launch_bounds__(128) invit_kernel(const double* __restrict__ d
     h ^= h >> 15; h *= 2246822519u; h ^= h >> 13;
     x[j * S] = 0.5 + (double)(h & 0xffff) * (1.0 / 65536.0);
   }
-  for (int iter = 0; iter < 4; iter++) {
+  for (int iter = 0; iter < 3; iter++) {
     // forward (L with the row interchanges)
     for (int j = 0; j + 1 < n; j++) {
       if (pv[j * S] == 0.0) x[(j + 1) * S] -= dl[j * S] * x[j * S];
@@ -260,7 +270,7 @@ __global__ void __launch_bounds__(256) backtransform_kernel(const cplx* __restri
 }  // namespace
 
 size_t tridiag_workspace_bytes(int n, int n_eig) {
-  return ws_round((size_t)n * sizeof(cplx)) * 2 + ws_round((size_t)n * sizeof(double)) * 2 + ws_round((size_t)6 * n * n_eig * sizeof(double)) + 1024;
+  return ws_round((size_t)n * sizeof(cplx)) * 2 + ws_round((size_t)n * sizeof(double)) * 2 + 1024;
 }
 
 // H (n x n Hermitian, row-major, leading dimension ld, not modified) -> C [n_eig][n] (rows = eigenvectors of the n_eig
@@ -272,7 +282,6 @@ int tridiag_eigh_lowest(rpa_ctx* ctx, WsAlloc& ws, const cplx* H, long long ld, 
   cplx* p = ws.get<cplx>(n);
   double* d = ws.get<double>(n);
   double* e = ws.get<double>(n);
-  double* iws = ws.get<double>((size_t)6 * n * n_eig);
   double* tnorm = ws.get<double>(8);
   if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_subspace_basis: workspace too small (need %zu bytes)", ws.off);
   RPA_CUDA(ctx, cudaMemcpy2DAsync(Abuf, (size_t)n * sizeof(cplx), H, (size_t)ld * sizeof(cplx), (size_t)n * sizeof(cplx), n,
@@ -280,7 +289,7 @@ int tridiag_eigh_lowest(rpa_ctx* ctx, WsAlloc& ws, const cplx* H, long long ld, 
   int coop = 0, per_sm = 0;
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device);
   const size_t smem1 = (size_t)2 * n * sizeof(cplx);
-  if (!coop || smem1 > 96 * 1024) return RPA_ERR_INVALID;
+  if (!coop || smem1 > 96 * 1024 || (size_t)6 * n * IV_NT * sizeof(double) > 200 * 1024) return RPA_ERR_INVALID;
   const void* fn = (const void*)hetrd_kernel;
   RPA_CUDA(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 256, smem1) != cudaSuccess || per_sm < 1) return RPA_ERR_INVALID;
@@ -289,10 +298,11 @@ int tridiag_eigh_lowest(rpa_ctx* ctx, WsAlloc& ws, const cplx* H, long long ld, 
   void* args[] = {&A_, &n_, &V_, &tau_, &d_, &e_, &p_};
   RPA_CUDA(ctx, cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(256), args, smem1, ctx->stream));
   ctx->launches++;
-  const int nb = (n_eig + 127) / 128;
-  bisect_kernel<<<nb, 128, (size_t)2 * n * sizeof(double), ctx->stream>>>(d, e, n, n_eig, lambda, tnorm);
+  bisect_kernel<<<(n_eig + 7) / 8, 256, (size_t)2 * n * sizeof(double), ctx->stream>>>(d, e, n, n_eig, lambda, tnorm);
   RPA_LAUNCH_CHECK(ctx);
-  invit_kernel<<<nb, 128, 0, ctx->stream>>>(d, e, n, n_eig, lambda, tnorm, iws, C);
+  const size_t smem3 = (size_t)6 * n * IV_NT * sizeof(double);
+  RPA_CUDA(ctx, cudaFuncSetAttribute(invit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+  invit_kernel<<<(n_eig + IV_NT - 1) / IV_NT, 32, smem3, ctx->stream>>>(d, e, n, n_eig, lambda, tnorm, C);
   RPA_LAUNCH_CHECK(ctx);
   const size_t smem4 = (size_t)BT_NV * n * sizeof(cplx);
   RPA_CUDA(ctx, cudaFuncSetAttribute(backtransform_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
