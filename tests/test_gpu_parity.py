@@ -613,3 +613,40 @@ def test_phase_invariance_and_degenerate_sizes():
         assert abs(e - 2.0 * (np.log1p(-mu) + mu) / (2 * np.pi)) <= 1e-12 * abs(e)
     finally:
         rpa.rpa_destroy(ctx)
+
+
+@pytest.mark.parametrize("n,n_eig", [(200, 50), (640, 212)])
+def test_subspace_basis_degenerate_and_clustered_spectrum(n, n_eig):
+    """a3 on spectra the tridiagonal route finds hard: exactly degenerate wanted eigenvalues (multiplicity 3 and 5), a
+    cluster of 8 eigenvalues within 1e-9 relative, and the cut N_eig placed right after a cluster.  Eigenvalues, residuals,
+    orthonormality and the spanned subspace must still meet the tolerances (the library may fall back to Jacobi)."""
+    import paper_2405_20258_b200 as rpa
+    import torch
+    rng = np.random.default_rng(7 * n + n_eig)
+    q, _ = np.linalg.qr(rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n)))
+    spec = -1.0 / (1.0 + np.arange(n)) ** (2.0 / 3.0)
+    spec[3:6] = spec[3]                                        # exact triple
+    spec[20:25] = spec[20]                                     # exact quintuple
+    spec[n_eig - 8:n_eig] = spec[n_eig - 8] * (1.0 + 1e-9 * np.arange(8))   # tight cluster ending at the cut
+    spec = np.sort(spec)
+    H = (q * spec[None, :]) @ q.conj().T
+    H = 0.5 * (H + H.conj().T)
+    cfgn = RpaConfig("b", 1, (30.0, 30.0, 30.0), (40, 40, 40), 0.3, 0.45 if n <= 380 else 1.1, 1, 1, (-0.6, 0.0), (0.05, 3.0), 1, 2)
+    base = make_inputs(cfgn)
+    assert base.n_g >= n
+    base = dataclasses.replace(base, g_eps=base.g_eps[:n], vcoul=base.vcoul[:n])
+    ctx = make_ctx(base, 1, 1, n_eig, 2)
+    try:
+        Cm = torch.empty((n_eig, n), dtype=torch.complex128, device="cuda")
+        lam = torch.empty(n_eig, dtype=torch.float64, device="cuda")
+        rpa.rpa_subspace_basis(ctx, dev(H), n_eig, 1e-12, Cm, lam)
+        Cg, lg = Cm.cpu().numpy(), lam.cpu().numpy()
+    finally:
+        rpa.rpa_destroy(ctx)
+    lref = np.linalg.eigvalsh(H)[:n_eig]
+    assert eig_rel(lg, lref) <= TOL_LAM
+    assert np.abs(Cg.conj() @ Cg.T - np.eye(n_eig)).max() <= 1e-11
+    res = H @ Cg.T - Cg.T * lg[None, :]
+    assert np.abs(res).max() <= 1e-9 * abs(lref[0])            # vectors inside a 1e-9 cluster mix: residual ~ cluster width
+    vec = np.linalg.eigh(H)[1][:, :n_eig]
+    assert projector_err(Cg, np.ascontiguousarray(vec.T)) <= 1e-8
