@@ -521,6 +521,10 @@ int block_size(int n, int n_eig) {
   return std::min(p, n);
 }
 bool use_direct(int n, int n_eig) { return 2 * block_size(n, n_eig) > n; }
+// tridiagonalisation + bisection + inverse iteration (tridiag_eig.cu): part of the spectrum, v and the Sturm data in shared memory
+bool use_tridiag(int n, int n_eig) {
+  return n >= 32 && n <= 12800 && 4 * n_eig <= 3 * n && !getenv("RPA_NO_TRIDIAG") && (n < jacobi_block_min() || !getenv("RPA_NO_TRIDIAG_LARGE"));
+}
 
 }  // namespace
 
@@ -530,9 +534,11 @@ size_t basis_workspace_bytes(const rpa_ctx* ctx, int n, int n_eig) {
   auto jac = [](size_t m) {   // A, V (padded to whole blocks) and the Gram / rotation matrices of the block iteration
     return 2 * ws_round((m + JB) * m * sizeof(cplx)) + 2 * ws_round(((m + JB) / JP + 1) * JP * JP * sizeof(cplx));
   };
-  if (use_direct(n, n_eig)) return jac(n) + small + tridiag_workspace_bytes(n, n_eig) + ws_round((size_t)n_eig * n_eig * sizeof(cplx));
+  const size_t direct = jac(n) + small + tridiag_workspace_bytes(n, n_eig) + ws_round((size_t)n_eig * n_eig * sizeof(cplx));
+  if (use_direct(n, n_eig)) return direct;
   const size_t p = block_size(n, n_eig);
-  return 3 * ws_round(p * n * sizeof(cplx)) + 2 * ws_round(p * p * sizeof(cplx)) + jac(p) + small;
+  const size_t iter = 3 * ws_round(p * n * sizeof(cplx)) + 2 * ws_round(p * p * sizeof(cplx)) + jac(p) + small;
+  return use_tridiag(n, n_eig) ? std::max(direct, iter) : iter;
 }
 
 int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, double tol, cplx* C, double* lambda,
@@ -552,14 +558,16 @@ int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, dou
   jw.info = ws.get<int>(4);
   int* d_info = ws.get<int>(4);
   int rc;
-  if (use_direct(n, n_eig)) {
+  const WsAlloc ws_iter = ws;   // the block iteration below restarts from here when the tridiagonal route fails
+  const bool direct = use_direct(n, n_eig);
+  if (direct || use_tridiag(n, n_eig)) {
     jw.A = ws.get<cplx>((size_t)(n + JB) * n);
     jw.V = ws.get<cplx>((size_t)(n + JB) * n);
     jw.Wb = ws.get<cplx>((size_t)((n + JB) / JP + 1) * JP * JP);
     jw.Ub = ws.get<cplx>((size_t)((n + JB) / JP + 1) * JP * JP);
     if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_subspace_basis: workspace too small (need %zu bytes)", ws.off);
-    if (n >= 32 && n < jacobi_block_min() && 4 * n_eig <= 3 * n && !getenv("RPA_NO_TRIDIAG")) {
-      // small matrix, part of the spectrum: tridiagonalisation + bisection + inverse iteration (tridiag_eig.cu), then a
+    if (use_tridiag(n, n_eig)) {
+      // part of the spectrum: tridiagonalisation + bisection + inverse iteration (tridiag_eig.cu), then a
       // CholeskyQR2 clean-up of the n_eig vectors; any failure (e.g. a numerically singular Gram matrix because wanted
       // eigenvalues coincide) falls through to the Jacobi iteration below
       WsAlloc wt = ws;
@@ -588,6 +596,8 @@ int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, dou
       }
       (void)cudaGetLastError();
     }
+  }
+  if (direct) {
     if ((rc = jacobi_eigh(ctx, chi0, n, n, false, n_eig, n_eig < n, jw, order_h, lam_h))) return rc;
     if ((rc = jacobi_vectors(ctx, jw, n, n_eig, C, n))) return rc;
     std::vector<double> ls(n_eig);
@@ -599,6 +609,7 @@ int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, dou
   }
 
   // ---- block subspace iteration ----
+  ws = ws_iter;
   const int p = block_size(n, n_eig);
   cplx* X = ws.get<cplx>((size_t)p * n);
   cplx* Y = ws.get<cplx>((size_t)p * n);

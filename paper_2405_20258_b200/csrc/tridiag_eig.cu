@@ -34,11 +34,12 @@ __device__ __forceinline__ cplx cmulf(cplx a, cplx b) { return make_double2(a.x 
 
 // (1) A: n x n Hermitian, row-major, both triangles (destroyed).  Vh[k][:] = reflector v_k (v_k[j] = 0 for j <= k,
 // v_k[k+1] = 1), tau[k]; T = tridiag(e, d, e).  256 threads per CTA, one warp per matrix row in the two O(m^2) phases.
+template <bool W_SMEM>
 __global__ void __launch_bounds__(256) hetrd_kernel(cplx* __restrict__ A, int n, cplx* __restrict__ Vh, cplx* __restrict__ tau,
                                                     double* __restrict__ d, double* __restrict__ e, cplx* __restrict__ p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx* v = reinterpret_cast<cplx*>(smem_raw);   // [n]
-  cplx* w = v + n;                               // [n]
+  cplx* w = v + n;                               // [n] (W_SMEM only; otherwise w_j = p_j + al2 v_j is formed on the fly)
   __shared__ double sh[4 * 8];
   cg::grid_group grid = cg::this_grid();
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -85,15 +86,22 @@ __global__ void __launch_bounds__(256) hetrd_kernel(cplx* __restrict__ A, int n,
     for (int i = k + 1 + tid; i < n; i += 256) { const cplx x = __ldcg(p + i), b = v[i]; q[0] += x.x * b.x + x.y * b.y; q[1] += x.x * b.y - x.y * b.x; }
     bsum<2>(q, sh);
     const cplx al2 = cmulf(make_double2(-0.5 * t.x, -0.5 * t.y), make_double2(q[0], q[1]));
-    for (int i = k + 1 + tid; i < n; i += 256) { const cplx x = __ldcg(p + i), av = cmulf(al2, v[i]); w[i] = make_double2(x.x + av.x, x.y + av.y); }
+    if (W_SMEM) {
+      for (int i = k + 1 + tid; i < n; i += 256) { const cplx x = __ldcg(p + i), av = cmulf(al2, v[i]); w[i] = make_double2(x.x + av.x, x.y + av.y); }
+    }
     __syncthreads();
+    auto wval = [&](int i) -> cplx {
+      if (W_SMEM) return w[i];
+      const cplx x = __ldcg(p + i), av = cmulf(al2, v[i]);
+      return make_double2(x.x + av.x, x.y + av.y);
+    };
     // ---- A22 -= v w^H + w v^H  (warp per row)
     if (t.x != 0.0 || t.y != 0.0) {
       for (int i = k + 1 + gw; i < n; i += nw) {
         cplx* ri = A + (long long)i * n;
-        const cplx vi = v[i], wi = w[i];
+        const cplx vi = v[i], wi = wval(i);
         for (int j = k + 1 + lane; j < n; j += 32) {
-          const cplx vj = v[j], wj = w[j];
+          const cplx vj = v[j], wj = wval(j);
           cplx a = __ldcg(ri + j);
           a.x -= vi.x * wj.x + vi.y * wj.y + wi.x * vj.x + wi.y * vj.y;      // v_i conj(w_j) + w_i conj(v_j)
           a.y -= vi.y * wj.x - vi.x * wj.y + wi.y * vj.x - wi.x * vj.y;
@@ -159,15 +167,18 @@ __global__ void __launch_bounds__(256) bisect_kernel(const double* __restrict__ 
 // (3) z_i = eigenvector of T for lam[i] by inverse iteration.  The solves are sequential in j, so what matters is the
 // latency of a step: IV_NT eigenvectors per CTA (one lane each), their LU factors in shared memory, layout [6][n][IV_NT].
 constexpr int IV_NT = 4;
-__global__ void __launch_bounds__(32) invit_kernel(const double* __restrict__ d, const double* __restrict__ e, int n, int n_eig,
-                                                   const double* __restrict__ lam, const double* __restrict__ tnorm,
-                                                   cplx* __restrict__ Z) {
+// element stride of the factor arrays: int in shared memory (a 64-bit stride there gave wrong vectors at n = 146, 147 with nvcc 12.9)
+template <bool SMEM> struct IvStride { using type = long long; };
+template <> struct IvStride<true> { using type = int; };
+template <bool SMEM>   // SMEM: launched with 32 threads, IV_NT of them active; otherwise 128 threads, gws = [6][n][n_eig]
+__global__ void __launch_bounds__(SMEM ? 32 : 128) invit_kernel(const double* __restrict__ d, const double* __restrict__ e, int n, int n_eig,
+                             const double* __restrict__ lam, const double* __restrict__ tnorm, double* __restrict__ gws,
+                             cplx* __restrict__ Z) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  double* ws = reinterpret_cast<double*>(smem_raw);
-  const int idx = blockIdx.x * IV_NT + threadIdx.x;
-  if (threadIdx.x >= IV_NT || idx >= n_eig) return;
-  const int S = IV_NT;
-  double* dl = ws + threadIdx.x;           // multipliers          dl[j] at dl[j * S]
+  const int idx = SMEM ? blockIdx.x * IV_NT + threadIdx.x : blockIdx.x * blockDim.x + threadIdx.x;
+  if ((SMEM && threadIdx.x >= IV_NT) || idx >= n_eig) return;
+  const typename IvStride<SMEM>::type S = SMEM ? IV_NT : n_eig;
+  double* dl = SMEM ? reinterpret_cast<double*>(smem_raw) + threadIdx.x : gws + idx;   // multipliers  dl[j] at dl[j * S]
   double* dd = dl + (long long)n * S;      // U diagonal
   double* du = dd + (long long)n * S;      // U first superdiagonal
   double* du2 = du + (long long)n * S;     // U second superdiagonal
@@ -269,8 +280,74 @@ __global__ void __launch_bounds__(256) backtransform_kernel(const cplx* __restri
 
 }  // namespace
 
+namespace {
+// Compact-WY factor of a block of nb reflectors (LAPACK zlarft, forward / columnwise):  H_k0 ... H_k0+nb-1 = I - V T V^H.
+// G[r][s] = sum_j v_r[j] conj(v_s[j]) (Gram of the block).  Writes Tc = conj(T), row-major [nb][ldt], zero below the diagonal.
+__global__ void __launch_bounds__(256) larft_kernel(const cplx* __restrict__ G, int ldg, const cplx* __restrict__ tau, int nb,
+                                                    cplx* __restrict__ Tc, int ldt) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx (*T)[65] = reinterpret_cast<cplx (*)[65]>(smem_raw);   // [64][65]
+  cplx* x = reinterpret_cast<cplx*>(smem_raw) + 64 * 65;      // [64]
+  const int tid = threadIdx.x;
+  for (int idx = tid; idx < nb * nb; idx += 256) T[idx / nb][idx % nb] = make_double2(0.0, 0.0);
+  __syncthreads();
+  for (int i = 0; i < nb; i++) {
+    const cplx ti = tau[i];
+    if (tid < i) x[tid] = G[(long long)i * ldg + tid];          // (V^H v_i)[s] = G[i][s]
+    __syncthreads();
+    if (tid < i) {                                              // T[0:i, i] = -tau_i T[0:i, 0:i] x
+      cplx acc = make_double2(0.0, 0.0);
+      for (int s = tid; s < i; s++) { const cplx a = T[tid][s], b = x[s]; acc.x += a.x * b.x - a.y * b.y; acc.y += a.x * b.y + a.y * b.x; }
+      T[tid][i] = make_double2(-(ti.x * acc.x - ti.y * acc.y), -(ti.x * acc.y + ti.y * acc.x));
+    }
+    if (tid == 0) T[i][i] = ti;
+    __syncthreads();
+  }
+  for (int idx = tid; idx < nb * nb; idx += 256) { const cplx a = T[idx / nb][idx % nb]; Tc[(long long)(idx / nb) * ldt + idx % nb] = make_double2(a.x, -a.y); }
+}
+}  // namespace
+
+// rows of Y [n_eig][n] <- Q y with Q = H_0 ... H_{n-2}, blocked: three DMMA GEMMs per block of 64 reflectors.
+// Wk: scratch of n_eig * 64 * 2 + 64 * 64 * 2 complex numbers.
+static int backtransform_wy(rpa_ctx* ctx, const cplx* Vh, const cplx* tau, int n, int n_eig, cplx* Y, cplx* Wk) {
+  const int NBK = 64;
+  cplx* W = Wk;
+  cplx* U = W + (size_t)n_eig * NBK;
+  cplx* G = U + (size_t)n_eig * NBK;
+  cplx* Tc = G + NBK * NBK;
+  const int nref = n - 1;
+  RPA_CUDA(ctx, cudaFuncSetAttribute(larft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+  for (int k0 = ((nref - 1) / NBK) * NBK; k0 >= 0; k0 -= NBK) {
+    const int nb = std::min(NBK, nref - k0);
+    const cplx* Vb = Vh + (long long)k0 * n;
+    int rc;
+    ZgemmParams g;   // G = Vb Vb^H
+    g.A = Vb; g.lda = n; g.a_km = false; g.B = Vb; g.ldb = n; g.b_kn = false; g.C = G; g.ldc = NBK;
+    g.M = nb; g.N = nb; g.K = n; g.conj_b = true; g.herm = true;
+    if ((rc = zgemm_dmma(ctx, g))) return rc;
+    larft_kernel<<<1, 256, (64 * 65 + 64) * sizeof(cplx), ctx->stream>>>(G, NBK, tau + k0, nb, Tc, NBK);
+    RPA_LAUNCH_CHECK(ctx);
+    ZgemmParams w;   // W[i][r] = sum_j Y[i][j] conj(Vb[r][j])  = (V^H y_i)[r]
+    w.A = Y; w.lda = n; w.a_km = false; w.B = Vb; w.ldb = n; w.b_kn = false; w.C = W; w.ldc = NBK;
+    w.M = n_eig; w.N = nb; w.K = n; w.conj_b = true;
+    if ((rc = zgemm_dmma(ctx, w))) return rc;
+    ZgemmParams u;   // U[i][r] = sum_s W[i][s] T[r][s]  (B = conj(T), conjugated again by the kernel)
+    u.A = W; u.lda = NBK; u.a_km = false; u.B = Tc; u.ldb = NBK; u.b_kn = false; u.C = U; u.ldc = NBK;
+    u.M = n_eig; u.N = nb; u.K = nb; u.conj_b = true; u.split_k = 1;
+    if ((rc = zgemm_dmma(ctx, u))) return rc;
+    ZgemmParams y;   // Y[i][j] -= sum_r U[i][r] Vb[r][j]
+    y.A = U; y.lda = NBK; y.a_km = false; y.B = Vb; y.ldb = n; y.b_kn = true; y.C = Y; y.ldc = n;
+    y.M = n_eig; y.N = n; y.K = nb; y.conj_b = false; y.accumulate = true; y.alpha = -1.0; y.split_k = 1;
+    if ((rc = zgemm_dmma(ctx, y))) return rc;
+  }
+  return RPA_OK;
+}
+
 size_t tridiag_workspace_bytes(int n, int n_eig) {
-  return ws_round((size_t)n * sizeof(cplx)) * 2 + ws_round((size_t)n * sizeof(double)) * 2 + 1024;
+  size_t b = ws_round((size_t)n * sizeof(cplx)) * 2 + ws_round((size_t)n * sizeof(double)) * 2 + 1024;
+  if ((size_t)6 * n * IV_NT * sizeof(double) > 200 * 1024) b += ws_round((size_t)6 * n * n_eig * sizeof(double));   // II factors in global memory
+  if (n >= 1024) b += ws_round(((size_t)2 * n_eig * 64 + 2 * 64 * 64) * sizeof(cplx));                      // blocked back-transformation
+  return b;
 }
 
 // H (n x n Hermitian, row-major, leading dimension ld, not modified) -> C [n_eig][n] (rows = eigenvectors of the n_eig
@@ -278,32 +355,50 @@ size_t tridiag_workspace_bytes(int n, int n_eig) {
 // Abuf, Vbuf: n x n scratch each.  Returns RPA_OK, or a negative code (the caller may fall back to Jacobi).
 int tridiag_eigh_lowest(rpa_ctx* ctx, WsAlloc& ws, const cplx* H, long long ld, int n, int n_eig, cplx* Abuf, cplx* Vbuf, cplx* C,
                         double* lambda) {
+  const bool iv_smem = (size_t)6 * n * sizeof(double) <= 190 * 1024;
+  const bool wy = n >= 1024;
   cplx* tau = ws.get<cplx>(n);
   cplx* p = ws.get<cplx>(n);
   double* d = ws.get<double>(n);
   double* e = ws.get<double>(n);
   double* tnorm = ws.get<double>(8);
+  double* iws = iv_smem ? nullptr : ws.get<double>((size_t)6 * n * n_eig);
+  cplx* Wk = wy ? ws.get<cplx>((size_t)2 * n_eig * 64 + 2 * 64 * 64) : nullptr;
   if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_subspace_basis: workspace too small (need %zu bytes)", ws.off);
   RPA_CUDA(ctx, cudaMemcpy2DAsync(Abuf, (size_t)n * sizeof(cplx), H, (size_t)ld * sizeof(cplx), (size_t)n * sizeof(cplx), n,
                                   cudaMemcpyDeviceToDevice, ctx->stream));
   int coop = 0, per_sm = 0;
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device);
-  const size_t smem1 = (size_t)2 * n * sizeof(cplx);
-  if (!coop || smem1 > 96 * 1024 || (size_t)6 * n * IV_NT * sizeof(double) > 200 * 1024) return RPA_ERR_INVALID;
-  const void* fn = (const void*)hetrd_kernel;
-  RPA_CUDA(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+  const bool w_smem = (size_t)2 * n * sizeof(cplx) <= 190 * 1024;
+  const size_t smem1 = (size_t)(w_smem ? 2 : 1) * n * sizeof(cplx);
+  if (!coop || smem1 > 200 * 1024 || (size_t)2 * n * sizeof(double) > 200 * 1024) return RPA_ERR_INVALID;
+  const void* fn = w_smem ? (const void*)hetrd_kernel<true> : (const void*)hetrd_kernel<false>;
+  RPA_CUDA(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 256, smem1) != cudaSuccess || per_sm < 1) return RPA_ERR_INVALID;
   const int grid = std::min(ctx->sm_count * std::min(per_sm, 2), (n + 7) / 8);
   cplx* A_ = Abuf; int n_ = n; cplx* V_ = Vbuf; cplx* tau_ = tau; double* d_ = d; double* e_ = e; cplx* p_ = p;
   void* args[] = {&A_, &n_, &V_, &tau_, &d_, &e_, &p_};
   RPA_CUDA(ctx, cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(256), args, smem1, ctx->stream));
   ctx->launches++;
+  RPA_CUDA(ctx, cudaFuncSetAttribute(bisect_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
   bisect_kernel<<<(n_eig + 7) / 8, 256, (size_t)2 * n * sizeof(double), ctx->stream>>>(d, e, n, n_eig, lambda, tnorm);
   RPA_LAUNCH_CHECK(ctx);
-  const size_t smem3 = (size_t)6 * n * IV_NT * sizeof(double);
-  RPA_CUDA(ctx, cudaFuncSetAttribute(invit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-  invit_kernel<<<(n_eig + IV_NT - 1) / IV_NT, 32, smem3, ctx->stream>>>(d, e, n, n_eig, lambda, tnorm, C);
+  if (iv_smem) {
+    const int nt = IV_NT;
+    const size_t smem3 = (size_t)6 * n * nt * sizeof(double);
+    if (smem3 <= 200 * 1024) {
+      RPA_CUDA(ctx, cudaFuncSetAttribute(invit_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+      invit_kernel<true><<<(n_eig + nt - 1) / nt, 32, smem3, ctx->stream>>>(d, e, n, n_eig, lambda, tnorm, nullptr, C);
+    } else {   // IV_NT vectors do not fit: one per CTA would waste the SMs, use global memory instead
+      iws = ws.get<double>((size_t)6 * n * n_eig);
+      if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_subspace_basis: workspace too small (need %zu bytes)", ws.off);
+      invit_kernel<false><<<(n_eig + 127) / 128, 128, 0, ctx->stream>>>(d, e, n, n_eig, lambda, tnorm, iws, C);
+    }
+  } else {
+    invit_kernel<false><<<(n_eig + 127) / 128, 128, 0, ctx->stream>>>(d, e, n, n_eig, lambda, tnorm, iws, C);
+  }
   RPA_LAUNCH_CHECK(ctx);
+  if (wy) return backtransform_wy(ctx, Vbuf, tau, n, n_eig, C, Wk);
   const size_t smem4 = (size_t)BT_NV * n * sizeof(cplx);
   RPA_CUDA(ctx, cudaFuncSetAttribute(backtransform_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
   backtransform_kernel<<<(n_eig + BT_NV - 1) / BT_NV, 256, smem4, ctx->stream>>>(Vbuf, tau, n, n_eig, C);
