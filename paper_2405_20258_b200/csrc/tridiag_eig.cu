@@ -1,10 +1,11 @@
-// Lowest eigenpairs of a small Hermitian matrix by the classical dense route, all on the device:
-//   (1) Householder tridiagonalisation  H = Q T Q^H  (unblocked, LAPACK zhetd2 'L' arithmetic) in ONE cooperative launch,
+// Lowest eigenpairs of a Hermitian matrix by the classical dense route, all on the device:
+//   (1) Householder tridiagonalisation  H = Q T Q^H  (unblocked, LAPACK zhetd2 'L' arithmetic) in ONE cooperative launch
+//       with one pass over the trailing matrix and one grid-wide barrier per column,
 //   (2) the n_eig smallest eigenvalues of the real symmetric tridiagonal T by bisection on the Sturm count,
 //   (3) their eigenvectors by inverse iteration (tridiagonal LU with partial pivoting),
-//   (4) back-transformation  c_i = Q z_i  (reflectors applied in reverse order),
-// followed, in basis.cu, by a CholeskyQR2 clean-up.  Used by the basis stage (a3) for n < 1024, where a
-// Jacobi sweep costs ~n dependent grid-wide rounds; here the only grid-wide dependencies are the 2 (n - 1) of step (1).
+//   (4) back-transformation  c_i = Q z_i  (reflectors applied in reverse order; compact-WY blocks + DMMA GEMMs for n >= 1024),
+// followed, in basis.cu, by a CholeskyQR clean-up.  Used by the basis stage (a3) whenever a part of the
+// spectrum is wanted (4 N_eig <= 3 n, n <= 12800): a Jacobi sweep costs ~n dependent grid-wide rounds and 12 n^3 flop.
 #include <algorithm>
 #include <cooperative_groups.h>
 
@@ -33,85 +34,185 @@ __device__ __forceinline__ void bsum(double (&v)[NV], double* sh /* [NV][8] */) 
 __device__ __forceinline__ cplx cmulf(cplx a, cplx b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 
 // (1) A: n x n Hermitian, row-major, both triangles (destroyed).  Vh[k][:] = reflector v_k (v_k[j] = 0 for j <= k,
-// v_k[k+1] = 1), tau[k]; T = tridiag(e, d, e).  256 threads per CTA, one warp per matrix row in the two O(m^2) phases.
-template <bool W_SMEM>
-__global__ void __launch_bounds__(256) hetrd_kernel(cplx* __restrict__ A, int n, cplx* __restrict__ Vh, cplx* __restrict__ tau,
-                                                    double* __restrict__ d, double* __restrict__ e, cplx* __restrict__ p) {
+// v_k[k+1] = 1), tau[k]; T = tridiag(e, d, e).  256 threads per CTA, one warp per matrix row in the O(m^2) phase.
+// Householder vector of x (x_0 = alpha, |x_1..|^2 = xn2), LAPACK zlarfg: H x = beta e_0, v = x / (alpha - beta) below the 1.
+struct Reflector { cplx tau, sc; double beta; };
+__device__ __forceinline__ Reflector make_reflector(double alr, double ali, double xn2) {
+  Reflector r;
+  r.tau = make_double2(0.0, 0.0); r.sc = make_double2(0.0, 0.0); r.beta = alr;
+  if (xn2 > 0.0 || ali != 0.0) {
+    const double nrm = sqrt(alr * alr + ali * ali + xn2);
+    r.beta = alr >= 0.0 ? -nrm : nrm;
+    r.tau = make_double2((r.beta - alr) / r.beta, -ali / r.beta);
+    const double dr = alr - r.beta, di = ali, den = dr * dr + di * di;     // 1 / (alpha - beta)
+    r.sc = make_double2(dr / den, -di / den);
+  }
+  return r;
+}
+
+// block-wide sums for any block size (<= 1024 threads), result in every thread
+template <int NV>
+__device__ __forceinline__ void bsumx(double (&v)[NV], double* sh /* [NV][32] */) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwc = blockDim.x >> 5;
+#pragma unroll
+  for (int k = 0; k < NV; k++) { v[k] = wsum(v[k]); if (lane == 0) sh[k * 32 + warp] = v[k]; }
+  __syncthreads();
+#pragma unroll
+  for (int k = 0; k < NV; k++) { double s = 0.0; for (int w = 0; w < nwc; w++) s += sh[k * 32 + w]; v[k] = s; }
+  __syncthreads();
+}
+// column chunks a row of the trailing matrix (m rows) is split into, so that all nw warps of the grid have work when
+// m < nw; each chunk leaves a partial sum of p_next (summed in a fixed order by the readers: deterministic)
+constexpr int HT_CMAX = 8;
+template <int MODE>
+__device__ __host__ __forceinline__ int ht_chunks(int m, int nw, int cmax) {
+  if (MODE != 0 || m < 1) return 1;                           // modes 1, 2 read p in the inner loop: one chunk
+  int c = nw / m;
+  c = c < m / 64 ? c : m / 64;                                // at least 64 columns per chunk
+  return c < 1 ? 1 : c > cmax ? cmax : c;
+}
+
+// (1') the same reduction with ONE pass over the trailing matrix and ONE grid-wide barrier per column: while a warp applies
+// the rank-2 update of column k to its row, it also accumulates that row's product with the NEXT reflector v_{k+1}, which
+// every CTA has formed beforehand from the updated row k+1 (one row: cheap, redundant).  MODE 0: v, v_next, w in shared
+// memory; 1: v, v_next (w_j = p_j + al2 v_j on the fly); 2: v_next only (v read back from Vh).
+template <int MODE>
+__global__ void __launch_bounds__(1024) hetrd_fused_kernel(cplx* __restrict__ A, int n, cplx* __restrict__ Vh, cplx* __restrict__ tau,
+                                                          double* __restrict__ d, double* __restrict__ e, cplx* __restrict__ P /* [2][HT_CMAX][n] */, int cmax) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  cplx* v = reinterpret_cast<cplx*>(smem_raw);   // [n]
-  cplx* w = v + n;                               // [n] (W_SMEM only; otherwise w_j = p_j + al2 v_j is formed on the fly)
-  __shared__ double sh[4 * 8];
+  cplx* buf0 = reinterpret_cast<cplx*>(smem_raw);            // v_next / v alternate between buf0 and buf1 (MODE 2: buf0 only)
+  cplx* buf1 = buf0 + n;
+  cplx* w = buf0 + 2 * n;                                    // MODE 0
+  __shared__ double sh[2 * 32];
   cg::grid_group grid = cg::this_grid();
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int gw = blockIdx.x * 8 + warp, nw = gridDim.x * 8;
-  for (int k = 0; k + 1 < n; k++) {
-    // ---- reflector of column k (every CTA, redundantly): x_i = A[i][k] = conj(A[k][i]), i > k
-    const cplx* rowk = A + (long long)k * n;
+  const int nthr = blockDim.x, nwc = nthr >> 5;
+  const int gw = blockIdx.x * nwc + warp, nw = gridDim.x * nwc;
+  if (n < 2) { if (blockIdx.x == 0 && tid == 0) { d[0] = A[0].x; e[0] = 0.0; } return; }
+  // ---- prologue: v_0 from row 0, p_0 = tau_0 A22 v_0
+  cplx* v = MODE == 2 ? nullptr : buf0;
+  cplx* vn = MODE == 2 ? buf0 : buf1;
+  cplx t;
+  {
     double s[1] = {0.0};
-    for (int i = k + 2 + tid; i < n; i += 256) { const cplx x = __ldcg(rowk + i); s[0] += x.x * x.x + x.y * x.y; }
-    bsum<1>(s, sh);
-    const cplx a0 = __ldcg(rowk + k + 1);
-    const double alr = a0.x, ali = -a0.y, xn2 = s[0];
-    cplx t = make_double2(0.0, 0.0), sc = make_double2(0.0, 0.0);
-    double beta = alr;
-    if (xn2 > 0.0 || ali != 0.0) {
-      const double nrm = sqrt(alr * alr + ali * ali + xn2);
-      beta = alr >= 0.0 ? -nrm : nrm;
-      t = make_double2((beta - alr) / beta, -ali / beta);
-      const double dr = alr - beta, di = ali, den = dr * dr + di * di;     // 1 / (alpha - beta)
-      sc = make_double2(dr / den, -di / den);
-    }
-    for (int i = tid; i < n; i += 256) {
+    for (int i = 2 + tid; i < n; i += nthr) { const cplx x = __ldcg(A + i); s[0] += x.x * x.x + x.y * x.y; }
+    bsumx<1>(s, sh);
+    const cplx a0 = __ldcg(A + 1);
+    const Reflector r = make_reflector(a0.x, -a0.y, s[0]);
+    t = r.tau;
+    cplx* v0 = buf0;
+    for (int i = tid; i < n; i += nthr) {
       cplx vi = make_double2(0.0, 0.0);
-      if (i == k + 1) vi = make_double2(1.0, 0.0);
-      else if (i > k + 1) { const cplx x = __ldcg(rowk + i); vi = cmulf(make_double2(x.x, -x.y), sc); }
-      v[i] = vi;
+      if (i == 1) vi = make_double2(1.0, 0.0);
+      else if (i > 1) { const cplx x = __ldcg(A + i); vi = cmulf(make_double2(x.x, -x.y), r.sc); }
+      v0[i] = vi;
     }
     __syncthreads();
     if (blockIdx.x == 0) {
-      for (int i = tid; i < n; i += 256) Vh[(long long)k * n + i] = v[i];
-      if (tid == 0) { tau[k] = t; e[k] = beta; d[k] = __ldcg(rowk + k).x; }
+      for (int i = tid; i < n; i += nthr) Vh[i] = v0[i];
+      if (tid == 0) { tau[0] = t; e[0] = r.beta; d[0] = __ldcg(A).x; }
     }
-    // ---- p = tau * A22 v  (warp per row)
-    for (int i = k + 1 + gw; i < n; i += nw) {
+    for (int i = 1 + gw; i < n; i += nw) {
       const cplx* ri = A + (long long)i * n;
       double pr = 0.0, pi = 0.0;
-      for (int j = k + 1 + lane; j < n; j += 32) { const cplx a = __ldcg(ri + j), b = v[j]; pr += a.x * b.x - a.y * b.y; pi += a.x * b.y + a.y * b.x; }
+      for (int j = 1 + lane; j < n; j += 32) { const cplx a = __ldcg(ri + j), b = v0[j]; pr += a.x * b.x - a.y * b.y; pi += a.x * b.y + a.y * b.x; }
       pr = wsum(pr); pi = wsum(pi);
-      if (lane == 0) p[i] = cmulf(t, make_double2(pr, pi));
-    }
-    grid.sync();
-    // ---- w = p - (tau/2) (p^H v) v  (every CTA, redundantly)
-    double q[2] = {0.0, 0.0};
-    for (int i = k + 1 + tid; i < n; i += 256) { const cplx x = __ldcg(p + i), b = v[i]; q[0] += x.x * b.x + x.y * b.y; q[1] += x.x * b.y - x.y * b.x; }
-    bsum<2>(q, sh);
-    const cplx al2 = cmulf(make_double2(-0.5 * t.x, -0.5 * t.y), make_double2(q[0], q[1]));
-    if (W_SMEM) {
-      for (int i = k + 1 + tid; i < n; i += 256) { const cplx x = __ldcg(p + i), av = cmulf(al2, v[i]); w[i] = make_double2(x.x + av.x, x.y + av.y); }
-    }
-    __syncthreads();
-    auto wval = [&](int i) -> cplx {
-      if (W_SMEM) return w[i];
-      const cplx x = __ldcg(p + i), av = cmulf(al2, v[i]);
-      return make_double2(x.x + av.x, x.y + av.y);
-    };
-    // ---- A22 -= v w^H + w v^H  (warp per row)
-    if (t.x != 0.0 || t.y != 0.0) {
-      for (int i = k + 1 + gw; i < n; i += nw) {
-        cplx* ri = A + (long long)i * n;
-        const cplx vi = v[i], wi = wval(i);
-        for (int j = k + 1 + lane; j < n; j += 32) {
-          const cplx vj = v[j], wj = wval(j);
-          cplx a = __ldcg(ri + j);
-          a.x -= vi.x * wj.x + vi.y * wj.y + wi.x * vj.x + wi.y * vj.y;      // v_i conj(w_j) + w_i conj(v_j)
-          a.y -= vi.y * wj.x - vi.x * wj.y + wi.y * vj.x - wi.x * vj.y;
-          __stcg(ri + j, a);
-        }
-      }
+      if (lane == 0) P[i] = cmulf(t, make_double2(pr, pi));    // chunk 0 of buffer 0
     }
     grid.sync();
   }
-  if (blockIdx.x == 0 && tid == 0) { d[n - 1] = __ldcg(A + (long long)(n - 1) * n + (n - 1)).x; e[n - 1] = 0.0; }
+  for (int k = 0; k + 1 < n; k++) {
+    // p_k = sum of the partial sums the row chunks of the last pass left; p_{k+1} goes to the other half (CTAs are not in step)
+    const cplx* pk = P + (size_t)(k & 1) * HT_CMAX * n;
+    cplx* pnext = P + (size_t)((k + 1) & 1) * HT_CMAX * n;
+    const int cprev = k == 0 ? 1 : ht_chunks<MODE>(n - k - 1, nw, cmax), ccur = ht_chunks<MODE>(n - k - 2, nw, cmax);
+    auto pval = [&](int i) -> cplx {
+      cplx x = __ldcg(pk + i);
+      for (int c = 1; c < cprev; c++) { const cplx y = __ldcg(pk + (size_t)c * n + i); x.x += y.x; x.y += y.y; }
+      return x;
+    };
+    const cplx* vrow = Vh + (long long)k * n;                 // MODE 2: v_k as written by CTA 0 one barrier ago
+    auto vval = [&](int i) -> cplx { return MODE == 2 ? vrow[i] : v[i]; };
+    // ---- w = p - (tau/2) (p^H v) v
+    double q[2] = {0.0, 0.0};
+    for (int i = k + 1 + tid; i < n; i += nthr) {
+      const cplx x = pval(i), b = vval(i);
+      if (MODE == 0) w[i] = x;                                 // p stays in shared memory for the second loop (same thread)
+      q[0] += x.x * b.x + x.y * b.y; q[1] += x.x * b.y - x.y * b.x;
+    }
+    bsumx<2>(q, sh);
+    const cplx al2 = cmulf(make_double2(-0.5 * t.x, -0.5 * t.y), make_double2(q[0], q[1]));
+    if (MODE == 0) {
+      for (int i = k + 1 + tid; i < n; i += nthr) { const cplx x = w[i], av = cmulf(al2, v[i]); w[i] = make_double2(x.x + av.x, x.y + av.y); }
+      __syncthreads();
+    }
+    auto wval = [&](int i) -> cplx {
+      if (MODE == 0) return w[i];
+      const cplx x = pval(i), av = cmulf(al2, vval(i));
+      return make_double2(x.x + av.x, x.y + av.y);
+    };
+    const bool upd = t.x != 0.0 || t.y != 0.0;
+    auto updated = [&](cplx a, cplx vi, cplx wi, cplx vj, cplx wj) -> cplx {   // a - v_i conj(w_j) - w_i conj(v_j)
+      if (upd) {
+        a.x -= vi.x * wj.x + vi.y * wj.y + wi.x * vj.x + wi.y * vj.y;
+        a.y -= vi.y * wj.x - vi.x * wj.y + wi.y * vj.x - wi.x * vj.y;
+      }
+      return a;
+    };
+    // ---- the updated row k+1 -> next reflector (every CTA, redundantly)
+    const int k1 = k + 1;
+    cplx tn = make_double2(0.0, 0.0);
+    {
+      const cplx* r1 = A + (long long)k1 * n;
+      const cplx vi = vval(k1), wi = wval(k1);
+      double s[1] = {0.0};
+      for (int j = k1 + tid; j < n; j += nthr) {
+        const cplx a = updated(__ldcg(r1 + j), vi, wi, vval(j), wval(j));
+        vn[j] = a;
+        if (j >= k1 + 2) s[0] += a.x * a.x + a.y * a.y;
+      }
+      bsumx<1>(s, sh);                                          // (its barriers also order the vn writes)
+      const double dk1 = vn[k1].x;
+      Reflector r; r.tau = make_double2(0.0, 0.0); r.sc = r.tau; r.beta = 0.0;
+      if (k1 + 1 < n) { const cplx a0 = vn[k1 + 1]; r = make_reflector(a0.x, -a0.y, s[0]); }
+      tn = r.tau;
+      __syncthreads();
+      for (int i = tid; i < n; i += nthr) {
+        cplx vi2 = make_double2(0.0, 0.0);
+        if (i == k1 + 1) vi2 = make_double2(1.0, 0.0);
+        else if (i > k1 + 1) { const cplx x = vn[i]; vi2 = cmulf(make_double2(x.x, -x.y), r.sc); }
+        vn[i] = vi2;
+      }
+      __syncthreads();
+      if (blockIdx.x == 0) {
+        if (k1 + 1 < n) for (int i = tid; i < n; i += nthr) Vh[(long long)k1 * n + i] = vn[i];
+        if (tid == 0) { d[k1] = dk1; e[k1] = k1 + 1 < n ? r.beta : 0.0; if (k1 + 1 < n) tau[k1] = tn; }
+      }
+    }
+    if (k1 + 1 >= n) break;
+    // ---- A22 -= v w^H + w v^H and p_next = tau_next A22' v_next in the same pass (warp per row; row k+1 is dead)
+    const int m = n - k1 - 1, clen = ((m + ccur - 1) / ccur + 31) & ~31;     // rows (= columns) k1+1 .. n-1 in ccur column chunks
+    for (long long task = gw; task < (long long)m * ccur; task += nw) {
+      const int i = k1 + 1 + (int)(task / ccur), c = (int)(task % ccur);
+      const int j0 = k1 + 1 + c * clen, j1 = min(n, j0 + clen);
+      cplx* ri = A + (long long)i * n;
+      const cplx vi = vval(i), wi = wval(i);
+      double pr = 0.0, pi = 0.0;
+#pragma unroll 4
+      for (int j = j0 + lane; j < j1; j += 32) {
+        const cplx a = updated(__ldcg(ri + j), vi, wi, vval(j), wval(j));
+        __stcg(ri + j, a);
+        const cplx b = vn[j];
+        pr += a.x * b.x - a.y * b.y; pi += a.x * b.y + a.y * b.x;
+      }
+      pr = wsum(pr); pi = wsum(pi);
+      if (lane == 0) pnext[(size_t)c * n + i] = cmulf(tn, make_double2(pr, pi));
+    }
+    grid.sync();
+    t = tn;
+    if (MODE == 2) { /* v_next stays in buf0; v is read from Vh */ }
+    else { cplx* tmp = v; v = vn; vn = tmp; }
+  }
 }
 
 }  // namespace
@@ -344,7 +445,7 @@ static int backtransform_wy(rpa_ctx* ctx, const cplx* Vh, const cplx* tau, int n
 }
 
 size_t tridiag_workspace_bytes(int n, int n_eig) {
-  size_t b = ws_round((size_t)n * sizeof(cplx)) * 2 + ws_round((size_t)n * sizeof(double)) * 2 + 1024;
+  size_t b = ws_round((size_t)n * sizeof(cplx)) + ws_round((size_t)2 * HT_CMAX * n * sizeof(cplx)) + ws_round((size_t)n * sizeof(double)) * 2 + 1024;
   if ((size_t)6 * n * IV_NT * sizeof(double) > 200 * 1024) b += ws_round((size_t)6 * n * n_eig * sizeof(double));   // II factors in global memory
   if (n >= 1024) b += ws_round(((size_t)2 * n_eig * 64 + 2 * 64 * 64) * sizeof(cplx));                      // blocked back-transformation
   return b;
@@ -358,7 +459,7 @@ int tridiag_eigh_lowest(rpa_ctx* ctx, WsAlloc& ws, const cplx* H, long long ld, 
   const bool iv_smem = (size_t)6 * n * sizeof(double) <= 190 * 1024;
   const bool wy = n >= 1024;
   cplx* tau = ws.get<cplx>(n);
-  cplx* p = ws.get<cplx>(n);
+  cplx* p = ws.get<cplx>((size_t)2 * HT_CMAX * n);
   double* d = ws.get<double>(n);
   double* e = ws.get<double>(n);
   double* tnorm = ws.get<double>(8);
@@ -369,16 +470,24 @@ int tridiag_eigh_lowest(rpa_ctx* ctx, WsAlloc& ws, const cplx* H, long long ld, 
                                   cudaMemcpyDeviceToDevice, ctx->stream));
   int coop = 0, per_sm = 0;
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device);
-  const bool w_smem = (size_t)2 * n * sizeof(cplx) <= 190 * 1024;
-  const size_t smem1 = (size_t)(w_smem ? 2 : 1) * n * sizeof(cplx);
-  if (!coop || smem1 > 200 * 1024 || (size_t)2 * n * sizeof(double) > 200 * 1024) return RPA_ERR_INVALID;
-  const void* fn = w_smem ? (const void*)hetrd_kernel<true> : (const void*)hetrd_kernel<false>;
+  const size_t row = (size_t)n * sizeof(cplx), cap = 200 * 1024;
+  int mode = 3 * row <= cap ? 0 : 2 * row <= cap ? 1 : 2;   // what of v, v_next, w fits in shared memory
+  if (const char* m = getenv("RPA_HETRD_MODE")) mode = std::max(mode, std::min(2, atoi(m)));   // tests: the large-n variants on small matrices
+  const size_t smem1 = (size_t)(3 - mode) * row;
+  if (!coop || smem1 > cap) return RPA_ERR_INVALID;
+  const void* fn = mode == 0 ? (const void*)hetrd_fused_kernel<0> : mode == 1 ? (const void*)hetrd_fused_kernel<1> : (const void*)hetrd_fused_kernel<2>;
   RPA_CUDA(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 256, smem1) != cudaSuccess || per_sm < 1) return RPA_ERR_INVALID;
-  const int grid = std::min(ctx->sm_count * std::min(per_sm, 2), (n + 7) / 8);
+  // large matrices stream from HBM: one CTA of 32 warps per SM (the shared-memory rows allow no second CTA); small ones are
+  // bound by the barrier latency: few small CTAs
+  int nthr = n > 3072 ? 1024 : n > 1536 ? 512 : 256;
+  if (const char* m = getenv("RPA_HETRD_THREADS")) nthr = std::max(64, std::min(1024, atoi(m) & ~31));
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, nthr, smem1) != cudaSuccess || per_sm < 1) return RPA_ERR_INVALID;
+  const int grid = std::min(ctx->sm_count * std::min(per_sm, 2), (n + nthr / 32 - 1) / (nthr / 32));
   cplx* A_ = Abuf; int n_ = n; cplx* V_ = Vbuf; cplx* tau_ = tau; double* d_ = d; double* e_ = e; cplx* p_ = p;
-  void* args[] = {&A_, &n_, &V_, &tau_, &d_, &e_, &p_};
-  RPA_CUDA(ctx, cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(256), args, smem1, ctx->stream));
+  int cmax = HT_CMAX;
+  if (const char* m = getenv("RPA_HETRD_CMAX")) cmax = std::max(1, std::min(HT_CMAX, atoi(m)));
+  void* args[] = {&A_, &n_, &V_, &tau_, &d_, &e_, &p_, &cmax};
+  RPA_CUDA(ctx, cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(nthr), args, smem1, ctx->stream));
   ctx->launches++;
   RPA_CUDA(ctx, cudaFuncSetAttribute(bisect_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
   bisect_kernel<<<(n_eig + 7) / 8, 256, (size_t)2 * n * sizeof(double), ctx->stream>>>(d, e, n, n_eig, lambda, tnorm);

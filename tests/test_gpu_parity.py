@@ -185,6 +185,15 @@ def test_subspace_basis_block_jacobi(n, n_eig, monkeypatch):
     check_basis(n, n_eig)
 
 
+@pytest.mark.parametrize("mode,threads,n,n_eig", [(1, 256, 147, 60), (2, 256, 300, 40), (2, 1024, 333, 100), (0, 1024, 691, 300)])
+def test_subspace_basis_tridiagonal_variants(mode, threads, n, n_eig, monkeypatch):
+    """The tridiagonalisation kernel's large-matrix variants (w formed on the fly, v read back from global memory,
+    32-warp CTAs) forced on small matrices, where the oracle's eigensolver is cheap."""
+    monkeypatch.setenv("RPA_HETRD_MODE", str(mode))
+    monkeypatch.setenv("RPA_HETRD_THREADS", str(threads))
+    check_basis(n, n_eig)
+
+
 def check_basis(n, n_eig):
     import paper_2405_20258_b200 as rpa
     import torch
