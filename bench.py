@@ -327,7 +327,7 @@ def main():
              "chi0": "zgemm_dmma_kernel<1,1,1,3> (CHI_SUM a2)", "proj": "zgemm_dmma_kernel<0,0,1,2> (projection a4)",
              "chis": "zgemm_dmma_kernel<1,1,1,3> batched over omega (chi_s a4)",
              "basis": "jacobi_persistent_kernel (a3: one-sided Jacobi of chi~0(0), all sweeps in one cooperative launch)" if jkind == 0
-             else "hetrd_kernel + bisect/invit/backtransform kernels (a3: tridiagonalisation route for the lowest N_eig eigenpairs)" if jkind == 2
+             else "hetrd_fused_kernel + bisect/invit/backtransform kernels (a3: tridiagonalisation route for the lowest N_eig eigenpairs)" if jkind == 2
              else "block Jacobi of chi~0(0) (a3: batched zgemm_dmma Gram + pair_rotations_kernel + batched zgemm_dmma update)"}
     tr = traffic_tab.get(f"{dom}:cfg{args.config}")
     if kwork[dom][0] == "B":

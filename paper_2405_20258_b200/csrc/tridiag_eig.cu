@@ -67,7 +67,7 @@ constexpr int HT_CMAX = 8;
 template <int MODE>
 __device__ __host__ __forceinline__ int ht_chunks(int m, int nw, int cmax) {
   if (MODE != 0 || m < 1) return 1;                           // modes 1, 2 read p in the inner loop: one chunk
-  int c = nw / m;
+  int c = nw / m;                                             // (balancing the rounds of the slowest warp instead was slower)
   c = c < m / 64 ? c : m / 64;                                // at least 64 columns per chunk
   return c < 1 ? 1 : c > cmax ? cmax : c;
 }
@@ -482,7 +482,8 @@ int tridiag_eigh_lowest(rpa_ctx* ctx, WsAlloc& ws, const cplx* H, long long ld, 
   int nthr = n > 3072 ? 1024 : n > 1536 ? 512 : 256;
   if (const char* m = getenv("RPA_HETRD_THREADS")) nthr = std::max(64, std::min(1024, atoi(m) & ~31));
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, nthr, smem1) != cudaSuccess || per_sm < 1) return RPA_ERR_INVALID;
-  const int grid = std::min(ctx->sm_count * std::min(per_sm, 2), (n + nthr / 32 - 1) / (nthr / 32));
+  // small matrices: no more warps than rows (a cheaper barrier); large ones: every SM (rows are split into chunks when warps > rows)
+  const int grid = nthr > 256 ? ctx->sm_count * per_sm : std::min(ctx->sm_count * std::min(per_sm, 2), (n + 7) / 8);
   cplx* A_ = Abuf; int n_ = n; cplx* V_ = Vbuf; cplx* tau_ = tau; double* d_ = d; double* e_ = e; cplx* p_ = p;
   int cmax = HT_CMAX;
   if (const char* m = getenv("RPA_HETRD_CMAX")) cmax = std::max(1, std::min(HT_CMAX, atoi(m)));
