@@ -324,8 +324,8 @@ def main():
     kd = kernels[dom]
     names = {"mtxel_plane": "pair_plane_fft8_kernel (MTXEL a1: pair product + pruned xy transforms)",
              "mtxel_z": "fft_axis_kernel<false,1> (MTXEL a1: z transform + sphere gather)",
-             "chi0": "zgemm_dmma_kernel<1,1,1,3> (CHI_SUM a2)", "proj": "zgemm_dmma_kernel<0,0,1,2> (projection a4)",
-             "chis": "zgemm_dmma_kernel<1,1,1,3> batched over omega (chi_s a4)",
+             "chi0": "zgemm_dmma_kernel<1,1,1,3,1> (CHI_SUM a2)", "proj": "zgemm_dmma_kernel<0,0,1,2,0> (projection a4)",
+             "chis": "zgemm_dmma_kernel<1,1,1,3,1> batched over omega (chi_s a4)",
              "basis": "jacobi_persistent_kernel (a3: one-sided Jacobi of chi~0(0), all sweeps in one cooperative launch)" if jkind == 0
              else "hetrd_fused_kernel + bisect/invit/backtransform kernels (a3: tridiagonalisation route for the lowest N_eig eigenpairs)" if jkind == 2
              else "block Jacobi of chi~0(0) (a3: batched zgemm_dmma Gram + pair_rotations_kernel + batched zgemm_dmma update)"}

@@ -73,7 +73,56 @@ __device__ __forceinline__ void load_tile(cplx* s, const cplx* g, long long ld, 
   }
 }
 
-template <bool A_KM, bool B_KN, bool CONJ_B, int STAGES>
+// The DMMAs of one warp on one staged k-tile.  MODE 0: a 4 x 4 block of 8 x 8 fragments at (mb, nb) (the 32 x 32 warp
+// tile).  MODE 1: a 3 x 3 block at (mb, nb).  MODE 2: three 2 x 2 lower fragment triangles on the diagonal at 0, 24, 48
+// (slot [t][0] = (24t, 24t), [t][1] = (24t+8, 24t), [t][2] = (24t+8, 24t+8)).  Modes 1 and 2 tile the 36 fragments on or
+// below the diagonal of a diagonal Hermitian tile, 9 per warp (see the kernel).
+template <bool A_KM, bool B_KN, bool CONJ_B, int MODE>
+__device__ __forceinline__ void mma_ktile(const cplx* __restrict__ a_s, const cplx* __restrict__ b_s,
+                                          const double* __restrict__ w_s, int g, int q, int mb, int nb,
+                                          double (&cre)[4][4][2], double (&cim)[4][4][2]) {
+  constexpr int NA = MODE == 0 ? 4 : (MODE == 1 ? 3 : 6);   // fragments loaded per operand
+#pragma unroll
+  for (int k4 = 0; k4 < BK / 4; k4++) {
+    const int k = k4 * 4 + q;
+    const double w = w_s[k];
+    double ar[NA], ai[NA], br[NA], bi[NA];
+#pragma unroll
+    for (int i = 0; i < NA; i++) {
+      const int m = MODE == 2 ? 24 * (i >> 1) + 8 * (i & 1) + g : mb + i * 8 + g;
+      cplx a = A_KM ? a_s[k * LD_KM + m] : a_s[m * LD_MK + k];
+      ar[i] = a.x * w; ai[i] = a.y * w;
+    }
+#pragma unroll
+    for (int j = 0; j < NA; j++) {
+      const int n = MODE == 2 ? 24 * (j >> 1) + 8 * (j & 1) + g : nb + j * 8 + g;
+      cplx b = B_KN ? b_s[k * LD_KM + n] : b_s[n * LD_MK + k];
+      br[j] = b.x; bi[j] = b.y;
+    }
+    // a conj(b): re += ar br + ai bi, im += ai br - ar bi;  a b: re += ar br - ai bi, im += ai br + ar bi.  The sign is
+    // a compile-time negation of the A operand, which DMMA takes as an operand modifier (no FP64 instruction).
+    constexpr int NS = MODE == 0 ? 4 : 3;
+#pragma unroll
+    for (int i = 0; i < NS; i++)
+#pragma unroll
+      for (int j = 0; j < NS; j++) {
+        const int ia = MODE == 2 ? 2 * i + (j >= 1) : i, jb = MODE == 2 ? 2 * i + (j == 2) : j;
+        dmma(cre[i][j][0], cre[i][j][1], ar[ia], br[jb]);
+        dmma(cim[i][j][0], cim[i][j][1], ai[ia], br[jb]);
+      }
+#pragma unroll
+    for (int i = 0; i < NS; i++)
+#pragma unroll
+      for (int j = 0; j < NS; j++) {
+        const int ia = MODE == 2 ? 2 * i + (j >= 1) : i, jb = MODE == 2 ? 2 * i + (j == 2) : j;
+        dmma(cre[i][j][0], cre[i][j][1], CONJ_B ? ai[ia] : -ai[ia], bi[jb]);
+        dmma(cim[i][j][0], cim[i][j][1], CONJ_B ? -ar[ia] : ar[ia], bi[jb]);
+      }
+  }
+}
+
+// HERM: compiled for Hermitian updates (p.herm set): only then do the diagonal-tile modes exist in the main loop.
+template <bool A_KM, bool B_KN, bool CONJ_B, int STAGES, bool HERM>
 __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int TA = A_KM ? TILE_KM : TILE_MK;
@@ -121,11 +170,16 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
     }
   };
 
-  // In a diagonal tile of a Hermitian update the warp (wm, wn) = (0, 1) owns rows 0..31 x columns 32..63: all above the
-  // diagonal, mirrored from the lower triangle in the epilogue.  It keeps loading and synchronising but issues no DMMA,
-  // which leaves the FP64 pipe to the other CTA resident on the SM.
-  const bool upper_only = p.herm && tm == tn && wm == 0 && wn == 1;
-  const bool diag_warp = p.herm && tm == tn && wm == wn;   // its own diagonal block: fragments with j > i are above the diagonal
+  // A diagonal tile of a Hermitian update stores only its lower triangle: 36 of its 64 8 x 8 fragments (the upper ones
+  // are mirrored in the epilogue).  Its four warps share them 9 each instead of keeping their 32 x 32 blocks, so the
+  // CTA issues 9/16 of a full tile's DMMAs *and finishes in 9/16 of its time*: warp 0 takes the three 2 x 2 fragment
+  // triangles on the diagonal (mode 2), warps 1-3 the 3 x 3 blocks at fragment rows 2-4 x columns 0-2, rows 5-7 x
+  // columns 0-2 and rows 5-7 x columns 3-5 (mode 1).
+  int mode = 0, mb = wm * 32, nb = wn * 32;
+  if (HERM && tm == tn) {
+    if (warp == 0) { mode = 2; mb = nb = 0; }
+    else { mode = 1; mb = warp == 1 ? 16 : 40; nb = warp == 3 ? 24 : 0; }
+  }
   double cre[4][4][2], cim[4][4][2];
 #pragma unroll
   for (int i = 0; i < 4; i++)
@@ -147,46 +201,12 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
       cp_async_commit();
     }
     const int st = it % STAGES;
-    if (upper_only) continue;   // this warp's 32 x 32 block lies strictly above the diagonal of a Hermitian tile: never stored
     const cplx* a_s = sA + st * TA;
     const cplx* b_s = sB + st * TB;
     const double* w_s = sW + st * BK;
-#pragma unroll
-    for (int k4 = 0; k4 < BK / 4; k4++) {
-      const int k = k4 * 4 + q;
-      const double w = w_s[k];
-      double ar[4], ai[4], br[4], bi[4];
-#pragma unroll
-      for (int i = 0; i < 4; i++) {
-        const int m = wm * 32 + i * 8 + g;
-        cplx a = A_KM ? a_s[k * LD_KM + m] : a_s[m * LD_MK + k];
-        ar[i] = a.x * w; ai[i] = a.y * w;
-      }
-#pragma unroll
-      for (int j = 0; j < 4; j++) {
-        const int n = wn * 32 + j * 8 + g;
-        cplx b = B_KN ? b_s[k * LD_KM + n] : b_s[n * LD_MK + k];
-        br[j] = b.x; bi[j] = b.y;
-      }
-      // a conj(b): re += ar br + ai bi, im += ai br - ar bi;  a b: re += ar br - ai bi, im += ai br + ar bi.  The sign is
-      // a compile-time negation of the A operand, which DMMA takes as an operand modifier (no FP64 instruction).
-#pragma unroll
-      for (int i = 0; i < 4; i++)
-#pragma unroll
-        for (int j = 0; j < 4; j++) {
-          if (diag_warp && j > i) continue;   // 8 x 8 fragment strictly above the diagonal: never stored
-          dmma(cre[i][j][0], cre[i][j][1], ar[i], br[j]);
-          dmma(cim[i][j][0], cim[i][j][1], ai[i], br[j]);
-        }
-#pragma unroll
-      for (int i = 0; i < 4; i++)
-#pragma unroll
-        for (int j = 0; j < 4; j++) {
-          if (diag_warp && j > i) continue;
-          dmma(cre[i][j][0], cre[i][j][1], CONJ_B ? ai[i] : -ai[i], bi[j]);
-          dmma(cim[i][j][0], cim[i][j][1], CONJ_B ? -ar[i] : ar[i], bi[j]);
-        }
-    }
+    if (!HERM || mode == 0) mma_ktile<A_KM, B_KN, CONJ_B, 0>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+    else if (mode == 1) mma_ktile<A_KM, B_KN, CONJ_B, 1>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+    else mma_ktile<A_KM, B_KN, CONJ_B, 2>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
   }
   cp_async_wait<0>();
 
@@ -194,14 +214,17 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
   const bool diag_tile = p.herm && (tm == tn);
 #pragma unroll
   for (int i = 0; i < 4; i++) {
-    const int r = m0 + wm * 32 + i * 8 + g;
-    if (r >= p.M) continue;
-    const double sr = p.alpha * (p.rs ? p.rs[r] : 1.0);
 #pragma unroll
     for (int j = 0; j < 4; j++) {
+      if (HERM && mode != 0 && (i == 3 || j == 3)) continue;   // 9 accumulator slots in the diagonal-tile modes
+      const int ro = HERM && mode == 2 ? 24 * i + (j >= 1 ? 8 : 0) : mb + i * 8;
+      const int co = HERM && mode == 2 ? 24 * i + (j == 2 ? 8 : 0) : nb + j * 8;
+      const int r = m0 + ro + g;
+      if (r >= p.M) continue;
+      const double sr = p.alpha * (p.rs ? p.rs[r] : 1.0);
 #pragma unroll
       for (int e = 0; e < 2; e++) {
-        const int c = n0 + wn * 32 + j * 8 + 2 * q + e;
+        const int c = n0 + co + 2 * q + e;
         if (c >= p.N) continue;
         const double sc = sr * (p.cs ? p.cs[c] : 1.0);
         double vr = sc * cre[i][j][e], vi = sc * cim[i][j][e];
@@ -235,13 +258,13 @@ __global__ void herm_mirror_kernel(cplx* C, long long ldc, long long strideC, in
   }
 }
 
-template <bool A_KM, bool B_KN, bool CONJ_B>
-int launch(rpa_ctx* ctx, const KArgs& ka, dim3 grid) {
+template <bool A_KM, bool B_KN, bool CONJ_B, bool HERM>
+int launch_h(rpa_ctx* ctx, const KArgs& ka, dim3 grid) {
   constexpr int STAGES = (A_KM || B_KN) ? 3 : 2;
   constexpr int TA = A_KM ? TILE_KM : TILE_MK;
   constexpr int TB = B_KN ? TILE_KM : TILE_MK;
   constexpr size_t smem = (size_t)STAGES * (TA + TB) * sizeof(cplx) + STAGES * BK * sizeof(double);
-  auto kern = zgemm_dmma_kernel<A_KM, B_KN, CONJ_B, STAGES>;
+  auto kern = zgemm_dmma_kernel<A_KM, B_KN, CONJ_B, STAGES, HERM>;
   static bool attr_set = false;
   if (!attr_set) {
     RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -250,6 +273,16 @@ int launch(rpa_ctx* ctx, const KArgs& ka, dim3 grid) {
   kern<<<grid, NTHREADS, smem, ctx->stream>>>(ka);
   RPA_LAUNCH_CHECK(ctx);
   return RPA_OK;
+}
+
+template <bool A_KM, bool B_KN, bool CONJ_B>
+int launch(rpa_ctx* ctx, const KArgs& ka, dim3 grid) {
+  if (ka.herm) {
+    // Hermitian updates come in two operand layouts only (CHI_SUM / chi_s: [k][m] x [k][n]; Gram matrices: [m][k] x [m][k])
+    if constexpr (A_KM == B_KN && CONJ_B) return launch_h<A_KM, B_KN, CONJ_B, true>(ctx, ka, grid);
+    else return rpa_fail(ctx, RPA_ERR_INVALID, "zgemm_dmma: Hermitian update in an operand layout not instantiated");
+  }
+  return launch_h<A_KM, B_KN, CONJ_B, false>(ctx, ka, grid);
 }
 
 }  // namespace
@@ -277,7 +310,25 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
     split = 1;
     int max_split = n_kt / 8;  // at least 8 k-tiles (128 k) per split
     if (base >= 8 * slots) max_split = std::min(max_split, 4);   // many waves already: only trim the last partial wave
-    if (max_split > 1 && base < 64 * slots) {
+    if (max_split > 1 && base < 8 * slots && !getenv("RPA_ZGEMM_COARSE_SPLIT")) {
+      // Few tiles (the contractions of the small configs, the Gram matrices of the basis stage): cut K finely and let the
+      // block scheduler balance.  Cost model in k-tiles of a full tile: the diagonal tiles of a Hermitian update issue
+      // 9/16 of the DMMAs, a CTA pays ~EPI k-tiles for the pipeline fill and the atomic epilogue, and the last CTAs to
+      // finish leave about 0.6 of a chunk idle.  (A single wave of equal CTAs would idle the slots it does not fill and
+      // those whose diagonal tiles finish early: 77 % -> 8x % of the DMMA peak for CHI_SUM at configs[1].)
+      const double EPI = 6.0;
+      const double w_tiles = p.herm ? (double)(tiles - tiles_m) + 0.5625 * tiles_m : (double)tiles;
+      const double W = w_tiles * p.batch * n_kt;
+      double best = 1e300;
+      for (int s = 1; s <= max_split && s <= 512; s++) {
+        const long long chunk = (n_kt + s - 1) / s;
+        const long long s_eff = (n_kt + chunk - 1) / chunk;
+        const long long ctas = base * s_eff;
+        double t = ctas <= slots ? (double)chunk : W / (double)slots + 0.6 * (double)chunk;
+        t += EPI * (double)((ctas + slots - 1) / slots);
+        if (t < best * (1.0 - 1e-3)) { best = t; split = s; }
+      }
+    } else if (max_split > 1 && base < 64 * slots) {
       double best = 0.0;
       for (int s = 1; s <= max_split && s <= 64; s++) {
         const long long ctas = base * s;
