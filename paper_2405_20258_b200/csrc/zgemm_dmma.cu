@@ -73,48 +73,48 @@ __device__ __forceinline__ void load_tile(cplx* s, const cplx* g, long long ld, 
   }
 }
 
-// The DMMAs of one warp on one staged k-tile.  MODE 0: a 4 x 4 block of 8 x 8 fragments at (mb, nb) (the 32 x 32 warp
-// tile).  MODE 1: a 3 x 3 block at (mb, nb).  MODE 2: three 2 x 2 lower fragment triangles on the diagonal at 0, 24, 48
-// (slot [t][0] = (24t, 24t), [t][1] = (24t+8, 24t), [t][2] = (24t+8, 24t+8)).  Modes 1 and 2 tile the 36 fragments on or
-// below the diagonal of a diagonal Hermitian tile, 9 per warp (see the kernel).
-template <bool A_KM, bool B_KN, bool CONJ_B, int MODE>
+// The DMMAs of one warp on one staged k-tile.  TRI = false: an NI x NJ block of 8 x 8 fragments at (mb, nb) -- 4 x 4 is
+// the 32 x 32 warp tile, 3 x 4 / 2 x 4 / 1 x 4 the warp's share of a ragged last tile row, 3 x 3 a share of a diagonal
+// Hermitian tile.  TRI = true: three 2 x 2 lower fragment triangles on the diagonal at 0, 24, 48 (slot [t][0] =
+// (24t, 24t), [t][1] = (24t+8, 24t), [t][2] = (24t+8, 24t+8)).  3 x 3 x 3 + TRI tile the 36 fragments on or below the
+// diagonal of a diagonal Hermitian tile, 9 per warp (see the kernel).
+template <bool A_KM, bool B_KN, bool CONJ_B, int NI, int NJ, bool TRI>
 __device__ __forceinline__ void mma_ktile(const cplx* __restrict__ a_s, const cplx* __restrict__ b_s,
                                           const double* __restrict__ w_s, int g, int q, int mb, int nb,
                                           double (&cre)[4][4][2], double (&cim)[4][4][2]) {
-  constexpr int NA = MODE == 0 ? 4 : (MODE == 1 ? 3 : 6);   // fragments loaded per operand
+  constexpr int NA = TRI ? 6 : NI, NB = TRI ? 6 : NJ;   // fragments loaded per operand
 #pragma unroll
   for (int k4 = 0; k4 < BK / 4; k4++) {
     const int k = k4 * 4 + q;
     const double w = w_s[k];
-    double ar[NA], ai[NA], br[NA], bi[NA];
+    double ar[NA], ai[NA], br[NB], bi[NB];
 #pragma unroll
     for (int i = 0; i < NA; i++) {
-      const int m = MODE == 2 ? 24 * (i >> 1) + 8 * (i & 1) + g : mb + i * 8 + g;
+      const int m = TRI ? 24 * (i >> 1) + 8 * (i & 1) + g : mb + i * 8 + g;
       cplx a = A_KM ? a_s[k * LD_KM + m] : a_s[m * LD_MK + k];
       ar[i] = a.x * w; ai[i] = a.y * w;
     }
 #pragma unroll
-    for (int j = 0; j < NA; j++) {
-      const int n = MODE == 2 ? 24 * (j >> 1) + 8 * (j & 1) + g : nb + j * 8 + g;
+    for (int j = 0; j < NB; j++) {
+      const int n = TRI ? 24 * (j >> 1) + 8 * (j & 1) + g : nb + j * 8 + g;
       cplx b = B_KN ? b_s[k * LD_KM + n] : b_s[n * LD_MK + k];
       br[j] = b.x; bi[j] = b.y;
     }
     // a conj(b): re += ar br + ai bi, im += ai br - ar bi;  a b: re += ar br - ai bi, im += ai br + ar bi.  The sign is
     // a compile-time negation of the A operand, which DMMA takes as an operand modifier (no FP64 instruction).
-    constexpr int NS = MODE == 0 ? 4 : 3;
 #pragma unroll
-    for (int i = 0; i < NS; i++)
+    for (int i = 0; i < NI; i++)
 #pragma unroll
-      for (int j = 0; j < NS; j++) {
-        const int ia = MODE == 2 ? 2 * i + (j >= 1) : i, jb = MODE == 2 ? 2 * i + (j == 2) : j;
+      for (int j = 0; j < NJ; j++) {
+        const int ia = TRI ? 2 * i + (j >= 1) : i, jb = TRI ? 2 * i + (j == 2) : j;
         dmma(cre[i][j][0], cre[i][j][1], ar[ia], br[jb]);
         dmma(cim[i][j][0], cim[i][j][1], ai[ia], br[jb]);
       }
 #pragma unroll
-    for (int i = 0; i < NS; i++)
+    for (int i = 0; i < NI; i++)
 #pragma unroll
-      for (int j = 0; j < NS; j++) {
-        const int ia = MODE == 2 ? 2 * i + (j >= 1) : i, jb = MODE == 2 ? 2 * i + (j == 2) : j;
+      for (int j = 0; j < NJ; j++) {
+        const int ia = TRI ? 2 * i + (j >= 1) : i, jb = TRI ? 2 * i + (j == 2) : j;
         dmma(cre[i][j][0], cre[i][j][1], CONJ_B ? ai[ia] : -ai[ia], bi[jb]);
         dmma(cim[i][j][0], cim[i][j][1], CONJ_B ? -ar[ia] : ar[ia], bi[jb]);
       }
@@ -180,6 +180,13 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
     if (warp == 0) { mode = 2; mb = nb = 0; }
     else { mode = 1; mb = warp == 1 ? 16 : 40; nb = warp == 3 ? 24 : 0; }
   }
+  // A ragged last tile row (M not a multiple of 64) has rv < 8 valid fragment rows: the two warp rows take ceil(rv / 2)
+  // of them each instead of 4 (N_eig = 300: 3, N_eig = 2400: 2), the rest of the tile is zero and never stored.
+  int ni = mode == 0 ? 4 : 3;
+  if (mode == 0 && p.M - m0 < BM - 8) {
+    ni = (((p.M - m0 + 7) >> 3) + 1) >> 1;
+    mb = wm * ni * 8;
+  }
   double cre[4][4][2], cim[4][4][2];
 #pragma unroll
   for (int i = 0; i < 4; i++)
@@ -204,9 +211,13 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
     const cplx* a_s = sA + st * TA;
     const cplx* b_s = sB + st * TB;
     const double* w_s = sW + st * BK;
-    if (!HERM || mode == 0) mma_ktile<A_KM, B_KN, CONJ_B, 0>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
-    else if (mode == 1) mma_ktile<A_KM, B_KN, CONJ_B, 1>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
-    else mma_ktile<A_KM, B_KN, CONJ_B, 2>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+    if (!HERM || mode == 0) {
+      if (ni == 4) mma_ktile<A_KM, B_KN, CONJ_B, 4, 4, false>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+      else if (ni == 3) mma_ktile<A_KM, B_KN, CONJ_B, 3, 4, false>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+      else if (ni == 2) mma_ktile<A_KM, B_KN, CONJ_B, 2, 4, false>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+      else mma_ktile<A_KM, B_KN, CONJ_B, 1, 4, false>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+    } else if (mode == 1) mma_ktile<A_KM, B_KN, CONJ_B, 3, 3, false>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+    else mma_ktile<A_KM, B_KN, CONJ_B, 3, 3, true>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
   }
   cp_async_wait<0>();
 
@@ -216,7 +227,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
   for (int i = 0; i < 4; i++) {
 #pragma unroll
     for (int j = 0; j < 4; j++) {
-      if (HERM && mode != 0 && (i == 3 || j == 3)) continue;   // 9 accumulator slots in the diagonal-tile modes
+      if (i >= ni || (HERM && mode != 0 && j == 3)) continue;   // accumulator slots this warp does not use
       const int ro = HERM && mode == 2 ? 24 * i + (j >= 1 ? 8 : 0) : mb + i * 8;
       const int co = HERM && mode == 2 ? 24 * i + (j == 2 ? 8 : 0) : nb + j * 8;
       const int r = m0 + ro + g;
