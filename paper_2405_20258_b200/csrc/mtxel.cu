@@ -339,8 +339,11 @@ namespace {
 
 struct MtxelSizes {
   int ncc;             // conduction bands per chunk
-  size_t u_v, u_c, t;  // bytes
+  size_t u_v, u_vp, u_c, t;  // bytes
 };
+
+int fft8_plane_size(const rpa_ctx* ctx);
+size_t fft8_lane_plane(int n8);
 
 MtxelSizes mtxel_sizes(const rpa_ctx* ctx, int nvb, int nc) {
   const MtxelPlan* mp = ctx->mtxel;
@@ -353,6 +356,8 @@ MtxelSizes mtxel_sizes(const rpa_ctx* ctx, int nvb, int nc) {
   MtxelSizes s;
   s.ncc = ncc;
   s.u_v = ws_round((size_t)nvb * n_r * sizeof(cplx));
+  // the valence functions once more, in the lane order of the fft8 plane kernels (pair_plane_fft8.cuh)
+  s.u_vp = ws_round((size_t)nvb * ctx->fft[2] * fft8_lane_plane(fft8_plane_size(ctx)) * sizeof(cplx));
   s.u_c = ws_round((size_t)ncc * n_r * sizeof(cplx));
   s.t = ws_round((size_t)nvb * ncc * ctx->fft[2] * J * sizeof(cplx));
   return s;
@@ -449,11 +454,29 @@ int fft8_plane_size(const rpa_ctx* ctx) {
   return smem <= 227 * 1024 ? N1 : 0;
 }
 
+// elements of one valence plane in lane order (0 = no fft8 kernel)
+size_t fft8_lane_plane(int n8) {
+  switch (n8) {
+    case 24: return fft8::Geo<24>::PP;
+    case 40: return fft8::Geo<40>::PP;
+    case 48: return fft8::Geo<48>::PP;
+    case 64: return fft8::Geo<64>::PP;
+    default: return 0;
+  }
+}
+
+template <int N>
+int launch_lane_order(rpa_ctx* ctx, const cplx* u_nat, cplx* u_lane, int nvb, int N3) {
+  fft8::uv_lane_order_kernel<N><<<dim3((unsigned)N3, (unsigned)nvb), fft8::Geo<N>::NWARP * 32, 0, ctx->stream>>>(u_nat, u_lane, N3);
+  RPA_LAUNCH_CHECK(ctx);
+  return RPA_OK;
+}
+
 }  // namespace
 
 size_t mtxel_workspace_bytes(const rpa_ctx* ctx, int nvb, int nc) {
   MtxelSizes s = mtxel_sizes(ctx, nvb, nc);
-  return s.u_v + s.u_c + s.t;
+  return s.u_v + s.u_vp + s.u_c + s.t;
 }
 
 int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx* psi_c, int nc, cplx* M) {
@@ -462,6 +485,8 @@ int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx*
   const long long n_r = ctx->n_r;
   const MtxelSizes sz = mtxel_sizes(ctx, nvb, nc);
   cplx* u_v = ws.get<cplx>((size_t)nvb * n_r);
+  const int n8 = ctx->force_generic_fft ? 0 : fft8_plane_size(ctx);
+  cplx* u_vp = n8 ? ws.get<cplx>((size_t)nvb * N3 * fft8_lane_plane(n8)) : nullptr;
   cplx* u_c = ws.get<cplx>((size_t)sz.ncc * n_r);
   const int nk1 = mp->ax[0].nk, nk2 = mp->ax[1].nk, nk3 = mp->ax[2].nk, J = nk1 * nk2;
   cplx* T = ws.get<cplx>((size_t)nvb * sz.ncc * N3 * J);
@@ -469,7 +494,6 @@ int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx*
 
   const int plane = N1 * N2, P1 = N1 | 1, P2 = N2 | 1;
   const size_t smem = ((size_t)2 * N1 * P2 + (size_t)2 * nk2 * P1) * sizeof(cplx) + (size_t)(nk1 + nk2) * sizeof(int);
-  const int n8 = ctx->force_generic_fft ? 0 : fft8_plane_size(ctx);
   if (n8 == 0 && smem > 227 * 1024)
     return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_mtxel: an xy plane of %d x %d does not fit in shared memory", N1, N2);
   // warps: about 32 lanes' worth of butterflies per warp in a radix-8 pass over its rows
@@ -483,7 +507,17 @@ int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx*
   RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
 
   int rc;
-  { ProfScope ps(ctx, RPA_PROF_MTXEL_WFN); rc = wfn_to_realspace(ctx, psi_v, nvb, u_v); }
+  {
+    ProfScope ps(ctx, RPA_PROF_MTXEL_WFN);
+    rc = wfn_to_realspace(ctx, psi_v, nvb, u_v);
+    if (!rc) switch (n8) {
+      case 24: rc = launch_lane_order<24>(ctx, u_v, u_vp, nvb, N3); break;
+      case 40: rc = launch_lane_order<40>(ctx, u_v, u_vp, nvb, N3); break;
+      case 48: rc = launch_lane_order<48>(ctx, u_v, u_vp, nvb, N3); break;
+      case 64: rc = launch_lane_order<64>(ctx, u_v, u_vp, nvb, N3); break;
+      default: break;
+    }
+  }
   if (rc) return rc;
   cplx* const u_c_scratch = u_c;
   const bool have_cache = ctx->uc_cache && ctx->uc_cache_src == psi_c && ctx->uc_cache_nc == nc;
@@ -500,10 +534,10 @@ int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx*
     if (rc) return rc;
     ProfScope* pp = new ProfScope(ctx, RPA_PROF_MTXEL_PLANE);
     switch (n8) {
-      case 24: rc = launch_fft8<24>(ctx, u_v, u_c, nvb, ncc, N3, mp, T); break;
-      case 40: rc = launch_fft8<40>(ctx, u_v, u_c, nvb, ncc, N3, mp, T); break;
-      case 48: rc = launch_fft8<48>(ctx, u_v, u_c, nvb, ncc, N3, mp, T); break;
-      case 64: rc = launch_fft8<64>(ctx, u_v, u_c, nvb, ncc, N3, mp, T); break;
+      case 24: rc = launch_fft8<24>(ctx, u_vp, u_c, nvb, ncc, N3, mp, T); break;
+      case 40: rc = launch_fft8<40>(ctx, u_vp, u_c, nvb, ncc, N3, mp, T); break;
+      case 48: rc = launch_fft8<48>(ctx, u_vp, u_c, nvb, ncc, N3, mp, T); break;
+      case 64: rc = launch_fft8<64>(ctx, u_vp, u_c, nvb, ncc, N3, mp, T); break;
       default:
         kern<<<(unsigned)(ncc * N3), nthr, smem, ctx->stream>>>(u_v, u_c, nvb, ncc, N1, N2, N3, mp->ax[0].fwd(),
                                                                 mp->ax[1].fwd(), mp->ax[0].d_kpos, mp->ax[1].d_kpos, nk1,

@@ -40,6 +40,12 @@ struct Geo {
   // valence bands per loop iteration: one block barrier per VB bands, and the VB x nk2 kept columns of an iteration
   // fill whole warps of the x transforms (bounded by shared memory: 2 CTAs/SM at N = 40, 1 at N = 48, 64)
   static constexpr int VB = N <= 24 ? 4 : (N <= 48 ? 3 : 1);
+  // Valence planes are read in LANE ORDER (uv_lane_order_kernel): the RW rows of warp w form a region of RW N elements
+  // at w RW N, and inside it element q of lane l sits at q QS + l -- so each of the 8 loads a lane issues per band is
+  // one contiguous run of RW R2 x 16 B per warp (4-5 L1 wavefronts) instead of RW runs of R2 x 16 B in RW different
+  // rows (~9 wavefronts: the LSU data pipe is this kernel's limiter).  PP = plane pitch in that layout.
+  static constexpr int QS = RW * R2;
+  static constexpr int PP = NWARP * RW * N;
   static constexpr int G = (R2 & 1) ? R2 : R2 + 1;   // pitch of an s-group in a pass-A output line (odd)
   static constexpr int LW = 8 * G;                   // length of a pass-A output line
   // pitches in 16-byte elements.  P = R2 (mod 8) makes (line, j) -> bank group linear in the lane index, so the
@@ -85,6 +91,7 @@ __device__ __forceinline__ void pair_plane_fft8_body(const cplx* __restrict__ u_
   const int z = blockIdx.x / ncc, c = blockIdx.x - z * ncc;
   constexpr int plane = N * N;
   const long long n_r = (long long)plane * N3;
+  const long long n_rp = (long long)GE::PP * N3;   // one valence band in lane order
   const cplx* ucp = u_c + (long long)c * n_r + (long long)z * plane;
   for (int idx = tid; idx < plane; idx += NTHR) {
     int x = idx / N, y = idx - x * N;
@@ -112,11 +119,11 @@ __device__ __forceinline__ void pair_plane_fft8_body(const cplx* __restrict__ u_
   cplx twj[8];
 #pragma unroll
   for (int s = 1; s < 8; s++) twj[s] = tw[(j * s) % N];
-  const cplx* uvp = u_v + (long long)z * plane + (long long)row * N + j;
+  const cplx* uvp = u_v + (long long)z * GE::PP + r0 * N + lane;   // lane order, see Geo
   cplx nxt[8];
   if (row_on) {
 #pragma unroll
-    for (int q = 0; q < 8; q++) nxt[q] = uvp[q * R2];
+    for (int q = 0; q < 8; q++) nxt[q] = uvp[q * GE::QS];
   }
   __syncthreads();
   const long long J = (long long)nk1 * nk2;
@@ -136,9 +143,9 @@ __device__ __forceinline__ void pair_plane_fft8_body(const cplx* __restrict__ u_
             x[q] = make_double2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x);   // conj(u_v) u_c
           }
           if (v0 + u + 1 < nvb) {
-            const cplx* nx = uvp + (long long)(v0 + u + 1) * n_r;
+            const cplx* nx = uvp + (long long)(v0 + u + 1) * n_rp;
 #pragma unroll
-            for (int q = 0; q < 8; q++) nxt[q] = nx[q * R2];
+            for (int q = 0; q < 8; q++) nxt[q] = nx[q * GE::QS];
           }
           fftsm::bfly8<false>(x);
           cplx* line = wk + row * PW + j;
@@ -254,6 +261,7 @@ __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict
   const int z = blockIdx.x / ncc, c = blockIdx.x - z * ncc;
   constexpr int plane = N * N;
   const long long n_r = (long long)plane * N3;
+  const long long n_rp = (long long)GE::PP * N3;   // one valence band in lane order
   const cplx* ucp = u_c + (long long)c * n_r + (long long)z * plane;
   for (int idx = tid; idx < plane; idx += NTHR) {
     int x = idx / N, y = idx - x * N;
@@ -281,11 +289,11 @@ __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict
   cplx twj[8];
 #pragma unroll
   for (int s = 1; s < 8; s++) twj[s] = tw[(j * s) % N];
-  const cplx* uvp = u_v + (long long)z * plane + (long long)row * N + j;
+  const cplx* uvp = u_v + (long long)z * GE::PP + r0 * N + lane;   // lane order, see Geo
   cplx nxt[8];
   if (row_on) {
 #pragma unroll
-    for (int q = 0; q < 8; q++) nxt[q] = uvp[q * R2];
+    for (int q = 0; q < 8; q++) nxt[q] = uvp[q * GE::QS];
   }
   __syncthreads();
   const long long J = (long long)nk1 * nk2;
@@ -345,9 +353,9 @@ __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict
         x[q] = make_double2(a.x * bb.x + a.y * bb.y, a.x * bb.y - a.y * bb.x);   // conj(u_v) u_c
       }
       if (it + 1 < nvb) {
-        const cplx* nx = uvp + (long long)(it + 1) * n_r;
+        const cplx* nx = uvp + (long long)(it + 1) * n_rp;
 #pragma unroll
-        for (int q = 0; q < 8; q++) nxt[q] = nx[q * R2];
+        for (int q = 0; q < 8; q++) nxt[q] = nx[q * GE::QS];
       }
       fftsm::bfly8<false>(x);
       cplx* line = wk + row * PW + j;
@@ -376,6 +384,22 @@ __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict
     if (it >= 1) cols(it - 1);
   }
   cols(nvb - 1);
+}
+
+// u_nat[v][z][x][y] (plane-major, as the wavefunction transforms leave it) -> u_lane[v][z][PP] in the lane order of the
+// plane kernels (Geo<N>::QS, PP).  One CTA of NWARP warps per (z, v) plane, the same lane roles as in the plane kernels.
+template <int N>
+__global__ void __launch_bounds__(Geo<N>::NWARP * 32) uv_lane_order_kernel(const cplx* __restrict__ u_nat, cplx* __restrict__ u_lane, int N3) {
+  using GE = Geo<N>;
+  constexpr int R2 = GE::R2, RW = GE::RW;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int ls = lane / R2, j = lane - ls * R2, r0 = warp * RW, row = r0 + ls;
+  if (lane >= RW * R2 || row >= N) return;
+  const long long pl = (long long)blockIdx.y * N3 + blockIdx.x;
+  const cplx* src = u_nat + pl * (N * N) + (long long)row * N + j;
+  cplx* dst = u_lane + pl * GE::PP + r0 * N + lane;
+#pragma unroll
+  for (int q = 0; q < 8; q++) dst[q * GE::QS] = src[q * R2];
 }
 
 #define RPA_FFT8_ARGS                                                                                              \
