@@ -40,12 +40,13 @@ struct Geo {
   // valence bands per loop iteration: one block barrier per VB bands, and the VB x nk2 kept columns of an iteration
   // fill whole warps of the x transforms (bounded by shared memory: 2 CTAs/SM at N = 40, 1 at N = 48, 64)
   static constexpr int VB = N <= 24 ? 4 : (N <= 48 ? 3 : 1);
-  // Valence planes are read in LANE ORDER (uv_lane_order_kernel): the RW rows of warp w form a region of RW N elements
-  // at w RW N, and inside it element q of lane l sits at q QS + l -- so each of the 8 loads a lane issues per band is
-  // one contiguous run of RW R2 x 16 B per warp (4-5 L1 wavefronts) instead of RW runs of R2 x 16 B in RW different
-  // rows (~9 wavefronts: the LSU data pipe is this kernel's limiter).  PP = plane pitch in that layout.
-  static constexpr int QS = RW * R2;
-  static constexpr int PP = NWARP * RW * N;
+  // Valence planes are read in LANE ORDER (uv_lane_order_kernel): warp w owns a region of 8 QS elements at w 8 QS of
+  // the plane, and inside it element q of lane l sits at q QS + l -- so each of the 8 loads a lane issues per band is
+  // one contiguous, 512-byte aligned run per warp (4 L1 wavefronts) instead of RW runs of R2 x 16 B in RW different
+  // rows (~9 wavefronts: the LSU data pipe is this kernel's limiter).  PP = plane pitch in that layout (lanes that
+  // hold no element leave holes that are never read).
+  static constexpr int QS = 32;
+  static constexpr int PP = NWARP * 8 * QS;
   static constexpr int G = (R2 & 1) ? R2 : R2 + 1;   // pitch of an s-group in a pass-A output line (odd)
   static constexpr int LW = 8 * G;                   // length of a pass-A output line
   // pitches in 16-byte elements.  P = R2 (mod 8) makes (line, j) -> bank group linear in the lane index, so the
@@ -119,7 +120,7 @@ __device__ __forceinline__ void pair_plane_fft8_body(const cplx* __restrict__ u_
   cplx twj[8];
 #pragma unroll
   for (int s = 1; s < 8; s++) twj[s] = tw[(j * s) % N];
-  const cplx* uvp = u_v + (long long)z * GE::PP + r0 * N + lane;   // lane order, see Geo
+  const cplx* uvp = u_v + (long long)z * GE::PP + warp * (8 * GE::QS) + lane;   // lane order, see Geo
   cplx nxt[8];
   if (row_on) {
 #pragma unroll
@@ -289,7 +290,7 @@ __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict
   cplx twj[8];
 #pragma unroll
   for (int s = 1; s < 8; s++) twj[s] = tw[(j * s) % N];
-  const cplx* uvp = u_v + (long long)z * GE::PP + r0 * N + lane;   // lane order, see Geo
+  const cplx* uvp = u_v + (long long)z * GE::PP + warp * (8 * GE::QS) + lane;   // lane order, see Geo
   cplx nxt[8];
   if (row_on) {
 #pragma unroll
@@ -397,7 +398,7 @@ __global__ void __launch_bounds__(Geo<N>::NWARP * 32) uv_lane_order_kernel(const
   if (lane >= RW * R2 || row >= N) return;
   const long long pl = (long long)blockIdx.y * N3 + blockIdx.x;
   const cplx* src = u_nat + pl * (N * N) + (long long)row * N + j;
-  cplx* dst = u_lane + pl * GE::PP + r0 * N + lane;
+  cplx* dst = u_lane + pl * GE::PP + warp * (8 * GE::QS) + lane;
 #pragma unroll
   for (int q = 0; q < 8; q++) dst[q * GE::QS] = src[q * R2];
 }
