@@ -76,13 +76,18 @@ __device__ __host__ __forceinline__ int ht_chunks(int m, int nw, int cmax) {
 // the rank-2 update of column k to its row, it also accumulates that row's product with the NEXT reflector v_{k+1}, which
 // every CTA has formed beforehand from the updated row k+1 (one row: cheap, redundant).  MODE 0: v, v_next, w in shared
 // memory; 1: v, v_next (w_j = p_j + al2 v_j on the fly); 2: v_next only (v read back from Vh).
+// MODE 3 (n <= 32 HT_RMAX, one warp per matrix row, 256 threads): as mode 0, but every warp keeps ITS row of the trailing
+// matrix in registers for the whole reduction (lane l holds columns l, l + 32, ...), so the rank-2 update and the product
+// with the next reflector touch no memory but the shared-memory vectors; only the row the next column needs is written
+// back (to A, where every CTA reads it after the barrier).
+constexpr int HT_RMAX = 24;
 template <int MODE>
-__global__ void __launch_bounds__(1024) hetrd_fused_kernel(cplx* __restrict__ A, int n, cplx* __restrict__ Vh, cplx* __restrict__ tau,
+__global__ void __launch_bounds__(MODE == 3 ? 256 : 1024) hetrd_fused_kernel(cplx* __restrict__ A, int n, cplx* __restrict__ Vh, cplx* __restrict__ tau,
                                                           double* __restrict__ d, double* __restrict__ e, cplx* __restrict__ P /* [2][HT_CMAX][n] */, int cmax) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx* buf0 = reinterpret_cast<cplx*>(smem_raw);            // v_next / v alternate between buf0 and buf1 (MODE 2: buf0 only)
   cplx* buf1 = buf0 + n;
-  cplx* w = buf0 + 2 * n;                                    // MODE 0
+  cplx* w = buf0 + 2 * n;                                    // MODE 0, 3
   __shared__ double sh[2 * 32];
   cg::grid_group grid = cg::this_grid();
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -121,6 +126,14 @@ __global__ void __launch_bounds__(1024) hetrd_fused_kernel(cplx* __restrict__ A,
     }
     grid.sync();
   }
+  cplx areg[MODE == 3 ? HT_RMAX : 1];
+  if (MODE == 3 && gw < n) {
+#pragma unroll
+    for (int r = 0; r < HT_RMAX; r++) {
+      const int j = lane + 32 * r;
+      areg[r] = j < n ? __ldcg(A + (long long)gw * n + j) : make_double2(0.0, 0.0);
+    }
+  }
   for (int k = 0; k + 1 < n; k++) {
     // p_k = sum of the partial sums the row chunks of the last pass left; p_{k+1} goes to the other half (CTAs are not in step)
     const cplx* pk = P + (size_t)(k & 1) * HT_CMAX * n;
@@ -137,17 +150,17 @@ __global__ void __launch_bounds__(1024) hetrd_fused_kernel(cplx* __restrict__ A,
     double q[2] = {0.0, 0.0};
     for (int i = k + 1 + tid; i < n; i += nthr) {
       const cplx x = pval(i), b = vval(i);
-      if (MODE == 0) w[i] = x;                                 // p stays in shared memory for the second loop (same thread)
+      if (MODE == 0 || MODE == 3) w[i] = x;                    // p stays in shared memory for the second loop (same thread)
       q[0] += x.x * b.x + x.y * b.y; q[1] += x.x * b.y - x.y * b.x;
     }
     bsumx<2>(q, sh);
     const cplx al2 = cmulf(make_double2(-0.5 * t.x, -0.5 * t.y), make_double2(q[0], q[1]));
-    if (MODE == 0) {
+    if (MODE == 0 || MODE == 3) {
       for (int i = k + 1 + tid; i < n; i += nthr) { const cplx x = w[i], av = cmulf(al2, v[i]); w[i] = make_double2(x.x + av.x, x.y + av.y); }
       __syncthreads();
     }
     auto wval = [&](int i) -> cplx {
-      if (MODE == 0) return w[i];
+      if (MODE == 0 || MODE == 3) return w[i];
       const cplx x = pval(i), av = cmulf(al2, vval(i));
       return make_double2(x.x + av.x, x.y + av.y);
     };
@@ -191,8 +204,28 @@ __global__ void __launch_bounds__(1024) hetrd_fused_kernel(cplx* __restrict__ A,
     }
     if (k1 + 1 >= n) break;
     // ---- A22 -= v w^H + w v^H and p_next = tau_next A22' v_next in the same pass (warp per row; row k+1 is dead)
+    if (MODE == 3) {
+      const int i = gw;                                        // this warp's row, resident in areg
+      if (i > k1 && i < n) {
+        const cplx vi = v[i], wi = w[i];
+        double pr = 0.0, pi = 0.0;
+#pragma unroll
+        for (int r = 0; r < HT_RMAX; r++) {
+          const int j = lane + 32 * r;
+          if (j > k1 && j < n) {
+            const cplx a = updated(areg[r], vi, wi, v[j], w[j]);
+            areg[r] = a;
+            if (i == k1 + 1) __stcg(A + (long long)i * n + j, a);   // the row the next column's reflector is formed from
+            const cplx b = vn[j];
+            pr += a.x * b.x - a.y * b.y; pi += a.x * b.y + a.y * b.x;
+          }
+        }
+        pr = wsum(pr); pi = wsum(pi);
+        if (lane == 0) pnext[i] = cmulf(tn, make_double2(pr, pi));
+      }
+    }
     const int m = n - k1 - 1, clen = ((m + ccur - 1) / ccur + 31) & ~31;     // rows (= columns) k1+1 .. n-1 in ccur column chunks
-    for (long long task = gw; task < (long long)m * ccur; task += nw) {
+    for (long long task = gw; MODE != 3 && task < (long long)m * ccur; task += nw) {
       const int i = k1 + 1 + (int)(task / ccur), c = (int)(task % ccur);
       const int j0 = k1 + 1 + c * clen, j1 = min(n, j0 + clen);
       cplx* ri = A + (long long)i * n;
@@ -476,6 +509,15 @@ int tridiag_eigh_lowest(rpa_ctx* ctx, WsAlloc& ws, const cplx* H, long long ld, 
   const size_t smem1 = (size_t)(3 - mode) * row;
   if (!coop || smem1 > cap) return RPA_ERR_INVALID;
   const void* fn = mode == 0 ? (const void*)hetrd_fused_kernel<0> : mode == 1 ? (const void*)hetrd_fused_kernel<1> : (const void*)hetrd_fused_kernel<2>;
+  // rows resident in registers (mode 3) when a warp per row fits on the device and a row fits in a warp's registers
+  bool rowreg = mode == 0 && n <= 32 * HT_RMAX && !getenv("RPA_HETRD_MODE") && !getenv("RPA_HETRD_THREADS") && !getenv("RPA_HETRD_NO_ROWREG");
+  if (rowreg) {
+    int ps = 0;
+    const void* f3 = (const void*)hetrd_fused_kernel<3>;
+    RPA_CUDA(ctx, cudaFuncSetAttribute(f3, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ps, f3, 256, smem1) != cudaSuccess || (long long)ps * ctx->sm_count < (n + 7) / 8) rowreg = false;
+    else fn = f3;
+  }
   RPA_CUDA(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
   // large matrices stream from HBM: one CTA of 32 warps per SM (the shared-memory rows allow no second CTA); small ones are
   // bound by the barrier latency: few small CTAs
@@ -483,7 +525,7 @@ int tridiag_eigh_lowest(rpa_ctx* ctx, WsAlloc& ws, const cplx* H, long long ld, 
   if (const char* m = getenv("RPA_HETRD_THREADS")) nthr = std::max(64, std::min(1024, atoi(m) & ~31));
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, nthr, smem1) != cudaSuccess || per_sm < 1) return RPA_ERR_INVALID;
   // small matrices: no more warps than rows (a cheaper barrier); large ones: every SM (rows are split into chunks when warps > rows)
-  const int grid = nthr > 256 ? ctx->sm_count * per_sm : std::min(ctx->sm_count * std::min(per_sm, 2), (n + 7) / 8);
+  const int grid = rowreg ? (n + 7) / 8 : nthr > 256 ? ctx->sm_count * per_sm : std::min(ctx->sm_count * std::min(per_sm, 2), (n + 7) / 8);
   cplx* A_ = Abuf; int n_ = n; cplx* V_ = Vbuf; cplx* tau_ = tau; double* d_ = d; double* e_ = e; cplx* p_ = p;
   int cmax = HT_CMAX;
   if (const char* m = getenv("RPA_HETRD_CMAX")) cmax = std::max(1, std::min(HT_CMAX, atoi(m)));

@@ -169,6 +169,33 @@ def test_chi_subspace_freq_random_basis():
         rpa.rpa_destroy(ctx)
 
 
+@pytest.mark.parametrize("n_eig", [1, 10, 30, 56, 64, 65, 81, 100, 128, 147])
+def test_chi_subspace_freq_every_tile_shape(n_eig):
+    """Hermitian zgemm warp shares: a ragged last tile row with 1..8 valid fragment rows (1, 2, 3 or 4 fragment rows per
+    warp row), diagonal tiles alone and next to full tiles, exact multiples of the tile; the projection with ragged M."""
+    import paper_2405_20258_b200 as rpa
+    import torch
+    rng = np.random.default_rng(40 + n_eig)
+    inp = make_inputs(0)
+    ng, nv, nc = inp.n_g, 2, 45
+    M = (rng.standard_normal((nv, nc, ng)) + 1j * rng.standard_normal((nv, nc, ng))) * 0.1
+    q, _ = np.linalg.qr(rng.standard_normal((ng, n_eig)) + 1j * rng.standard_normal((ng, n_eig)))
+    Cm = np.ascontiguousarray(q.T)
+    om = np.array([0.0, 0.7])
+    ctx = make_ctx(inp, nv, nc, n_eig, 2)
+    try:
+        chis = torch.full((2, n_eig, n_eig), 3.0, dtype=torch.complex128, device="cuda")
+        rpa.rpa_chi_subspace_freq(ctx, dev(M), dev(inp.e_v[:nv]), dev(inp.e_c[:nc]), dev(Cm), n_eig, dev(om), False, chis)
+        ref = orc.chi_subspace_freq(M, inp.e_v[:nv], inp.e_c[:nc], inp.vcoul, Cm, om)
+        got = chis.cpu().numpy()
+        assert maxnorm_rel(got, ref) <= 1e-13
+        assert np.abs(got - got.conj().transpose(0, 2, 1)).max() == 0.0     # mirrored exactly
+        rpa.rpa_chi_subspace_freq(ctx, dev(M), dev(inp.e_v[:nv]), dev(inp.e_c[:nc]), dev(Cm), n_eig, dev(om), True, chis)
+        assert maxnorm_rel(chis.cpu().numpy(), 2 * ref) <= 1e-13
+    finally:
+        rpa.rpa_destroy(ctx)
+
+
 @pytest.mark.parametrize("n,n_eig", [(147, 1), (147, 20), (147, 60), (147, 147), (300, 40), (333, 333)])
 def test_subspace_basis_direct_and_iterative(n, n_eig):
     """a3 alone on random negative-semidefinite matrices with an n^-2/3-like spectrum: direct Jacobi path
