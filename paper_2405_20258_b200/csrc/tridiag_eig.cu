@@ -144,6 +144,16 @@ __global__ void __launch_bounds__(MODE == 3 ? 256 : 1024) hetrd_fused_kernel(cpl
       for (int c = 1; c < cprev; c++) { const cplx y = __ldcg(pk + (size_t)c * n + i); x.x += y.x; x.y += y.y; }
       return x;
     };
+    // MODE 3: this thread's elements of row k+1 (needed after the reductions below) are requested now, so their L2 round
+    // trip overlaps the one of p_k
+    cplx r1pre[MODE == 3 ? (32 * HT_RMAX + 255) / 256 : 1];
+    if (MODE == 3) {
+#pragma unroll
+      for (int m = 0; m < (32 * HT_RMAX + 255) / 256; m++) {
+        const int j = k + 1 + tid + m * 256;
+        r1pre[m] = j < n ? __ldcg(A + (long long)(k + 1) * n + j) : make_double2(0.0, 0.0);
+      }
+    }
     const cplx* vrow = Vh + (long long)k * n;                 // MODE 2: v_k as written by CTA 0 one barrier ago
     auto vval = [&](int i) -> cplx { return MODE == 2 ? vrow[i] : v[i]; };
     // ---- w = p - (tau/2) (p^H v) v
@@ -179,7 +189,18 @@ __global__ void __launch_bounds__(MODE == 3 ? 256 : 1024) hetrd_fused_kernel(cpl
       const cplx* r1 = A + (long long)k1 * n;
       const cplx vi = vval(k1), wi = wval(k1);
       double s[1] = {0.0};
-      for (int j = k1 + tid; j < n; j += nthr) {
+      if (MODE == 3) {
+#pragma unroll
+        for (int m = 0; m < (32 * HT_RMAX + 255) / 256; m++) {
+          const int j = k1 + tid + m * 256;
+          if (j < n) {
+            const cplx a = updated(r1pre[m], vi, wi, vval(j), wval(j));
+            vn[j] = a;
+            if (j >= k1 + 2) s[0] += a.x * a.x + a.y * a.y;
+          }
+        }
+      }
+      for (int j = k1 + tid; MODE != 3 && j < n; j += nthr) {
         const cplx a = updated(__ldcg(r1 + j), vi, wi, vval(j), wval(j));
         vn[j] = a;
         if (j >= k1 + 2) s[0] += a.x * a.x + a.y * a.y;
