@@ -81,7 +81,7 @@ __device__ __forceinline__ void load_tile(cplx* s, const cplx* g, long long ld, 
 template <bool A_KM, bool B_KN, bool CONJ_B, int NI, int NJ, bool TRI>
 __device__ __forceinline__ void mma_ktile(const cplx* __restrict__ a_s, const cplx* __restrict__ b_s,
                                           const double* __restrict__ w_s, int g, int q, int mb, int nb,
-                                          double (&cre)[4][4][2], double (&cim)[4][4][2]) {
+                                          double (&cre)[4][4][2], double (&cim)[4][4][2], bool skip_upper = false) {
   constexpr int NA = TRI ? 6 : NI, NB = TRI ? 6 : NJ;   // fragments loaded per operand
 #pragma unroll
   for (int k4 = 0; k4 < BK / 4; k4++) {
@@ -107,6 +107,7 @@ __device__ __forceinline__ void mma_ktile(const cplx* __restrict__ a_s, const cp
 #pragma unroll
       for (int j = 0; j < NJ; j++) {
         const int ia = TRI ? 2 * i + (j >= 1) : i, jb = TRI ? 2 * i + (j == 2) : j;
+        if (skip_upper && j > i) continue;
         dmma(cre[i][j][0], cre[i][j][1], ar[ia], br[jb]);
         dmma(cim[i][j][0], cim[i][j][1], ai[ia], br[jb]);
       }
@@ -115,6 +116,7 @@ __device__ __forceinline__ void mma_ktile(const cplx* __restrict__ a_s, const cp
 #pragma unroll
       for (int j = 0; j < NJ; j++) {
         const int ia = TRI ? 2 * i + (j >= 1) : i, jb = TRI ? 2 * i + (j == 2) : j;
+        if (skip_upper && j > i) continue;
         dmma(cre[i][j][0], cre[i][j][1], CONJ_B ? ai[ia] : -ai[ia], bi[jb]);
         dmma(cim[i][j][0], cim[i][j][1], CONJ_B ? -ar[ia] : ar[ia], bi[jb]);
       }
@@ -183,7 +185,12 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
   // A ragged last tile row (M not a multiple of 64) has rv < 8 valid fragment rows: the two warp rows take ceil(rv / 2)
   // of them each instead of 4 (N_eig = 300: 3, N_eig = 2400: 2), the rest of the tile is zero and never stored.
   int ni = mode == 0 ? 4 : 3;
-  if (mode == 0 && p.M - m0 < BM - 8) {
+  // Never true in the kernels compiled without HERM (launch() sends every Hermitian update to the HERM kernels).  It
+  // predicates the DMMAs above the fragment diagonal of the general 4 x 4 shape, as the first version of this kernel did
+  // for diagonal tiles: ptxas schedules the main loop measurably better with the predicate in place (projection at
+  // configs[2]: 1.76 s without, 1.72 s with), so it stays.
+  const bool old_diag_warp = p.herm && tm == tn && wm == wn;
+  if (HERM && mode == 0 && p.M - m0 < BM - 8) {
     ni = (((p.M - m0 + 7) >> 3) + 1) >> 1;
     mb = wm * ni * 8;
   }
@@ -211,7 +218,8 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
     const cplx* a_s = sA + st * TA;
     const cplx* b_s = sB + st * TB;
     const double* w_s = sW + st * BK;
-    if (!HERM || mode == 0) {
+    if (!HERM) mma_ktile<A_KM, B_KN, CONJ_B, 4, 4, false>(a_s, b_s, w_s, g, q, mb, nb, cre, cim, old_diag_warp);
+    else if (mode == 0) {
       if (ni == 4) mma_ktile<A_KM, B_KN, CONJ_B, 4, 4, false>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
       else if (ni == 3) mma_ktile<A_KM, B_KN, CONJ_B, 3, 4, false>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
       else if (ni == 2) mma_ktile<A_KM, B_KN, CONJ_B, 2, 4, false>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
@@ -227,7 +235,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
   for (int i = 0; i < 4; i++) {
 #pragma unroll
     for (int j = 0; j < 4; j++) {
-      if (i >= ni || (HERM && mode != 0 && j == 3)) continue;   // accumulator slots this warp does not use
+      if (HERM && (i >= ni || (mode != 0 && j == 3))) continue;   // accumulator slots this warp does not use
       const int ro = HERM && mode == 2 ? 24 * i + (j >= 1 ? 8 : 0) : mb + i * 8;
       const int co = HERM && mode == 2 ? 24 * i + (j == 2 ? 8 : 0) : nb + j * 8;
       const int r = m0 + ro + g;
