@@ -391,7 +391,8 @@ __global__ void __launch_bounds__(SMEM ? 32 : 128) invit_kernel(const double* __
 }
 
 // (4) rows of Z <- Q z:  y <- H_0 H_1 ... H_{n-2} y,  H_k = I - tau_k v_k v_k^H.  NV vectors per CTA, kept in shared memory.
-constexpr int BT_NV = 4;
+constexpr int BT_NV = 2;      // vectors per CTA (300 vectors -> 150 CTAs: every SM has one)
+constexpr int BT_NE = 4;      // elements of a reflector per thread: n <= 1024 (larger matrices take the blocked route)
 __global__ void __launch_bounds__(256) backtransform_kernel(const cplx* __restrict__ Vh, const cplx* __restrict__ tau, int n, int n_eig,
                                                             cplx* __restrict__ Z) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -403,29 +404,54 @@ __global__ void __launch_bounds__(256) backtransform_kernel(const cplx* __restri
     y[idx] = u < nv ? Z[(long long)(v0 + u) * n + j] : make_double2(0.0, 0.0);
   }
   __syncthreads();
+  // The elements of v_k this thread needs (at most BT_NE: the kernel serves n < 1024) live in registers for both phases, and
+  // v_{k-1}, tau_{k-1} are requested before the reduction of reflector k, so their L2 round trip hides behind it.
+  cplx vcur[BT_NE], tcur;
+  auto loadv = [&](int k, cplx (&v)[BT_NE], cplx& t) {
+    t = k >= 0 ? tau[k] : make_double2(0.0, 0.0);
+#pragma unroll
+    for (int m = 0; m < BT_NE; m++) {
+      const int j = k + 1 + tid + 256 * m;
+      v[m] = (k >= 0 && j < n) ? Vh[(long long)k * n + j] : make_double2(0.0, 0.0);
+    }
+  };
+  loadv(n - 2, vcur, tcur);
   for (int k = n - 2; k >= 0; k--) {
-    const cplx t = tau[k];
-    if (t.x == 0.0 && t.y == 0.0) continue;
-    const cplx* vk = Vh + (long long)k * n;
-    double s[2 * BT_NV];
+    cplx vnx[BT_NE], tnx;
+    loadv(k - 1, vnx, tnx);
+    const cplx t = tcur;
+    if (t.x != 0.0 || t.y != 0.0) {
+      double s[2 * BT_NV];
 #pragma unroll
-    for (int u = 0; u < 2 * BT_NV; u++) s[u] = 0.0;
-    for (int j = k + 1 + tid; j < n; j += 256) {
-      const cplx v = vk[j];
+      for (int u = 0; u < 2 * BT_NV; u++) s[u] = 0.0;
 #pragma unroll
-      for (int u = 0; u < BT_NV; u++) { const cplx yy = y[u * n + j]; s[2 * u] += v.x * yy.x + v.y * yy.y; s[2 * u + 1] += v.x * yy.y - v.y * yy.x; }
-    }
-    bsum<2 * BT_NV>(s, sh);
-    for (int j = k + 1 + tid; j < n; j += 256) {
-      const cplx v = vk[j];
+      for (int m = 0; m < BT_NE; m++) {
+        const int j = k + 1 + tid + 256 * m;
+        if (j < n) {
+          const cplx v = vcur[m];
 #pragma unroll
-      for (int u = 0; u < BT_NV; u++) {
-        const cplx f = cmulf(t, make_double2(s[2 * u], s[2 * u + 1]));     // tau (v^H y)
-        const cplx g = cmulf(f, v);
-        y[u * n + j].x -= g.x; y[u * n + j].y -= g.y;
+          for (int u = 0; u < BT_NV; u++) { const cplx yy = y[u * n + j]; s[2 * u] += v.x * yy.x + v.y * yy.y; s[2 * u + 1] += v.x * yy.y - v.y * yy.x; }
+        }
       }
+      bsum<2 * BT_NV>(s, sh);
+#pragma unroll
+      for (int m = 0; m < BT_NE; m++) {
+        const int j = k + 1 + tid + 256 * m;
+        if (j < n) {
+          const cplx v = vcur[m];
+#pragma unroll
+          for (int u = 0; u < BT_NV; u++) {
+            const cplx f = cmulf(t, make_double2(s[2 * u], s[2 * u + 1]));     // tau (v^H y)
+            const cplx g = cmulf(f, v);
+            y[u * n + j].x -= g.x; y[u * n + j].y -= g.y;
+          }
+        }
+      }
+      __syncthreads();
     }
-    __syncthreads();
+#pragma unroll
+    for (int m = 0; m < BT_NE; m++) vcur[m] = vnx[m];
+    tcur = tnx;
   }
   for (int idx = tid; idx < nv * n; idx += 256) {
     const int u = idx / n, j = idx - u * n;
