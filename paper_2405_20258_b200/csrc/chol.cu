@@ -110,15 +110,26 @@ __global__ void __launch_bounds__(TC) diag_solve_kernel(const cplx* L, long long
   const bool ok = c < ncols;
   for (int i = 0; i < nb; i++) sx[i * (TC + 1) + threadIdx.x] = ok ? X[(long long)(r0 + i) * ldx + c] : make_double2(0, 0);
   __syncthreads();
+  // row-oriented forward substitution: x_i = (b_i - sum_{k<i} L_ik x_k) / L_ii.  The sum only READS shared memory (the
+  // column-oriented form updated every later row through shared memory, one dependent read-modify-write per term), with
+  // two independent accumulator pairs.
   for (int i = 0; i < nb; i++) {
+    double ar0 = 0.0, ai0 = 0.0, ar1 = 0.0, ai1 = 0.0;
+    int k = 0;
+    for (; k + 1 < i; k += 2) {
+      const cplx l0 = sl[i * LDB + k], x0 = sx[k * (TC + 1) + threadIdx.x];
+      const cplx l1 = sl[i * LDB + k + 1], x1 = sx[(k + 1) * (TC + 1) + threadIdx.x];
+      ar0 += l0.x * x0.x - l0.y * x0.y; ai0 += l0.x * x0.y + l0.y * x0.x;
+      ar1 += l1.x * x1.x - l1.y * x1.y; ai1 += l1.x * x1.y + l1.y * x1.x;
+    }
+    if (k < i) {
+      const cplx l0 = sl[i * LDB + k], x0 = sx[k * (TC + 1) + threadIdx.x];
+      ar0 += l0.x * x0.x - l0.y * x0.y; ai0 += l0.x * x0.y + l0.y * x0.x;
+    }
     cplx xi = sx[i * (TC + 1) + threadIdx.x];
     const double dinv = 1.0 / sl[i * LDB + i].x;
-    xi.x *= dinv; xi.y *= dinv;
+    xi.x = (xi.x - (ar0 + ar1)) * dinv; xi.y = (xi.y - (ai0 + ai1)) * dinv;
     sx[i * (TC + 1) + threadIdx.x] = xi;
-    for (int k = i + 1; k < nb; k++) {
-      cplx u = cmul_(sl[k * LDB + i], xi);
-      sx[k * (TC + 1) + threadIdx.x].x -= u.x; sx[k * (TC + 1) + threadIdx.x].y -= u.y;
-    }
   }
   if (ok)
     for (int i = 0; i < nb; i++) X[(long long)(r0 + i) * ldx + c] = sx[i * (TC + 1) + threadIdx.x];
