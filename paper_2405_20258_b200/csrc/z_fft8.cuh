@@ -28,14 +28,17 @@ struct Args {
 
 constexpr int MAXT = 8 * ((MAXO + 1) / 2);   // pass-B tasks (at least 2 kept outputs per task)
 
+// N3 = 120: two CTAs per SM (64 registers per thread; the pass-A twiddles are read from shared memory, warp-uniform, instead
+// of living in 28 registers) -- with one CTA the only latency hiding is the prefetch of the next tile behind pass B.
 template <int N3>
-__global__ void __launch_bounds__(32 * (N3 / 8)) z_fft8_scatter_kernel(Args a) {
+__global__ void __launch_bounds__(32 * (N3 / 8), N3 == 120 ? 2 : 1) z_fft8_scatter_kernel(Args a) {
   constexpr int R3 = N3 / 8, P = N3 | 1, NTHR = 32 * R3;
   constexpr int OG = R3 >= 20 ? 3 : 2;                  // kept outputs per pass-B task: about one round of tasks per tile
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx* y = reinterpret_cast<cplx*>(smem_raw);          // [32][P]   y_s[j3] at s*R3 + j3
   cplx* twb = y + 32 * P;                               // [8][MAXO][R3]  w_R3^{j3 s2} of the kept outputs of residue s
   int* oidx = reinterpret_cast<int*>(twb + 8 * MAXO * R3);   // [8][MAXO] index into the kept list, or -1
+  cplx* twa_s = reinterpret_cast<cplx*>(oidx + 8 * MAXO);    // [R3][8] w_N3^{j3 s} (pass A), used when TWA_SMEM
   __shared__ long long s_row[32];
   __shared__ int s_j[32];
   __shared__ int t_s[MAXT], t_o0[MAXT], n_task;         // pass-B tasks: residue s, outputs o0 .. o0 + OG - 1 of it
@@ -62,9 +65,14 @@ __global__ void __launch_bounds__(32 * (N3 / 8)) z_fft8_scatter_kernel(Args a) {
     twb[i] = w;
   }
   const int j3 = warp;                                   // pass A role
-  cplx twa[8];
+  constexpr bool TWA_SMEM = N3 == 120;
+  cplx twa[TWA_SMEM ? 1 : 8];
+  if (TWA_SMEM) {
+    for (int i = tid; i < R3 * 8; i += NTHR) twa_s[i] = a.tw[((i >> 3) * (i & 7)) % N3];
+  } else {
 #pragma unroll
-  for (int sA = 1; sA < 8; sA++) twa[sA] = a.tw[(j3 * sA) % N3];
+    for (int sA = 1; sA < 8; sA++) twa[sA] = a.tw[(j3 * sA) % N3];
+  }
   const long long n_tiles = (a.n_lines + 31) / 32;
   // prefetch of the first tile
   long long tile = blockIdx.x;
@@ -91,7 +99,7 @@ __global__ void __launch_bounds__(32 * (N3 / 8)) z_fft8_scatter_kernel(Args a) {
     cplx* dst = y + lane * P + j3;
     dst[0] = x[0];
 #pragma unroll
-    for (int sA = 1; sA < 8; sA++) dst[sA * R3] = fftsm::cmul(x[sA], twa[sA]);
+    for (int sA = 1; sA < 8; sA++) dst[sA * R3] = fftsm::cmul(x[sA], TWA_SMEM ? twa_s[j3 * 8 + sA] : twa[sA]);
     if (warp == 0) { s_row[lane] = row_n; s_j[lane] = j_n; }
     __syncthreads();
     fetch(tile + gridDim.x);                             // next tile's loads fly while pass B runs
@@ -133,7 +141,7 @@ __global__ void __launch_bounds__(32 * (N3 / 8)) z_fft8_scatter_kernel(Args a) {
 template <int N3>
 size_t smem_bytes() {
   constexpr int R3 = N3 / 8, P = N3 | 1;
-  return ((size_t)32 * P + (size_t)8 * MAXO * R3) * sizeof(cplx) + 8 * MAXO * sizeof(int);
+  return ((size_t)32 * P + (size_t)8 * MAXO * R3) * sizeof(cplx) + 8 * MAXO * sizeof(int) + (size_t)R3 * 8 * sizeof(cplx);
 }
 
 }  // namespace zfft8
