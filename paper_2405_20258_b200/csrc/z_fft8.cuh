@@ -31,7 +31,7 @@ constexpr int MAXT = 8 * ((MAXO + 1) / 2);   // pass-B tasks (at least 2 kept ou
 // N3 = 120: two CTAs per SM (64 registers per thread; the pass-A twiddles are read from shared memory, warp-uniform, instead
 // of living in 28 registers) -- with one CTA the only latency hiding is the prefetch of the next tile behind pass B.
 template <int N3>
-__global__ void __launch_bounds__(32 * (N3 / 8), N3 == 120 ? 2 : 1) z_fft8_scatter_kernel(Args a) {
+__global__ void __launch_bounds__(32 * (N3 / 8), N3 == 120 ? 2 : 0) z_fft8_scatter_kernel(Args a) {
   constexpr int R3 = N3 / 8, P = N3 | 1, NTHR = 32 * R3;
   constexpr int OG = R3 >= 20 ? 3 : 2;                  // kept outputs per pass-B task: about one round of tasks per tile
   extern __shared__ __align__(16) unsigned char smem_raw[];
