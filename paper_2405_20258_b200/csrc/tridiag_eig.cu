@@ -391,7 +391,7 @@ __global__ void __launch_bounds__(SMEM ? 32 : 128) invit_kernel(const double* __
 }
 
 // (4) rows of Z <- Q z:  y <- H_0 H_1 ... H_{n-2} y,  H_k = I - tau_k v_k v_k^H.  NV vectors per CTA, kept in shared memory.
-constexpr int BT_NV = 2;      // vectors per CTA (300 vectors -> 150 CTAs: every SM has one)
+constexpr int BT_NV = 1;      // vectors per CTA (300 vectors -> 300 CTAs, two per SM)
 constexpr int BT_NE = 4;      // elements of a reflector per thread: n <= 1024 (larger matrices take the blocked route)
 __global__ void __launch_bounds__(256) backtransform_kernel(const cplx* __restrict__ Vh, const cplx* __restrict__ tau, int n, int n_eig,
                                                             cplx* __restrict__ Z) {
