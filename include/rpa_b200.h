@@ -41,13 +41,18 @@ enum {
 /* Statement of the problem: cell, FFT grid, the epsilon G-sphere with v(q+G), and
  * the wavefunction G-sphere.
  *   cell   host [9]   row-major lattice vectors a1,a2,a3 in bohr (kept for reference only)
- *   fft    host [3]   FFT grid (N1,N2,N3); every axis must factor into 2,3,5 and be <= 4096
+ *   fft    host [3]   FFT grid (N1,N2,N3); every axis must factor into 2,3,5 and be <= 1024.  An xy plane must fit in
+ *                     shared memory: square planes of 24, 40, 48 or 64 take the specialised kernels; any other N1 x N2
+ *                     needs 16 B x (2 N1 (N2|1) + 2 nk2 (N1|1)) <= 227 KB (nk2 = distinct epsilon-sphere indices on axis 2;
+ *                     roughly N1 N2 <= 80 x 80), else rpa_mtxel returns RPA_ERR_INVALID
  *   g_eps  host [n_g][3]  Miller indices of the epsilon sphere, any order (order defines M's G order)
  *   vcoul  host [n_g]     v(q+G) >= 0 (bare Coulomb 4 pi/(Omega |q+G|^2) in the configs)
  *   g_wfn  host [n_pw][3] Miller indices of the wavefunction sphere, any order
  *   |Miller index| must be < N/2 on each axis.  The pair product is alias-free (exact G-space
  *   convolution) when 2 max|n_wfn| + max|n_eps| < N; the library does not require it.
- *   device / cuda_stream: CUDA device ordinal and the caller's stream.
+ *   device / cuda_stream: CUDA device ordinal (compute capability 10.0 exactly: the library holds sm_100a code only)
+ *   and the caller's stream.  Several contexts, on the same or on different devices, may live in one process; a context
+ *   must not be used from two threads at once.
  * Synchronises once (uploads plans: twiddles, index maps, v^1/2).                              */
 int rpa_create(rpa_ctx** out, const double cell[9], const int fft[3], int n_g, const int32_t* g_eps,
                const double* vcoul, int n_pw, const int32_t* g_wfn, int device, void* cuda_stream);
@@ -77,8 +82,11 @@ int rpa_chi0_static(rpa_ctx* ctx, const void* M, int nvb, int nc, const double* 
 /* (a3) Static subspace basis; reading R9.  The n_eig eigenpairs of Hermitian chi0 with
  *   the greatest |lambda| (chi0 is negative-semidefinite: the most negative ones).
  *   C dev out [n_eig][n_g], row i = eigenvector i (unit 2-norm); lambda dev out [n_eig] ascending.
- *   tol: relative residual target ||chi0 c_i - lambda_i c_i|| <= tol |lambda_1| (<= 0 selects 1e-11).
- *   iters_out host, optional: subspace iterations used (0 = direct Jacobi of the whole matrix).
+ *   tol: relative residual target ||chi0 c_i - lambda_i c_i|| <= tol |lambda_1| (<= 0 selects 1e-11).  Every route
+ *   measures it on its result, together with max|C C^H - 1| <= max(10 tol, 1e-11), before returning: the direct
+ *   tridiagonalisation route falls back to Jacobi / block subspace iteration when it misses either, and those return
+ *   RPA_ERR_NO_CONVERGENCE when they do (or when the iteration hits its cap).
+ *   iters_out host, optional: subspace iterations used (0 = a direct eigen-decomposition of the whole matrix).
  *   Synchronises (convergence is checked on the host).                                           */
 int rpa_subspace_basis(rpa_ctx* ctx, const void* chi0, int n_eig, double tol, void* C, double* lambda,
                        int* iters_out);
@@ -134,7 +142,19 @@ int rpa_energy_host(rpa_ctx* ctx, const void* psi_v, int nv, const void* psi_c, 
                     const double* weight, int n_w, int keep_m, double* e_c_out, double* lambda_out,
                     double* per_freq, double* stage_ms);
 
-/* Measurement helpers (bench.py / profiles): register-only FP64 peaks on the context's device.
+/* ---------------------------------------------------------------------------------------------------------------------
+ * Diagnostics -- NOT part of the method's ABI (nothing below computes any step of the path); used by bench.py, the
+ * profiles and the tests.
+ *
+ * Environment switches, read ONCE by rpa_create (never on a launch path):
+ *   RPA_GENERIC_FFT=1        MTXEL runs its generic mixed-radix plane / z kernels even where a specialised one exists
+ *   RPA_NO_TRIDIAG=1         a3 skips the tridiagonalisation route: block subspace iteration + CholeskyQR2 + Jacobi
+ *                            Rayleigh-Ritz when 4 N_eig <= n_g (about), direct Jacobi otherwise
+ *   RPA_JACOBI_BLOCK_MIN=n   smallest matrix for which the Jacobi solver takes its GEMM block form (default 1024)
+ *   RPA_HETRD_MODE=0|1|2, RPA_HETRD_THREADS=n   force a large-matrix variant / CTA size of the tridiagonalisation kernel
+ *   RPA_VERBOSE=1            route decisions and kernel resources on stderr
+ * --------------------------------------------------------------------------------------------------------------------- */
+/* Register-only FP64 peaks on the context's device.
  *   kind 0: mma.sync m8n8k4 f64 (DMMA), kind 1: DFMA.  Returns TFLOP/s in *tflops; runs `iters`
  *   launches of a fixed-size kernel on the context stream and synchronises.                      */
 int rpa_fp64_peak(rpa_ctx* ctx, int kind, int iters, double* tflops);
@@ -148,10 +168,15 @@ enum { RPA_PROF_MTXEL_PLANE = 0, RPA_PROF_MTXEL_Z = 1, RPA_PROF_MTXEL_WFN = 2, R
        RPA_PROF_CHIS = 5, RPA_PROF_BASIS = 6, RPA_PROF_ENERGY = 7, RPA_PROF_NCLASS = 8 };
 int rpa_profile_begin(rpa_ctx* ctx);
 int rpa_profile_end(rpa_ctx* ctx, double* ms, long long* launches);
-/* The last Jacobi eigen-decomposition run by the basis stage (for bench.py's work model): matrix size, sweeps done,
- * kind 0 = vector one-sided Jacobi (44 n FLOP per rotated pair, n(n-1)/2 pairs per sweep), 1 = block Jacobi (32 n^3
- * GEMM FLOP per sweep).  Host out.                                                                                 */
+/* Route taken by the last rpa_subspace_basis / basis stage (bench.py's work model; the tests assert it): n = size of the
+ * last dense eigen-decomposition (n_g, or the block size p of the subspace iteration), sweeps = Jacobi sweeps done,
+ * kind 0 = vector one-sided Jacobi (44 n FLOP per rotated pair, n(n-1)/2 pairs per sweep), 1 = block Jacobi (32 n^3 GEMM
+ * FLOP per sweep), 2 = tridiagonalisation + bisection + inverse iteration.  Whether the block subspace iteration ran is
+ * what rpa_subspace_basis returns in iters_out (> 0).  Host out.                                                    */
 int rpa_basis_info(const rpa_ctx* ctx, int* n, int* sweeps, int* kind);
+/* What the last rpa_subspace_basis / basis stage measured on its own result before returning (every route checks it
+ * against tol): residual = max_i ||chi0 c_i - lambda_i c_i|| / |lambda_1|, orthogonality = max |C C^H - 1|.  Host out. */
+int rpa_basis_quality(const rpa_ctx* ctx, double* residual, double* orthogonality);
 /* Number of kernels launched by this context since creation (for bench.py's gpu_launches). */
 long long rpa_launch_count(const rpa_ctx* ctx);
 

@@ -18,7 +18,7 @@ EXPORTED_SYMBOLS = [
     "rpa_set_workspace", "rpa_mtxel", "rpa_chi0_static", "rpa_subspace_basis", "rpa_chi_subspace_freq",
     "rpa_correlation_energy", "rpa_energy_device", "rpa_energy_host", "rpa_fp64_peak", "rpa_launch_count",
     "rpa_profile_begin", "rpa_profile_end", "rpa_chi0_static_occ", "rpa_chi_subspace_freq_occ",
-    "rpa_epsilon_inverse", "rpa_epsilon_inverse_workspace_bytes", "rpa_basis_info",
+    "rpa_epsilon_inverse", "rpa_epsilon_inverse_workspace_bytes", "rpa_basis_info", "rpa_basis_quality",
 ]
 
 
@@ -42,9 +42,10 @@ def load_library(build_if_missing: bool = True):
         from . import _build
         try:
             _build.build()
-        except Exception:
+        except FileNotFoundError:       # no nvcc on this machine: an existing library is used as it is
             if not os.path.exists(path):
                 raise
+        # any other failure (a compile error after a source edit) propagates: never run a stale binary silently
     if not os.path.exists(path):
         raise RpaError(-3, f"{path} is missing: build it with `python -m paper_2405_20258_b200._build` (no CPU fallback)")
     lib = C.CDLL(path)
@@ -92,6 +93,8 @@ def load_library(build_if_missing: bool = True):
     lib.rpa_profile_end.restype = ci
     lib.rpa_basis_info.argtypes = [vp, pi, pi, pi]
     lib.rpa_basis_info.restype = ci
+    lib.rpa_basis_quality.argtypes = [vp, pd, pd]
+    lib.rpa_basis_quality.restype = ci
     lib.rpa_launch_count.argtypes = [vp]
     lib.rpa_launch_count.restype = C.c_longlong
     _LIB = lib
@@ -114,6 +117,14 @@ def _dev(t, dtype=None):
     if dtype is not None and t.dtype != dtype:
         raise TypeError(f"expected dtype {dtype}, got {t.dtype}")
     return C.c_void_p(t.data_ptr())
+
+
+def _shape(name, t, *dims):
+    """The C ABI receives raw pointers, so a mis-shaped tensor would be an out-of-bounds device access with no error:
+    every array is checked against the sizes the call passes to the library before the call is made."""
+    got = tuple(int(x) for x in t.shape)
+    if got != tuple(int(d) for d in dims):
+        raise TypeError(f"{name}: expected shape {tuple(int(d) for d in dims)}, got {got}")
 
 
 class RpaContext:
@@ -181,13 +192,37 @@ def rpa_set_workspace(ctx, tensor):
 def rpa_mtxel(ctx, psi_v, psi_c, M):
     import torch
     nvb, nc = psi_v.shape[0], psi_c.shape[0]
+    _shape("psi_v", psi_v, nvb, ctx.n_pw)
+    _shape("psi_c", psi_c, nc, ctx.n_pw)
+    _shape("M", M, nvb, nc, ctx.n_g)
     _check(ctx.handle, load_library().rpa_mtxel(ctx.handle, _dev(psi_v, torch.complex128), nvb,
                                                 _dev(psi_c, torch.complex128), nc, _dev(M, torch.complex128)))
     return M
 
 
+def _pair_shapes(ctx, M, e_v, e_c, f_v=None, f_c=None):
+    nvb, nc = e_v.shape[0], e_c.shape[0]
+    _shape("e_v", e_v, nvb)
+    _shape("e_c", e_c, nc)
+    _shape("M", M, nvb, nc, ctx.n_g)
+    if f_v is not None:
+        _shape("f_v", f_v, nvb)
+        _shape("f_c", f_c, nc)
+
+
+def _freq_shapes(ctx, Cmat, n_eig, omega, chi_s):
+    if Cmat is not None:
+        _shape("C", Cmat, n_eig, ctx.n_g)
+    elif n_eig != ctx.n_g:
+        raise TypeError(f"C is None (full basis): n_eig must be n_g = {ctx.n_g}, got {n_eig}")
+    _shape("omega", omega, omega.shape[0])
+    _shape("chi_s", chi_s, omega.shape[0], n_eig, n_eig)
+
+
 def rpa_chi0_static(ctx, M, e_v, e_c, accumulate, chi0):
     import torch
+    _pair_shapes(ctx, M, e_v, e_c)
+    _shape("chi0", chi0, ctx.n_g, ctx.n_g)
     _check(ctx.handle, load_library().rpa_chi0_static(ctx.handle, _dev(M, torch.complex128), e_v.shape[0], e_c.shape[0],
                                                       _dev(e_v, torch.float64), _dev(e_c, torch.float64),
                                                       int(bool(accumulate)), _dev(chi0, torch.complex128)))
@@ -196,6 +231,9 @@ def rpa_chi0_static(ctx, M, e_v, e_c, accumulate, chi0):
 
 def rpa_subspace_basis(ctx, chi0, n_eig, tol, Cmat, lam):
     import torch
+    _shape("chi0", chi0, ctx.n_g, ctx.n_g)
+    _shape("C", Cmat, n_eig, ctx.n_g)
+    _shape("lambda", lam, n_eig)
     iters = C.c_int(0)
     _check(ctx.handle, load_library().rpa_subspace_basis(ctx.handle, _dev(chi0, torch.complex128), n_eig, float(tol),
                                                          _dev(Cmat, torch.complex128), _dev(lam, torch.float64),
@@ -205,6 +243,8 @@ def rpa_subspace_basis(ctx, chi0, n_eig, tol, Cmat, lam):
 
 def rpa_chi_subspace_freq(ctx, M, e_v, e_c, Cmat, n_eig, omega, accumulate, chi_s):
     import torch
+    _pair_shapes(ctx, M, e_v, e_c)
+    _freq_shapes(ctx, Cmat, n_eig, omega, chi_s)
     _check(ctx.handle, load_library().rpa_chi_subspace_freq(
         ctx.handle, _dev(M, torch.complex128), e_v.shape[0], e_c.shape[0], _dev(e_v, torch.float64),
         _dev(e_c, torch.float64), _dev(Cmat, torch.complex128) if Cmat is not None else None, n_eig,
@@ -215,6 +255,8 @@ def rpa_chi_subspace_freq(ctx, M, e_v, e_c, Cmat, n_eig, omega, accumulate, chi_
 def rpa_chi0_static_occ(ctx, M, e_v, e_c, f_v, f_c, accumulate, chi0):
     import torch
     f64, c128 = torch.float64, torch.complex128
+    _pair_shapes(ctx, M, e_v, e_c, f_v, f_c)
+    _shape("chi0", chi0, ctx.n_g, ctx.n_g)
     _check(ctx.handle, load_library().rpa_chi0_static_occ(ctx.handle, _dev(M, c128), e_v.shape[0], e_c.shape[0], _dev(e_v, f64),
                                                           _dev(e_c, f64), _dev(f_v, f64), _dev(f_c, f64), int(bool(accumulate)),
                                                           _dev(chi0, c128)))
@@ -224,6 +266,8 @@ def rpa_chi0_static_occ(ctx, M, e_v, e_c, f_v, f_c, accumulate, chi0):
 def rpa_chi_subspace_freq_occ(ctx, M, e_v, e_c, f_v, f_c, Cmat, n_eig, omega, accumulate, chi_s):
     import torch
     f64, c128 = torch.float64, torch.complex128
+    _pair_shapes(ctx, M, e_v, e_c, f_v, f_c)
+    _freq_shapes(ctx, Cmat, n_eig, omega, chi_s)
     _check(ctx.handle, load_library().rpa_chi_subspace_freq_occ(
         ctx.handle, _dev(M, c128), e_v.shape[0], e_c.shape[0], _dev(e_v, f64), _dev(e_c, f64), _dev(f_v, f64), _dev(f_c, f64),
         _dev(Cmat, c128) if Cmat is not None else None, n_eig, _dev(omega, f64), omega.shape[0], int(bool(accumulate)),
@@ -238,6 +282,8 @@ def rpa_epsilon_inverse_workspace_bytes(ctx, n_eig, n_w) -> int:
 def rpa_epsilon_inverse(ctx, chi_s, eps_inv):
     import torch
     n_w, n_eig = chi_s.shape[0], chi_s.shape[1]
+    _shape("chi_s", chi_s, n_w, n_eig, n_eig)
+    _shape("eps_inv", eps_inv, n_w, n_eig, n_eig)
     _check(ctx.handle, load_library().rpa_epsilon_inverse(ctx.handle, _dev(chi_s, torch.complex128), n_eig, n_w,
                                                           _dev(eps_inv, torch.complex128)))
     return eps_inv
@@ -246,6 +292,8 @@ def rpa_epsilon_inverse(ctx, chi_s, eps_inv):
 def rpa_correlation_energy(ctx, chi_s, n_eig, weight):
     import torch
     n_w = weight.shape[0]
+    _shape("weight", weight, n_w)
+    _shape("chi_s", chi_s, n_w, n_eig, n_eig)
     e = C.c_double(0.0)
     per = (C.c_double * n_w)()
     _check(ctx.handle, load_library().rpa_correlation_energy(ctx.handle, _dev(chi_s, torch.complex128), n_eig,
@@ -255,6 +303,13 @@ def rpa_correlation_energy(ctx, chi_s, n_eig, weight):
 
 def _energy(fn_name, ctx, psi_v, psi_c, e_v, e_c, nvb, n_eig, tol, omega, weight, keep_m, ptr):
     nv, nc, n_w = psi_v.shape[0], psi_c.shape[0], omega.shape[0]
+    _shape("psi_v", psi_v, nv, ctx.n_pw)
+    _shape("psi_c", psi_c, nc, ctx.n_pw)
+    _shape("e_v", e_v, nv)
+    _shape("e_c", e_c, nc)
+    _shape("weight", weight, n_w)
+    if not (1 <= int(n_eig) <= ctx.n_g):
+        raise TypeError(f"n_eig = {n_eig} not in 1..n_g = {ctx.n_g}")
     e = C.c_double(0.0)
     lam = (C.c_double * n_eig)()
     per = (C.c_double * n_w)()
@@ -318,3 +373,11 @@ def rpa_basis_info(ctx):
     n, sw, kind = C.c_int(0), C.c_int(0), C.c_int(0)
     _check(ctx.handle, load_library().rpa_basis_info(ctx.handle, C.byref(n), C.byref(sw), C.byref(kind)))
     return n.value, sw.value, kind.value
+
+
+def rpa_basis_quality(ctx):
+    """(residual, orthogonality) the last basis stage measured on its result: max_i ||chi0 c_i - lambda_i c_i|| / |lambda_1|
+    and max |C C^H - 1|."""
+    r, o = C.c_double(0.0), C.c_double(0.0)
+    _check(ctx.handle, load_library().rpa_basis_quality(ctx.handle, C.byref(r), C.byref(o)))
+    return r.value, o.value

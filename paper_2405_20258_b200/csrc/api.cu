@@ -127,14 +127,24 @@ int rpa_create(rpa_ctx** out, const double cell[9], const int fft[3], int n_g, c
   memcpy(ctx->cell, cell, sizeof(ctx->cell));
   for (int a = 0; a < 3; a++) ctx->fft[a] = fft[a];
   ctx->n_g = n_g; ctx->n_pw = n_pw;
-  { const char* e = getenv("RPA_GENERIC_FFT"); ctx->force_generic_fft = e && e[0] == '1'; }
+  {  // diagnostic switches (rpa_b200.h "Diagnostics"): read here, once, never on the launch paths
+    auto on = [](const char* k) { const char* e = getenv(k); return e && e[0] == '1'; };
+    auto num = [](const char* k, int dflt) { const char* e = getenv(k); return e && *e ? atoi(e) : dflt; };
+    ctx->opt.generic_fft = on("RPA_GENERIC_FFT");
+    ctx->opt.verbose = on("RPA_VERBOSE");
+    ctx->opt.no_tridiag = on("RPA_NO_TRIDIAG");
+    ctx->opt.jacobi_block_min = std::max(2, num("RPA_JACOBI_BLOCK_MIN", 1024));
+    ctx->opt.hetrd_mode = num("RPA_HETRD_MODE", -1);
+    ctx->opt.hetrd_threads = num("RPA_HETRD_THREADS", 0);
+  }
   auto fail = [&](int rc) { g_null_err = ctx->err; rpa_destroy(ctx); return rc; };
   if ((e = cudaSetDevice(device)) != cudaSuccess) return fail(rpa_fail(ctx, RPA_ERR_CUDA, "cudaSetDevice: %s", cudaGetErrorString(e)));
   cudaDeviceProp prop;
   if ((e = cudaGetDeviceProperties(&prop, device)) != cudaSuccess)
     return fail(rpa_fail(ctx, RPA_ERR_CUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e)));
   ctx->sm_count = prop.multiProcessorCount;
-  if (prop.major < 10) return fail(rpa_fail(ctx, RPA_ERR_CUDA, "device %d is sm_%d%d; this library is built for sm_100a only", device, prop.major, prop.minor));
+  if (prop.major != 10 || prop.minor != 0)   // the .so holds sm_100a SASS only (arch-specific: no PTX JIT to other parts)
+    return fail(rpa_fail(ctx, RPA_ERR_CUDA, "device %d is sm_%d%d; this library is built for sm_100a (compute capability 10.0) only", device, prop.major, prop.minor));
   long long nr = 1;
   for (int a = 0; a < 3; a++) {
     if (fft[a] < 1) return fail(rpa_fail(ctx, RPA_ERR_INVALID, "rpa_create: fft[%d] = %d", a, fft[a]));
@@ -147,12 +157,15 @@ int rpa_create(rpa_ctx** out, const double cell[9], const int fft[3], int n_g, c
   double* d_v = nullptr;
   if (cudaMalloc(&d_v, n_g * sizeof(double)) != cudaSuccess || cudaMalloc(&ctx->d_vsqrt, n_g * sizeof(double)) != cudaSuccess)
     return fail(rpa_fail(ctx, RPA_ERR_CUDA, "rpa_create: cudaMalloc failed"));
-  cudaMemcpy(d_v, vcoul, n_g * sizeof(double), cudaMemcpyHostToDevice);
-  sqrt_kernel<<<(n_g + 255) / 256, 256, 0, ctx->stream>>>(d_v, n_g, ctx->d_vsqrt);
-  ctx->launches++;
-  e = cudaStreamSynchronize(ctx->stream);
+  e = cudaMemcpy(d_v, vcoul, n_g * sizeof(double), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) {
+    sqrt_kernel<<<(n_g + 255) / 256, 256, 0, ctx->stream>>>(d_v, n_g, ctx->d_vsqrt);
+    ctx->launches++;
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
   cudaFree(d_v);
-  if (e != cudaSuccess) return fail(rpa_fail(ctx, RPA_ERR_CUDA, "rpa_create: %s", cudaGetErrorString(e)));
+  if (e != cudaSuccess) return fail(rpa_fail(ctx, RPA_ERR_CUDA, "rpa_create: upload of v(G): %s", cudaGetErrorString(e)));
   *out = ctx;
   return RPA_OK;
 }
@@ -175,6 +188,12 @@ long long rpa_launch_count(const rpa_ctx* ctx) { return ctx ? ctx->launches : 0;
 int rpa_basis_info(const rpa_ctx* ctx, int* n, int* sweeps, int* kind) {
   if (!ctx || !n || !sweeps || !kind) return RPA_ERR_INVALID;
   *n = ctx->jac_n; *sweeps = ctx->jac_sweeps; *kind = ctx->jac_kind;
+  return RPA_OK;
+}
+
+int rpa_basis_quality(const rpa_ctx* ctx, double* residual, double* orthogonality) {
+  if (!ctx || !residual || !orthogonality) return RPA_ERR_INVALID;
+  *residual = ctx->basis_residual; *orthogonality = ctx->basis_ortho;
   return RPA_OK;
 }
 

@@ -216,6 +216,27 @@ __global__ void residual_kernel(const cplx* __restrict__ X, const cplx* __restri
   if (threadIdx.x == 0) res[blockIdx.x] = sqrt(v[0]);
 }
 
+// q[0] = max_i res[i], q[1] = max_ij |S[i][j] - delta_ij|  (both >= 0: the bit patterns of non-negative doubles order like
+// unsigned integers, so the maximum is an integer atomicMax).  One row of S per CTA; q must be zeroed first.
+__global__ void quality_kernel(const double* __restrict__ res, const cplx* __restrict__ S, int p, double* __restrict__ q) {
+  __shared__ double sh[32];
+  const int i = blockIdx.x;
+  double m = 0.0;
+  for (int j = threadIdx.x; j < p; j += blockDim.x) {
+    const cplx x = S[(long long)i * p + j];
+    m = fmax(m, fmax(fabs(x.x - (i == j ? 1.0 : 0.0)), fabs(x.y)));
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < (int)(blockDim.x >> 5); w++) m = fmax(m, sh[w]);
+    atomicMax(reinterpret_cast<unsigned long long*>(q + 1), (unsigned long long)__double_as_longlong(m));
+    atomicMax(reinterpret_cast<unsigned long long*>(q), (unsigned long long)__double_as_longlong(res[i]));
+  }
+}
+
 struct JacobiWs {
   cplx* A; cplx* V; double* lam; double* scale; int* order; double* scal;  // scal[0] = gmax, scal[1] = off_max
   double* off; int* info;   // [64] per-sweep off-norm, [2] sweeps / converged (persistent kernel)
@@ -355,10 +376,8 @@ __global__ void __launch_bounds__(256) pair_rotations_kernel(const cplx* __restr
   }
 }
 
-int jacobi_block_min() {   // matrices smaller than this use the vector iteration (RPA_JACOBI_BLOCK_MIN overrides)
-  const char* e = getenv("RPA_JACOBI_BLOCK_MIN");
-  return e ? atoi(e) : 1024;
-}
+// matrices smaller than this use the vector iteration (1024; RPA_JACOBI_BLOCK_MIN, read by rpa_create, overrides)
+int jacobi_block_min(const rpa_ctx* ctx) { return ctx->opt.jacobi_block_min; }
 
 // One sweep (nblk steps) of the block iteration on the n_pad = nblk * JB vectors of length n in A (and V if with_v).
 int block_jacobi_sweep(rpa_ctx* ctx, cplx* A, cplx* V, bool with_v, int n, int nblk, cplx* Wb, cplx* Ub, const double* gmax,
@@ -395,15 +414,13 @@ int block_jacobi_sweep(rpa_ctx* ctx, cplx* A, cplx* V, bool with_v, int n, int n
 // some wanted eigenvalue is numerically null (its column of G V cannot be normalised); that case reruns with V.
 int jacobi_eigh(rpa_ctx* ctx, const cplx* src, long long ld, int n, bool src_is_hc, int n_need, bool try_without_v,
                 JacobiWs& jw, std::vector<int>& order_h, std::vector<double>& lam_h) {
-  static bool attr = false;
-  if (!attr) {
+  if (ctx->attr_once(RPA_ATTR_JACOBI)) {
     RPA_CUDA(ctx, cudaFuncSetAttribute(jacobi_round_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
     RPA_CUDA(ctx, cudaFuncSetAttribute(jacobi_round_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
     RPA_CUDA(ctx, cudaFuncSetAttribute(pair_rotations_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        (int)((size_t)2 * JP * JLD * sizeof(cplx))));
-    attr = true;
   }
-  const bool verbose = getenv("RPA_VERBOSE") != nullptr;
+  const bool verbose = ctx->opt.verbose;
   for (int attempt = try_without_v ? 0 : 1; attempt < 2; attempt++) {
     const bool with_v = attempt == 1;
     jw.with_v = with_v;
@@ -415,7 +432,7 @@ int jacobi_eigh(rpa_ctx* ctx, const cplx* src, long long ld, int n, bool src_is_
     RPA_LAUNCH_CHECK(ctx);
     const int m_even = (n + 1) & ~1;
     const double stop = std::max(1e-14, 4.0 * std::sqrt((double)n) * 1.1e-16);
-    const bool block = jw.Wb != nullptr && n >= jacobi_block_min();
+    const bool block = jw.Wb != nullptr && n >= jacobi_block_min(ctx);
     const int n_rows = block ? (n + JB - 1) / JB * JB : n;   // vectors held in jw.A (the block iteration pads with zeros)
     const size_t stash_bytes = (size_t)2 * n * sizeof(cplx);
     const bool stash = stash_bytes <= 96 * 1024;
@@ -444,7 +461,7 @@ int jacobi_eigh(rpa_ctx* ctx, const cplx* src, long long ld, int n, bool src_is_
       }
       persistent = true;   // skip the per-round launch loop below
     }
-    if (!block && !converged && !getenv("RPA_JACOBI_LAUNCHES")) {
+    if (!block && !converged) {
       // one cooperative launch for all sweeps, if the device can co-schedule a useful number of CTAs
       const void* fn = with_v ? (stash ? (const void*)jacobi_persistent_kernel<true, true> : (const void*)jacobi_persistent_kernel<true, false>)
                               : (stash ? (const void*)jacobi_persistent_kernel<false, true> : (const void*)jacobi_persistent_kernel<false, false>);
@@ -522,14 +539,11 @@ int block_size(int n, int n_eig) {
 }
 bool use_direct(int n, int n_eig) { return 2 * block_size(n, n_eig) > n; }
 // tridiagonalisation + bisection + inverse iteration (tridiag_eig.cu): part of the spectrum, v and the Sturm data in shared memory
-bool use_tridiag(int n, int n_eig) {
-  return n >= 32 && n <= 12800 && 4 * n_eig <= 3 * n && !getenv("RPA_NO_TRIDIAG") && (n < jacobi_block_min() || !getenv("RPA_NO_TRIDIAG_LARGE"));
-}
+bool use_tridiag(const rpa_ctx* ctx, int n, int n_eig) { return n >= 32 && n <= 12800 && 4 * n_eig <= 3 * n && !ctx->opt.no_tridiag; }
 
 }  // namespace
 
 size_t basis_workspace_bytes(const rpa_ctx* ctx, int n, int n_eig) {
-  (void)ctx;
   const size_t small = ws_round((size_t)(n + JB) * sizeof(double)) * 4 + ws_round((size_t)(n + JB) * sizeof(int)) + 8 * 256;
   auto jac = [](size_t m) {   // A, V (padded to whole blocks) and the Gram / rotation matrices of the block iteration
     return 2 * ws_round((m + JB) * m * sizeof(cplx)) + 2 * ws_round(((m + JB) / JP + 1) * JP * JP * sizeof(cplx));
@@ -538,7 +552,7 @@ size_t basis_workspace_bytes(const rpa_ctx* ctx, int n, int n_eig) {
   if (use_direct(n, n_eig)) return direct;
   const size_t p = block_size(n, n_eig);
   const size_t iter = 3 * ws_round(p * n * sizeof(cplx)) + 2 * ws_round(p * p * sizeof(cplx)) + jac(p) + small;
-  return use_tridiag(n, n_eig) ? std::max(direct, iter) : iter;
+  return use_tridiag(ctx, n, n_eig) ? std::max(direct, iter) : iter;
 }
 
 int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, double tol, cplx* C, double* lambda,
@@ -557,16 +571,47 @@ int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, dou
   jw.off = ws.get<double>(64);
   jw.info = ws.get<int>(4);
   int* d_info = ws.get<int>(4);
+  double* d_quality = ws.get<double>(2);
   int rc;
+  // What the header promises for every route (P13): residuals ||chi0 c_i - lambda_i c_i|| <= tol |lambda_1| and
+  // C C^H = 1.  X [p][n] are the vectors, lam_dev their eigenvalues, Y [p][n] and S [p][p] scratch.  Returns 1 when the
+  // p vectors meet the targets, 0 when not, < 0 on error; the two measures are kept for rpa_basis_quality.
+  const double ortho_tol = std::max(10.0 * tol, 1e-11);
+  auto verify = [&](const cplx* X, const double* lam_dev, int p, cplx* Y, cplx* S) -> int {
+    ZgemmParams g;   // Y[i][G] = sum_G' chi0[G][G'] X[i][G']  (chi0 Hermitian)
+    g.A = X; g.lda = n; g.a_km = false; g.B = chi0; g.ldb = n; g.b_kn = true; g.C = Y; g.ldc = n;
+    g.M = p; g.N = n; g.K = n; g.conj_b = true;
+    int r = zgemm_dmma(ctx, g);
+    if (r) return r;
+    residual_kernel<<<p, 256, 0, ctx->stream>>>(X, Y, lam_dev, n, d_res);
+    RPA_LAUNCH_CHECK(ctx);
+    ZgemmParams h;   // S = X X^H
+    h.A = X; h.lda = n; h.a_km = false; h.B = X; h.ldb = n; h.b_kn = false; h.C = S; h.ldc = p;
+    h.M = p; h.N = p; h.K = n; h.conj_b = true; h.herm = true;
+    if ((r = zgemm_dmma(ctx, h))) return r;
+    RPA_CUDA(ctx, cudaMemsetAsync(d_quality, 0, 2 * sizeof(double), ctx->stream));
+    quality_kernel<<<p, 256, 0, ctx->stream>>>(d_res, S, p, d_quality);
+    RPA_LAUNCH_CHECK(ctx);
+    double q[3] = {0.0, 0.0, 0.0};
+    RPA_CUDA(ctx, cudaMemcpyAsync(q, d_quality, 2 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    RPA_CUDA(ctx, cudaMemcpyAsync(q + 2, lam_dev, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    const double scale = std::fabs(q[2]) > 0.0 ? std::fabs(q[2]) : 1.0;
+    ctx->basis_residual = q[0] / scale; ctx->basis_ortho = q[1];
+    if (ctx->opt.verbose)
+      fprintf(stderr, "[rpa] basis check: n=%d p=%d residual %.3e |lambda_1| (target %.1e), max|C C^H - 1| %.3e (target %.1e)\n", n, p,
+              ctx->basis_residual, tol, ctx->basis_ortho, ortho_tol);
+    return (std::isfinite(q[0]) && std::isfinite(q[1]) && ctx->basis_residual <= tol && ctx->basis_ortho <= ortho_tol) ? 1 : 0;
+  };
   const WsAlloc ws_iter = ws;   // the block iteration below restarts from here when the tridiagonal route fails
   const bool direct = use_direct(n, n_eig);
-  if (direct || use_tridiag(n, n_eig)) {
+  if (direct || use_tridiag(ctx, n, n_eig)) {
     jw.A = ws.get<cplx>((size_t)(n + JB) * n);
     jw.V = ws.get<cplx>((size_t)(n + JB) * n);
     jw.Wb = ws.get<cplx>((size_t)((n + JB) / JP + 1) * JP * JP);
     jw.Ub = ws.get<cplx>((size_t)((n + JB) / JP + 1) * JP * JP);
     if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_subspace_basis: workspace too small (need %zu bytes)", ws.off);
-    if (use_tridiag(n, n_eig)) {
+    if (use_tridiag(ctx, n, n_eig)) {
       // part of the spectrum: tridiagonalisation + bisection + inverse iteration (tridiag_eig.cu), then a
       // CholeskyQR2 clean-up of the n_eig vectors; any failure (e.g. a numerically singular Gram matrix because wanted
       // eigenvalues coincide) falls through to the Jacobi iteration below
@@ -587,7 +632,12 @@ int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, dou
         if (info_h != 0) { ok = false; break; }
         if ((rc = ztrsm_left_lower(ctx, S, n_eig, n_eig, C, n, n))) return rc;
       }
-      if (getenv("RPA_VERBOSE")) fprintf(stderr, "[rpa] tridiagonal eigensolver n=%d n_eig=%d %s\n", n, n_eig, ok ? "ok" : "failed -> Jacobi");
+      if (ok) {   // the route has no convergence test of its own (and no reorthogonalisation inside clusters): check it
+        const int v = verify(C, lambda, n_eig, jw.A, jw.V);
+        if (v < 0) return v;
+        ok = v == 1;
+      }
+      if (ctx->opt.verbose) fprintf(stderr, "[rpa] tridiagonal eigensolver n=%d n_eig=%d %s\n", n, n_eig, ok ? "ok" : "failed -> Jacobi / block iteration");
       if (ok) {
         ctx->jac_n = n; ctx->jac_sweeps = 0; ctx->jac_kind = 2;
         RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
@@ -605,6 +655,11 @@ int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, dou
     RPA_CUDA(ctx, cudaMemcpyAsync(lambda, ls.data(), n_eig * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
     RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     if (iters_out) *iters_out = 0;
+    const int v = verify(C, lambda, n_eig, jw.A, jw.V);   // the eigenvectors have left jw.A / jw.V
+    if (v < 0) return v;
+    if (v == 0)
+      return rpa_fail(ctx, RPA_ERR_NO_CONVERGENCE, "rpa_subspace_basis: Jacobi eigenvectors miss the targets: residual %.3e |lambda_1| (tol %.1e), "
+                      "max|C C^H - 1| %.3e (tol %.1e)", ctx->basis_residual, tol, ctx->basis_ortho, ortho_tol);
     return RPA_OK;
   }
 
@@ -689,6 +744,12 @@ int basis_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* chi0, int n, int n_eig, dou
   RPA_CUDA(ctx, cudaMemcpy2DAsync(C, (size_t)n * sizeof(cplx), X, (size_t)n * sizeof(cplx), (size_t)n * sizeof(cplx), n_eig,
                                   cudaMemcpyDeviceToDevice, ctx->stream));
   RPA_CUDA(ctx, cudaMemcpyAsync(lambda, d_lam_sorted, n_eig * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
-  RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+  {
+    const int v = verify(C, lambda, n_eig, Y, S);   // residuals were the stopping test; this adds orthonormality
+    if (v < 0) return v;
+    if (v == 0)
+      return rpa_fail(ctx, RPA_ERR_NO_CONVERGENCE, "rpa_subspace_basis: Ritz vectors miss the targets: residual %.3e |lambda_1| (tol %.1e), "
+                      "max|C C^H - 1| %.3e (tol %.1e)", ctx->basis_residual, tol, ctx->basis_ortho, ortho_tol);
+  }
   return RPA_OK;
 }

@@ -142,11 +142,9 @@ int zpotrf_batched(rpa_ctx* ctx, cplx* A, int n, long long lda, int batch, long 
                    double* dvec) {
   RPA_CUDA(ctx, cudaMemsetAsync(d_info, 0, batch * sizeof(int), ctx->stream));
   const size_t smem = (size_t)NB * LDB * sizeof(cplx);
-  static bool attr = false;
-  if (!attr) {
+  if (ctx->attr_once(RPA_ATTR_POTRF)) {
     RPA_CUDA(ctx, cudaFuncSetAttribute(potf2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     RPA_CUDA(ctx, cudaFuncSetAttribute(panel_trsm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr = true;
   }
   for (int k0 = 0; k0 < n; k0 += NB) {
     const int nb = n - k0 < NB ? n - k0 : NB;
@@ -172,11 +170,8 @@ int zpotrf_batched(rpa_ctx* ctx, cplx* A, int n, long long lda, int batch, long 
 // X <- L^{-1} X, L lower triangular p x p (row-major), X [p][ncols] row-major.
 int ztrsm_left_lower(rpa_ctx* ctx, const cplx* L, long long ldl, int p, cplx* X, long long ldx, int ncols) {
   const size_t smem = ((size_t)NB * LDB + (size_t)NB * (TC + 1)) * sizeof(cplx);
-  static bool attr = false;
-  if (!attr) {
+  if (ctx->attr_once(RPA_ATTR_TRSM))
     RPA_CUDA(ctx, cudaFuncSetAttribute(diag_solve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr = true;
-  }
   for (int r0 = 0; r0 < p; r0 += NB) {
     const int nb = p - r0 < NB ? p - r0 : NB;
     if (r0 > 0) {

@@ -377,8 +377,8 @@ int launch_axis(rpa_ctx* ctx, cplx* data, const Plan& pl, long long n_lines, int
   const int tl = axis_tile_lines(pl.n);
   const size_t smem = (size_t)tl * (pl.n | 1) * sizeof(cplx);
   auto kern = fft_axis_kernel<INV, MODE>;
-  static bool attr = false;
-  if (!attr) { RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)); attr = true; }
+  if (ctx->attr_once(RPA_ATTR_AXIS + (INV ? 1 : 0) + 2 * MODE))
+    RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
   const long long blocks = (n_lines + tl - 1) / tl;
   if (blocks > 2147483647LL) return rpa_fail(ctx, RPA_ERR_INVALID, "fft grid too large");
   kern<<<(unsigned)blocks, 256, smem, ctx->stream>>>(data, pl, n_lines, inner, tl, zs);
@@ -411,21 +411,18 @@ int wfn_to_realspace(rpa_ctx* ctx, const cplx* psi, int nb, cplx* u) {
 template <int N>
 int launch_fft8(rpa_ctx* ctx, const cplx* u_v, const cplx* u_c, int nvb, int ncc, int N3, const MtxelPlan* mp, cplx* T) {
   const int nk1 = mp->ax[0].nk, nk2 = mp->ax[1].nk;
-  // ring variant (no block barrier in the band loop) where one CTA fits per SM anyway; RPA_FFT8_RING=0/1 overrides
-  static const char* ring_env = getenv("RPA_FFT8_RING");
+  // ring variant (no block barrier in the band loop) where one CTA fits per SM anyway (N = 48, 64)
   const size_t smem_ring = fft8::smem_bytes_ring<N>(nk2);
   const bool ring_ok = smem_ring <= 227 * 1024 && (nk2 + fft8::Geo<N>::RW - 1) / fft8::Geo<N>::RW <= fft8::Geo<N>::NWARP;
-  const bool ring = ring_ok && (ring_env ? ring_env[0] == '1' : N >= 48);
+  const bool ring = ring_ok && N >= 48;
   const size_t smem = ring ? smem_ring : fft8::smem_bytes<N>(nk1, nk2);
   auto kern = ring ? fft8::pair_plane_fft8_kernel_ring<N>
                    : (fft8::Geo<N>::MAXREG > 0 ? fft8::pair_plane_fft8_kernel_r<N> : fft8::pair_plane_fft8_kernel_b<N>);
-  static bool attr = false;
-  if (!attr) {
+  if (ctx->attr_once(RPA_ATTR_FFT8 + (N == 24 ? 0 : N == 40 ? 1 : N == 48 ? 2 : 3))) {
     RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_ring<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_r<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_b<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-    attr = true;
-    if (getenv("RPA_VERBOSE")) {
+    if (ctx->opt.verbose) {
       cudaFuncAttributes fa;
       cudaFuncGetAttributes(&fa, kern);
       fprintf(stderr, "[rpa] pair_plane_fft8_kernel<%d>: %d regs, max %d threads/block, launching %d threads, %zu B smem\n", N,
@@ -485,7 +482,7 @@ int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx*
   const long long n_r = ctx->n_r;
   const MtxelSizes sz = mtxel_sizes(ctx, nvb, nc);
   cplx* u_v = ws.get<cplx>((size_t)nvb * n_r);
-  const int n8 = ctx->force_generic_fft ? 0 : fft8_plane_size(ctx);
+  const int n8 = ctx->opt.generic_fft ? 0 : fft8_plane_size(ctx);
   cplx* u_vp = n8 ? ws.get<cplx>((size_t)nvb * N3 * fft8_lane_plane(n8)) : nullptr;
   cplx* u_c = ws.get<cplx>((size_t)sz.ncc * n_r);
   const int nk1 = mp->ax[0].nk, nk2 = mp->ax[1].nk, nk3 = mp->ax[2].nk, J = nk1 * nk2;
@@ -504,7 +501,7 @@ int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx*
   const int LW = (N1 + nwarp - 1) / nwarp;
   const bool prefetch = LW * N2 <= 8 * 32;
   auto kern = prefetch ? pair_plane_kernel<8> : pair_plane_kernel<0>;
-  RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  if (n8 == 0) RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
 
   int rc;
   {
@@ -553,22 +550,20 @@ int mtxel_run(rpa_ctx* ctx, WsAlloc& ws, const cplx* psi_v, int nvb, const cplx*
     {
       ProfScope ps(ctx, RPA_PROF_MTXEL_Z);
       const long long n_lines = (long long)nvb * ncc * J;
-      const bool z8 = !ctx->force_generic_fft && (N3 == 40 || N3 == 120 || N3 == 160) && mp->ax[2].max_res8 <= zfft8::MAXO &&
+      const bool z8 = !ctx->opt.generic_fft && (N3 == 40 || N3 == 120 || N3 == 160) && mp->ax[2].max_res8 <= zfft8::MAXO &&
                       (n_lines + 31) / 32 <= 2147483647LL;
       if (z8) {
         zfft8::Args za;
         za.T = T; za.n_lines = n_lines; za.J = J; za.tw = mp->ax[2].d_tw_fwd; za.kfreq3 = mp->ax[2].d_kfreq; za.nk3 = nk3;
         za.inv_map = mp->d_inv_map; za.M = M; za.ncc = ncc; za.nc = nc; za.c0 = c0; za.n_g = ctx->n_g; za.scale = zs.scale;
-        static bool zattr = false;
-        static int per_sm[3] = {0, 0, 0};   // resident CTAs per SM of the three instantiations (persistent grid)
-        if (!zattr) {
+        int* per_sm = ctx->z_per_sm;   // resident CTAs per SM of the three instantiations (persistent grid)
+        if (ctx->attr_once(RPA_ATTR_ZFFT8)) {
           RPA_CUDA(ctx, cudaFuncSetAttribute(zfft8::z_fft8_scatter_kernel<40>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zfft8::smem_bytes<40>()));
           RPA_CUDA(ctx, cudaFuncSetAttribute(zfft8::z_fft8_scatter_kernel<120>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zfft8::smem_bytes<120>()));
           RPA_CUDA(ctx, cudaFuncSetAttribute(zfft8::z_fft8_scatter_kernel<160>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zfft8::smem_bytes<160>()));
           cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[0], zfft8::z_fft8_scatter_kernel<40>, 32 * 5, zfft8::smem_bytes<40>());
           cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[1], zfft8::z_fft8_scatter_kernel<120>, 32 * 15, zfft8::smem_bytes<120>());
           cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm[2], zfft8::z_fft8_scatter_kernel<160>, 32 * 20, zfft8::smem_bytes<160>());
-          zattr = true;
         }
         const int occ = std::max(1, per_sm[N3 == 40 ? 0 : (N3 == 120 ? 1 : 2)]);
         const unsigned zb = (unsigned)std::min<long long>((n_lines + 31) / 32, (long long)ctx->sm_count * occ);

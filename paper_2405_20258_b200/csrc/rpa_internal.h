@@ -17,8 +17,24 @@ struct rpa_ctx {
   cudaStream_t stream = nullptr;
   std::string err;
   long long launches = 0;
-  bool force_generic_fft = false;  // RPA_GENERIC_FFT=1: use the generic MTXEL plane kernel (tests)
   int sm_count = 148;
+
+  // Diagnostic switches, read ONCE from the environment by rpa_create (listed under "Diagnostics" in rpa_b200.h); the
+  // tests use them to force the routes that the default size rules would not take on small test inputs.
+  struct Options {
+    bool generic_fft = false;      // RPA_GENERIC_FFT=1: generic mixed-radix MTXEL kernels instead of the radix-8 x R ones
+    bool verbose = false;          // RPA_VERBOSE=1: route decisions and kernel resources on stderr
+    bool no_tridiag = false;       // RPA_NO_TRIDIAG=1: a3 skips the tridiagonalisation route (block iteration / Jacobi run)
+    int jacobi_block_min = 1024;   // RPA_JACOBI_BLOCK_MIN: smallest matrix that takes the GEMM block Jacobi
+    int hetrd_mode = -1;           // RPA_HETRD_MODE=0..2: force a large-matrix variant of the tridiagonalisation kernel
+    int hetrd_threads = 0;         // RPA_HETRD_THREADS: its CTA size
+  } opt;
+
+  // Kernel function attributes (dynamic shared memory > 48 KB) are per device: each launch site sets them the first time
+  // THIS context reaches it (attr_once), never once per process.  Resident-CTA counts queried with them live here too.
+  unsigned long long attr_mask = 0;
+  bool attr_once(int id) { const unsigned long long b = 1ull << id; if (attr_mask & b) return false; attr_mask |= b; return true; }
+  int z_per_sm[3] = {0, 0, 0};     // z_fft8_scatter_kernel<40/120/160>
 
   // problem statement
   double cell[9];
@@ -40,6 +56,8 @@ struct rpa_ctx {
 
   // last direct Jacobi eigen-decomposition of the basis stage: matrix size, sweeps, 0 = vector iteration / 1 = block
   int jac_n = 0, jac_sweeps = 0, jac_kind = 0;
+  // what the last basis stage measured on its result: max_i ||chi0 c_i - lambda_i c_i|| / |lambda_1| and max|C C^H - 1|
+  double basis_residual = -1.0, basis_ortho = -1.0;
 
   // per-kernel-class device timers (rpa_profile_begin / rpa_profile_end): event pairs around the launches of a class
   bool prof = false;
@@ -47,6 +65,11 @@ struct rpa_ctx {
   std::vector<ProfRec> prof_recs;
   std::vector<cudaEvent_t> prof_pool;
 };
+
+// attr_once ids
+enum { RPA_ATTR_ZGEMM = 0 /* + 16 layout/HERM combinations */, RPA_ATTR_AXIS = 16 /* + 4 */, RPA_ATTR_FFT8 = 20 /* + 4 */,
+       RPA_ATTR_ZFFT8 = 24, RPA_ATTR_POTRF = 25, RPA_ATTR_TRSM = 26, RPA_ATTR_JACOBI = 27, RPA_ATTR_PLANE_GENERIC = 28 /* + 2 */,
+       RPA_ATTR_WFN = 30 /* + 4 */ };
 
 int rpa_fail(rpa_ctx* ctx, int code, const char* fmt, ...);
 #define RPA_CUDA(ctx, call)                                                              \

@@ -552,12 +552,12 @@ int tridiag_eigh_lowest(rpa_ctx* ctx, WsAlloc& ws, const cplx* H, long long ld, 
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device);
   const size_t row = (size_t)n * sizeof(cplx), cap = 200 * 1024;
   int mode = 3 * row <= cap ? 0 : 2 * row <= cap ? 1 : 2;   // what of v, v_next, w fits in shared memory
-  if (const char* m = getenv("RPA_HETRD_MODE")) mode = std::max(mode, std::min(2, atoi(m)));   // tests: the large-n variants on small matrices
+  if (ctx->opt.hetrd_mode >= 0) mode = std::max(mode, std::min(2, ctx->opt.hetrd_mode));   // tests: the large-n variants on small matrices
   const size_t smem1 = (size_t)(3 - mode) * row;
   if (!coop || smem1 > cap) return RPA_ERR_INVALID;
   const void* fn = mode == 0 ? (const void*)hetrd_fused_kernel<0> : mode == 1 ? (const void*)hetrd_fused_kernel<1> : (const void*)hetrd_fused_kernel<2>;
   // rows resident in registers (mode 3) when a warp per row fits on the device and a row fits in a warp's registers
-  bool rowreg = mode == 0 && n <= 32 * HT_RMAX && !getenv("RPA_HETRD_MODE") && !getenv("RPA_HETRD_THREADS") && !getenv("RPA_HETRD_NO_ROWREG");
+  bool rowreg = mode == 0 && n <= 32 * HT_RMAX && ctx->opt.hetrd_mode < 0 && ctx->opt.hetrd_threads == 0;
   if (rowreg) {
     int ps = 0;
     const void* f3 = (const void*)hetrd_fused_kernel<3>;
@@ -569,13 +569,12 @@ int tridiag_eigh_lowest(rpa_ctx* ctx, WsAlloc& ws, const cplx* H, long long ld, 
   // large matrices stream from HBM: one CTA of 32 warps per SM (the shared-memory rows allow no second CTA); small ones are
   // bound by the barrier latency: few small CTAs
   int nthr = n > 3072 ? 1024 : n > 1536 ? 512 : 256;
-  if (const char* m = getenv("RPA_HETRD_THREADS")) nthr = std::max(64, std::min(1024, atoi(m) & ~31));
+  if (ctx->opt.hetrd_threads > 0) nthr = std::max(64, std::min(1024, ctx->opt.hetrd_threads & ~31));
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, nthr, smem1) != cudaSuccess || per_sm < 1) return RPA_ERR_INVALID;
   // small matrices: no more warps than rows (a cheaper barrier); large ones: every SM (rows are split into chunks when warps > rows)
   const int grid = rowreg ? (n + 7) / 8 : nthr > 256 ? ctx->sm_count * per_sm : std::min(ctx->sm_count * std::min(per_sm, 2), (n + 7) / 8);
   cplx* A_ = Abuf; int n_ = n; cplx* V_ = Vbuf; cplx* tau_ = tau; double* d_ = d; double* e_ = e; cplx* p_ = p;
   int cmax = HT_CMAX;
-  if (const char* m = getenv("RPA_HETRD_CMAX")) cmax = std::max(1, std::min(HT_CMAX, atoi(m)));
   void* args[] = {&A_, &n_, &V_, &tau_, &d_, &e_, &p_, &cmax};
   RPA_CUDA(ctx, cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(nthr), args, smem1, ctx->stream));
   ctx->launches++;

@@ -284,11 +284,8 @@ int launch_h(rpa_ctx* ctx, const KArgs& ka, dim3 grid) {
   constexpr int TB = B_KN ? TILE_KM : TILE_MK;
   constexpr size_t smem = (size_t)STAGES * (TA + TB) * sizeof(cplx) + STAGES * BK * sizeof(double);
   auto kern = zgemm_dmma_kernel<A_KM, B_KN, CONJ_B, STAGES, HERM>;
-  static bool attr_set = false;
-  if (!attr_set) {
+  if (ctx->attr_once(RPA_ATTR_ZGEMM + (A_KM ? 1 : 0) + (B_KN ? 2 : 0) + (CONJ_B ? 4 : 0) + (HERM ? 8 : 0)))
     RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_set = true;
-  }
   kern<<<grid, NTHREADS, smem, ctx->stream>>>(ka);
   RPA_LAUNCH_CHECK(ctx);
   return RPA_OK;
@@ -329,7 +326,7 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
     split = 1;
     int max_split = n_kt / 8;  // at least 8 k-tiles (128 k) per split
     if (base >= 8 * slots) max_split = std::min(max_split, 4);   // many waves already: only trim the last partial wave
-    if (max_split > 1 && base < 8 * slots && !getenv("RPA_ZGEMM_COARSE_SPLIT")) {
+    if (max_split > 1 && base < 8 * slots) {
       // Few tiles (the contractions of the small configs, the Gram matrices of the basis stage): cut K finely and let the
       // block scheduler balance.  Cost model in k-tiles of a full tile: the diagonal tiles of a Hermitian update issue
       // 9/16 of the DMMAs, a CTA pays ~EPI k-tiles for the pipeline fill and the atomic epilogue, and the last CTAs to

@@ -196,20 +196,41 @@ def test_chi_subspace_freq_every_tile_shape(n_eig):
         rpa.rpa_destroy(ctx)
 
 
-@pytest.mark.parametrize("n,n_eig", [(147, 1), (147, 20), (147, 60), (147, 147), (300, 40), (333, 333)])
-def test_subspace_basis_direct_and_iterative(n, n_eig):
-    """a3 alone on random negative-semidefinite matrices with an n^-2/3-like spectrum: direct Jacobi path
-    (2 p > n) and block subspace iteration (small n_eig); eigenvalues, residuals (P13), orthonormality."""
-    check_basis(n, n_eig)
+# Routes of a3 (rpa_basis_info kind / iters_out): 2 = tridiagonalisation + bisection + inverse iteration (default whenever
+# 4 N_eig <= 3 n), 0 = vector one-sided Jacobi, 1 = GEMM block Jacobi (n >= RPA_JACOBI_BLOCK_MIN, default 1024);
+# iters_out > 0 = block subspace iteration + CholeskyQR2 with a Jacobi Rayleigh-Ritz of the p x p projected matrix
+# (north_star's algorithm for a3), reached when the tridiagonal route is off or fails and 2 p <= n.
+@pytest.mark.parametrize("n,n_eig,kind", [(147, 1, 2), (147, 20, 2), (147, 60, 2), (147, 147, 0), (300, 40, 2), (333, 333, 0)])
+def test_subspace_basis_default_routes(n, n_eig, kind):
+    """a3 alone on random negative-semidefinite matrices with an n^-2/3-like spectrum, default route selection: the
+    tridiagonal route for 4 N_eig <= 3 n, the direct vector Jacobi for N_eig = n; eigenvalues, residuals (P13),
+    orthonormality, projector."""
+    check_basis(n, n_eig, expect_kind=kind, expect_iterative=False)
 
 
-@pytest.mark.parametrize("n,n_eig", [(147, 60), (147, 147), (300, 40), (333, 333), (1100, 400)])
-def test_subspace_basis_block_jacobi(n, n_eig, monkeypatch):
-    """The same with the GEMM-rich block Jacobi iteration forced on small matrices (it is the default from
-    n = 1024 up; (1100, 400) takes it by default): ragged last block, zero padding vectors, null eigenvalues."""
-    if n < 1024:
-        monkeypatch.setenv("RPA_JACOBI_BLOCK_MIN", "32")
-    check_basis(n, n_eig)
+@pytest.mark.parametrize("n,n_eig,block_min", [(147, 20, None), (300, 40, None), (1100, 100, None), (300, 40, 32), (2100, 512, None)])
+def test_subspace_basis_block_iteration_forced(n, n_eig, block_min, monkeypatch):
+    """north_star's a3 algorithm: RPA_NO_TRIDIAG=1 sends these sizes to the block subspace iteration with
+    p = 2 N_eig vectors + CholeskyQR2 + one-sided Jacobi Rayleigh-Ritz + residual test.  The Rayleigh-Ritz solver is the
+    vector Jacobi for p < 1024 and the GEMM block Jacobi for p >= 1024 ((2100, 512): p = 1024) or where
+    RPA_JACOBI_BLOCK_MIN forces it ((300, 40) with 32: p = 80)."""
+    monkeypatch.setenv("RPA_NO_TRIDIAG", "1")
+    if block_min:
+        monkeypatch.setenv("RPA_JACOBI_BLOCK_MIN", str(block_min))
+    p = max(2 * n_eig, n_eig + 16)
+    kind = 1 if p >= (block_min or 1024) else 0
+    check_basis(n, n_eig, expect_kind=kind, expect_iterative=True, expect_n=p)
+
+
+@pytest.mark.parametrize("n,n_eig", [(147, 60), (147, 147), (300, 140), (333, 333), (1100, 400)])
+def test_subspace_basis_direct_jacobi_forced(n, n_eig, monkeypatch):
+    """The direct Jacobi eigen-decomposition of the whole matrix (2 p > n) with the tridiagonal route off: vector form,
+    then the GEMM block form forced on the same sizes (it is the default from n = 1024 up: (1100, 400)): ragged last
+    block, zero padding vectors, null eigenvalues."""
+    monkeypatch.setenv("RPA_NO_TRIDIAG", "1")
+    check_basis(n, n_eig, expect_kind=1 if n >= 1024 else 0, expect_iterative=False, expect_n=n)
+    monkeypatch.setenv("RPA_JACOBI_BLOCK_MIN", "32")
+    check_basis(n, n_eig, expect_kind=1, expect_iterative=False, expect_n=n)
 
 
 @pytest.mark.parametrize("mode,threads,n,n_eig", [(1, 256, 147, 60), (2, 256, 300, 40), (2, 1024, 333, 100), (0, 1024, 691, 300)])
@@ -218,10 +239,10 @@ def test_subspace_basis_tridiagonal_variants(mode, threads, n, n_eig, monkeypatc
     32-warp CTAs) forced on small matrices, where the oracle's eigensolver is cheap."""
     monkeypatch.setenv("RPA_HETRD_MODE", str(mode))
     monkeypatch.setenv("RPA_HETRD_THREADS", str(threads))
-    check_basis(n, n_eig)
+    check_basis(n, n_eig, expect_kind=2, expect_iterative=False)
 
 
-def check_basis(n, n_eig):
+def check_basis(n, n_eig, expect_kind=None, expect_iterative=None, expect_n=None):
     import paper_2405_20258_b200 as rpa
     import torch
     rng = np.random.default_rng(n + n_eig)
@@ -231,7 +252,7 @@ def check_basis(n, n_eig):
     H = (q * spec[None, :]) @ q.conj().T
     H = 0.5 * (H + H.conj().T)
     # the basis stage only needs n_g = n: build a context whose epsilon sphere has n points
-    cfgn = RpaConfig("b", 1, (30.0, 30.0, 30.0), (40, 40, 40), 0.3, 0.45 if n <= 600 else 1.1, 1, 1, (-0.6, 0.0), (0.05, 3.0), 1, 2)
+    cfgn = RpaConfig("b", 1, (30.0, 30.0, 30.0), (40, 40, 40), 0.3, 0.45 if n <= 600 else (1.1 if n <= 1400 else 1.7), 1, 1, (-0.6, 0.0), (0.05, 3.0), 1, 2)
     base = make_inputs(cfgn)
     assert base.n_g >= n
     base = dataclasses.replace(base, g_eps=base.g_eps[:n], vcoul=base.vcoul[:n])
@@ -239,12 +260,21 @@ def check_basis(n, n_eig):
     try:
         Cm = torch.empty((n_eig, n), dtype=torch.complex128, device="cuda")
         lam = torch.empty(n_eig, dtype=torch.float64, device="cuda")
-        rpa.rpa_subspace_basis(ctx, dev(H), n_eig, 1e-12, Cm, lam)
+        iters = rpa.rpa_subspace_basis(ctx, dev(H), n_eig, 1e-12, Cm, lam)
         Cg, lg = Cm.cpu().numpy(), lam.cpu().numpy()
+        jn, _, jkind = rpa.rpa_basis_info(ctx)
+        q_res, q_orth = rpa.rpa_basis_quality(ctx)
     finally:
         rpa.rpa_destroy(ctx)
+    if expect_kind is not None:                               # the route the docstring of the calling test names
+        assert jkind == expect_kind, f"route kind {jkind}, expected {expect_kind}"
+    if expect_iterative is not None:
+        assert (iters > 0) == expect_iterative, f"subspace iterations {iters}"
+    if expect_n is not None:
+        assert jn == expect_n
     lref, Cref = orc.subspace_basis(H, n_eig)
     assert eig_rel(lg, lref) <= TOL_LAM
+    assert 0 <= q_res <= 1e-12 and 0 <= q_orth <= 1e-11        # what the library measured on its own result (tol = 1e-12)
     assert np.abs(Cg.conj() @ Cg.T - np.eye(n_eig)).max() <= 1e-12
     res = H @ Cg.T - Cg.T * lg[None, :]
     keep = np.abs(lg) > 1e-12
