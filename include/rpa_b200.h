@@ -142,6 +142,35 @@ int rpa_energy_host(rpa_ctx* ctx, const void* psi_v, int nv, const void* psi_c, 
                     const double* weight, int n_w, int keep_m, double* e_c_out, double* lambda_out,
                     double* per_freq, double* stage_ms);
 
+/* Pass-level calls: the same two-pass loop split at the two points where a multi-GPU run exchanges data (PAPER.md:104-108
+ * eq. 9: conduction bands over ranks; :127-129 eq. 13: the per-rank contributions to chi are summed).  Each rank opens a
+ * sequence on ITS conduction slice; the partial chi~0(0) and chi_s stay inside the workspace, the calls hand out device
+ * pointers to them and the caller reduces them in place (one all-reduce each) before the next call:
+ *
+ *   rpa_pass_begin -> rpa_pass1_chi0 -> [all-reduce chi0] -> rpa_pass_basis(compute on one rank) -> [broadcast C, lambda]
+ *   -> rpa_pass2_chis -> [all-reduce chi_s] -> rpa_pass_energy -> rpa_pass_end
+ *
+ * rpa_energy_device is exactly this sequence with no exchange, so one rank reproduces it bit for bit.  What the library
+ * keeps resident across the valence blocks (all M blocks and the real-space conduction functions, keep_m) is the same.
+ *   rpa_pass_begin   arguments as rpa_energy_device (all dev); timing != 0 records the stage timers.  EXCEPTION to the
+ *                    ownership rule: the library keeps the input pointers until rpa_pass_end -- the arrays must stay alive
+ *                    and unchanged.  Needs rpa_energy_workspace_bytes of workspace.  Ends any sequence still open.
+ *   rpa_pass1_chi0   {a1, a2} over all valence blocks.  *chi0 (optional) = dev pointer INTO THE WORKSPACE [n_g][n_g].
+ *   rpa_pass_basis   compute != 0: a3 on the (reduced) chi0; compute == 0: skip it, the caller fills C and lambda.
+ *                    *C = dev pointer into the workspace [n_eig][n_g], *lambda [n_eig] (both optional).
+ *   rpa_pass2_chis   {a1 again unless M was kept, a4} over all valence blocks.  *chi_s = dev pointer into the workspace
+ *                    [n_w][n_eig][n_eig].
+ *   rpa_pass_energy  a5 on the (reduced) chi_s; outputs as rpa_energy_device.  Synchronises.
+ *   rpa_pass_end     closes the sequence; the pointers handed out become invalid (so do they on rpa_set_workspace).
+ * Calls out of order return RPA_ERR_INVALID.                                                                           */
+int rpa_pass_begin(rpa_ctx* ctx, const void* psi_v, int nv, const void* psi_c, int nc, const double* e_v, const double* e_c,
+                   int nvb, int n_eig, const double* omega, int n_w, int keep_m, int timing);
+int rpa_pass1_chi0(rpa_ctx* ctx, void** chi0);
+int rpa_pass_basis(rpa_ctx* ctx, double tol, int compute, void** C, double** lambda);
+int rpa_pass2_chis(rpa_ctx* ctx, void** chi_s);
+int rpa_pass_energy(rpa_ctx* ctx, const double* weight, double* e_c_out, double* lambda_out, double* per_freq, double* stage_ms);
+int rpa_pass_end(rpa_ctx* ctx);
+
 /* ---------------------------------------------------------------------------------------------------------------------
  * Diagnostics -- NOT part of the method's ABI (nothing below computes any step of the path); used by bench.py, the
  * profiles and the tests.

@@ -7,7 +7,8 @@ from .binding import (RpaContext, RpaError, load_library, library_path, EXPORTED
                       rpa_correlation_energy, rpa_energy_device, rpa_energy_host, rpa_fp64_peak, rpa_launch_count,
                       rpa_profile_begin, rpa_profile_end, PROFILE_CLASSES,
                       rpa_chi0_static_occ, rpa_chi_subspace_freq_occ,
-                      rpa_epsilon_inverse, rpa_epsilon_inverse_workspace_bytes, rpa_basis_info, rpa_basis_quality)
+                      rpa_epsilon_inverse, rpa_epsilon_inverse_workspace_bytes, rpa_basis_info, rpa_basis_quality,
+                      rpa_pass_begin, rpa_pass1_chi0, rpa_pass_basis, rpa_pass2_chis, rpa_pass_energy, rpa_pass_end)
 
 from .sharded import shard_range, Comm, rpa_energy_sharded
 
@@ -17,4 +18,5 @@ __all__ = ["shard_range", "Comm", "rpa_energy_sharded", "RpaContext", "RpaError"
            "rpa_correlation_energy", "rpa_energy_device", "rpa_energy_host", "rpa_fp64_peak", "rpa_launch_count",
            "rpa_profile_begin", "rpa_profile_end", "PROFILE_CLASSES",
            "rpa_chi0_static_occ", "rpa_chi_subspace_freq_occ",
-           "rpa_epsilon_inverse", "rpa_epsilon_inverse_workspace_bytes", "rpa_basis_info", "rpa_basis_quality"]
+           "rpa_epsilon_inverse", "rpa_epsilon_inverse_workspace_bytes", "rpa_basis_info", "rpa_basis_quality",
+           "rpa_pass_begin", "rpa_pass1_chi0", "rpa_pass_basis", "rpa_pass2_chis", "rpa_pass_energy", "rpa_pass_end"]

@@ -19,6 +19,7 @@ EXPORTED_SYMBOLS = [
     "rpa_correlation_energy", "rpa_energy_device", "rpa_energy_host", "rpa_fp64_peak", "rpa_launch_count",
     "rpa_profile_begin", "rpa_profile_end", "rpa_chi0_static_occ", "rpa_chi_subspace_freq_occ",
     "rpa_epsilon_inverse", "rpa_epsilon_inverse_workspace_bytes", "rpa_basis_info", "rpa_basis_quality",
+    "rpa_pass_begin", "rpa_pass1_chi0", "rpa_pass_basis", "rpa_pass2_chis", "rpa_pass_energy", "rpa_pass_end",
 ]
 
 
@@ -85,6 +86,18 @@ def load_library(build_if_missing: bool = True):
     lib.rpa_energy_device.restype = ci
     lib.rpa_energy_host.argtypes = energy_args
     lib.rpa_energy_host.restype = ci
+    lib.rpa_pass_begin.argtypes = [vp, vp, ci, vp, ci, vp, vp, ci, ci, vp, ci, ci, ci]
+    lib.rpa_pass_begin.restype = ci
+    lib.rpa_pass1_chi0.argtypes = [vp, C.POINTER(vp)]
+    lib.rpa_pass1_chi0.restype = ci
+    lib.rpa_pass_basis.argtypes = [vp, cd, ci, C.POINTER(vp), C.POINTER(vp)]
+    lib.rpa_pass_basis.restype = ci
+    lib.rpa_pass2_chis.argtypes = [vp, C.POINTER(vp)]
+    lib.rpa_pass2_chis.restype = ci
+    lib.rpa_pass_energy.argtypes = [vp, vp, pd, pd, pd, pd]
+    lib.rpa_pass_energy.restype = ci
+    lib.rpa_pass_end.argtypes = [vp]
+    lib.rpa_pass_end.restype = ci
     lib.rpa_fp64_peak.argtypes = [vp, ci, ci, pd]
     lib.rpa_fp64_peak.restype = ci
     lib.rpa_profile_begin.argtypes = [vp]
@@ -135,6 +148,7 @@ class RpaContext:
         self.device = device
         self.workspace = None
         self.n_g, self.n_pw = n_g, n_pw
+        self._pass = None
 
     def close(self):
         if self.handle:
@@ -340,6 +354,80 @@ def rpa_energy_host(ctx, psi_v, psi_c, e_v, e_c, nvb, n_eig, tol, omega, weight,
         return C.c_void_p(a.ctypes.data)
 
     return _energy("rpa_energy_host", ctx, psi_v, psi_c, e_v, e_c, nvb, n_eig, tol, omega, weight, keep_m, hptr)
+
+
+def _ws_view(ctx, ptr, dtype, *shape):
+    """A torch view (no copy) of an array the library placed inside the workspace tensor the context was lent."""
+    import torch
+    ws = ctx.workspace
+    if ws is None or ptr is None:
+        raise RpaError(-2, "no workspace tensor is lent to the context")
+    n = int(np.prod(shape)) * torch.empty((), dtype=dtype).element_size()
+    off = int(ptr) - ws.data_ptr()
+    if off < 0 or off + n > ws.numel() * ws.element_size():
+        raise RpaError(-2, "pointer returned by the library lies outside the workspace tensor")
+    return ws[off:off + n].view(dtype).view(*shape)
+
+
+def rpa_pass_begin(ctx, psi_v, psi_c, e_v, e_c, nvb, n_eig, omega, keep_m=True, timing=True):
+    """Opens the pass-level sequence (rpa_b200.h): all inputs are CUDA tensors, kept alive by the context until rpa_pass_end."""
+    import torch
+    nv, nc, n_w = psi_v.shape[0], psi_c.shape[0], omega.shape[0]
+    _shape("psi_v", psi_v, nv, ctx.n_pw)
+    _shape("psi_c", psi_c, nc, ctx.n_pw)
+    _shape("e_v", e_v, nv)
+    _shape("e_c", e_c, nc)
+    if not (1 <= int(n_eig) <= ctx.n_g):
+        raise TypeError(f"n_eig = {n_eig} not in 1..n_g = {ctx.n_g}")
+    c128, f64 = torch.complex128, torch.float64
+    _check(ctx.handle, load_library().rpa_pass_begin(ctx.handle, _dev(psi_v, c128), nv, _dev(psi_c, c128), nc, _dev(e_v, f64), _dev(e_c, f64),
+                                                     int(nvb), int(n_eig), _dev(omega, f64), n_w, int(bool(keep_m)), int(bool(timing))))
+    ctx._pass = dict(refs=(psi_v, psi_c, e_v, e_c, omega), n_eig=int(n_eig), n_w=n_w)
+
+
+def rpa_pass1_chi0(ctx):
+    """{a1, a2} over all valence blocks; returns the partial chi~0(0) [n_g][n_g] as a view into the workspace."""
+    import torch
+    p = C.c_void_p()
+    _check(ctx.handle, load_library().rpa_pass1_chi0(ctx.handle, C.byref(p)))
+    return _ws_view(ctx, p.value, torch.complex128, ctx.n_g, ctx.n_g)
+
+
+def rpa_pass_basis(ctx, tol=0.0, compute=True):
+    """a3 on the (reduced) chi~0(0) when `compute`; returns (C [n_eig][n_g], lambda [n_eig]) as views into the workspace."""
+    import torch
+    pc, pl = C.c_void_p(), C.c_void_p()
+    _check(ctx.handle, load_library().rpa_pass_basis(ctx.handle, float(tol), int(bool(compute)), C.byref(pc), C.byref(pl)))
+    n_eig = ctx._pass["n_eig"]
+    return _ws_view(ctx, pc.value, torch.complex128, n_eig, ctx.n_g), _ws_view(ctx, pl.value, torch.float64, n_eig)
+
+
+def rpa_pass2_chis(ctx):
+    """{a1 unless M was kept, a4} over all valence blocks; returns the partial chi_s [n_w][n_eig][n_eig] (workspace view)."""
+    import torch
+    p = C.c_void_p()
+    _check(ctx.handle, load_library().rpa_pass2_chis(ctx.handle, C.byref(p)))
+    n_eig, n_w = ctx._pass["n_eig"], ctx._pass["n_w"]
+    return _ws_view(ctx, p.value, torch.complex128, n_w, n_eig, n_eig)
+
+
+def rpa_pass_energy(ctx, weight):
+    """a5 on the (reduced) chi_s; same dict as rpa_energy_device."""
+    import torch
+    n_eig, n_w = ctx._pass["n_eig"], ctx._pass["n_w"]
+    _shape("weight", weight, n_w)
+    e = C.c_double(0.0)
+    lam = (C.c_double * n_eig)()
+    per = (C.c_double * n_w)()
+    ms = (C.c_double * 5)()
+    _check(ctx.handle, load_library().rpa_pass_energy(ctx.handle, _dev(weight, torch.float64), C.byref(e), lam, per, ms))
+    return dict(E_c=e.value, lam=np.array(lam[:]), t=np.array(per[:]),
+                stage_ms=dict(zip(("mtxel", "chi0_static", "basis", "chi_freq", "energy"), ms[:])))
+
+
+def rpa_pass_end(ctx):
+    _check(ctx.handle, load_library().rpa_pass_end(ctx.handle))
+    ctx._pass = None
 
 
 def rpa_fp64_peak(ctx, kind: int, iters: int = 20) -> float:

@@ -173,6 +173,8 @@ int rpa_create(rpa_ctx** out, const double cell[9], const int fft[3], int n_g, c
 int rpa_destroy(rpa_ctx* ctx) {
   if (!ctx) return RPA_OK;
   cudaSetDevice(ctx->device);
+  for (auto e : ctx->pass.evs) cudaEventDestroy(e);
+  ctx->pass.evs.clear();
   mtxel_plan_destroy(ctx);
   cudaFree(ctx->d_vsqrt);
   for (auto& r : ctx->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
@@ -234,6 +236,7 @@ size_t rpa_workspace_bytes(const rpa_ctx* ctx, int nvb, int nc, int n_eig, int n
 int rpa_set_workspace(rpa_ctx* ctx, void* dev_ptr, size_t bytes) {
   if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
   if (dev_ptr && ((uintptr_t)dev_ptr & 255)) return rpa_fail(ctx, RPA_ERR_INVALID, "workspace must be 256-byte aligned");
+  if (ctx->pass.active) rpa_pass_end(ctx);   // an open pass sequence lives in the old workspace
   ctx->ws = (char*)dev_ptr;
   ctx->ws_bytes = dev_ptr ? bytes : 0;
   return RPA_OK;
@@ -353,102 +356,188 @@ size_t rpa_energy_workspace_bytes(const rpa_ctx* ctx, int nv, int nc, int nvb, i
   return inputs + energy_persistent_bytes(ctx, nv, nc, nvb, n_eig, n_w, false) + rpa_workspace_bytes(ctx, nvb, nc, n_eig, n_w);
 }
 
-int rpa_energy_device(rpa_ctx* ctx, const void* psi_v_, int nv, const void* psi_c_, int nc, const double* e_v, const double* e_c,
-                      int nvb, int n_eig, double tol, const double* omega, const double* weight, int n_w, int keep_m,
-                      double* e_c_out, double* lambda_out, double* per_freq, double* stage_ms) {
-  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
-  if (!psi_v_ || !psi_c_ || !e_v || !e_c || !omega || !weight || !e_c_out || nv < 1 || nc < 1 || n_w < 1)
-    return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_energy: invalid argument");
-  if (n_eig < 1 || n_eig > ctx->n_g) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_energy: n_eig = %d not in 1..%d", n_eig, ctx->n_g);
-  if (nvb < 1 || nvb > nv) nvb = nv;
-  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
-  const cplx* psi_v = (const cplx*)psi_v_;
-  const cplx* psi_c = (const cplx*)psi_c_;
-  const int n_g = ctx->n_g, n_pw = ctx->n_pw;
-  const int nblocks = (nv + nvb - 1) / nvb;
-  const size_t stage_need = rpa_workspace_bytes(ctx, nvb, nc, n_eig, n_w);
-  bool keep_all = keep_m && nblocks > 0 &&
-                  energy_persistent_bytes(ctx, nv, nc, nvb, n_eig, n_w, true) + stage_need <= ctx->ws_bytes;
-  if (nblocks == 1) keep_all = true;
-  WsAlloc ws(ctx->ws, ctx->ws_bytes);
-  cplx* chi0 = ws.get<cplx>((size_t)n_g * n_g);
-  cplx* C = ws.get<cplx>((size_t)n_eig * n_g);
-  double* lam = ws.get<double>(n_eig);
-  cplx* chi_s = ws.get<cplx>((size_t)n_w * n_eig * n_eig);
-  cplx* Mbuf = ws.get<cplx>((size_t)(keep_all ? nv : nvb) * nc * n_g);
-  if (!ws.ok || ws.off + stage_need > ctx->ws_bytes)
-    return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_energy: workspace too small (need %zu bytes, have %zu)", ws.off + stage_need,
-                    ctx->ws_bytes);
-  // several MTXEL calls on the same conduction bands: keep their real-space functions too if there is room
-  const int n_mtxel = keep_all ? nblocks : 2 * nblocks;
-  const size_t per_band = (size_t)ctx->n_r * sizeof(cplx);
+// The two-pass loop, split at the points where a multi-GPU run exchanges data (rpa_b200.h "Pass-level calls").  The state
+// lives in ctx->pass between rpa_pass_begin and rpa_pass_end; rpa_energy_device is these calls in sequence.
+namespace {
+
+void pass_tic(rpa_ctx* ctx, int stage) {
+  rpa_ctx::PassState& ps = ctx->pass;
+  if (!ps.timing) return;
+  cudaEvent_t a; cudaEventCreate(&a); cudaEventRecord(a, ctx->stream); ps.evs.push_back(a); ps.ev_stage.push_back(stage);
+}
+void pass_toc(rpa_ctx* ctx) {
+  rpa_ctx::PassState& ps = ctx->pass;
+  if (!ps.timing) return;
+  cudaEvent_t b; cudaEventCreate(&b); cudaEventRecord(b, ctx->stream); ps.evs.push_back(b); ps.ev_stage.push_back(-1);
+}
+void pass_reset(rpa_ctx* ctx) {
+  rpa_ctx::PassState& ps = ctx->pass;
+  for (auto e : ps.evs) cudaEventDestroy(e);
+  ps = rpa_ctx::PassState();
   ctx->uc_cache = nullptr; ctx->uc_cache_filled = false; ctx->uc_cache_rows = 0;
+}
+int pass_need(rpa_ctx* ctx, const char* who, int stage) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  if (!ctx->pass.active) return rpa_fail(ctx, RPA_ERR_INVALID, "%s: no pass sequence is open (call rpa_pass_begin first)", who);
+  if (ctx->pass.stage != stage)
+    return rpa_fail(ctx, RPA_ERR_INVALID, "%s: called out of order (the sequence is begin, pass1, basis, pass2, energy, end)", who);
+  return RPA_OK;
+}
+
+}  // namespace
+
+int rpa_pass_begin(rpa_ctx* ctx, const void* psi_v, int nv, const void* psi_c, int nc, const double* e_v, const double* e_c, int nvb,
+                   int n_eig, const double* omega, int n_w, int keep_m, int timing) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  if (!psi_v || !psi_c || !e_v || !e_c || !omega || nv < 1 || nc < 1 || n_w < 1) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_pass_begin: invalid argument");
+  if (n_eig < 1 || n_eig > ctx->n_g) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_pass_begin: n_eig = %d not in 1..%d", n_eig, ctx->n_g);
+  if (nvb < 1 || nvb > nv) nvb = nv;
+  if ((long long)nvb * nc > 2147483647LL) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_pass_begin: too many pairs in one block");
+  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
+  pass_reset(ctx);
+  rpa_ctx::PassState& ps = ctx->pass;
+  const int n_g = ctx->n_g;
+  ps.psi_v = (const cplx*)psi_v; ps.psi_c = (const cplx*)psi_c; ps.e_v = e_v; ps.e_c = e_c; ps.omega = omega;
+  ps.nv = nv; ps.nc = nc; ps.nvb = nvb; ps.n_eig = n_eig; ps.n_w = n_w; ps.timing = timing != 0;
+  ps.nblocks = (nv + nvb - 1) / nvb;
+  const size_t stage_need = rpa_workspace_bytes(ctx, nvb, nc, n_eig, n_w);
+  ps.keep_all = keep_m && energy_persistent_bytes(ctx, nv, nc, nvb, n_eig, n_w, true) + stage_need <= ctx->ws_bytes;
+  if (ps.nblocks == 1) ps.keep_all = true;
+  WsAlloc ws(ctx->ws, ctx->ws_bytes);
+  ps.chi0 = ws.get<cplx>((size_t)n_g * n_g);
+  ps.C = ws.get<cplx>((size_t)n_eig * n_g);
+  ps.lam = ws.get<double>(n_eig);
+  ps.chi_s = ws.get<cplx>((size_t)n_w * n_eig * n_eig);
+  ps.Mbuf = ws.get<cplx>((size_t)(ps.keep_all ? nv : nvb) * nc * n_g);
+  if (!ws.ok || ws.off + stage_need > ctx->ws_bytes) {
+    const size_t need = ws.off + stage_need;
+    pass_reset(ctx);
+    return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_energy: workspace too small (need %zu bytes, have %zu)", need, ctx->ws_bytes);
+  }
+  // several MTXEL calls on the same conduction bands: keep their real-space functions too if there is room
+  const int n_mtxel = ps.keep_all ? ps.nblocks : 2 * ps.nblocks;
+  const size_t per_band = (size_t)ctx->n_r * sizeof(cplx);
   if (keep_m && n_mtxel > 1 && ws.off + stage_need + 256 < ctx->ws_bytes) {
     const size_t room = ctx->ws_bytes - ws.off - stage_need - 256;
     const int rows = (int)std::min<size_t>((size_t)nc, room / per_band);   // as many bands as fit: the rest is recomputed
     if (rows >= 64 || rows == nc) {
       ctx->uc_cache = ws.get<cplx>((size_t)rows * ctx->n_r);
-      ctx->uc_cache_src = psi_c; ctx->uc_cache_nc = nc; ctx->uc_cache_rows = rows;
+      ctx->uc_cache_src = ps.psi_c; ctx->uc_cache_nc = nc; ctx->uc_cache_rows = rows;
     }
   }
-  struct CacheGuard { rpa_ctx* c; ~CacheGuard() { c->uc_cache = nullptr; c->uc_cache_filled = false; } } cache_guard{ctx};
-  char* scratch = ctx->ws + ws.off;
-  const size_t scratch_bytes = ctx->ws_bytes - ws.off;
+  ps.scratch = ctx->ws + ws.off;
+  ps.scratch_bytes = ctx->ws_bytes - ws.off;
+  ps.active = true; ps.stage = 0;
+  return RPA_OK;
+}
 
-  // stage timers: events are recorded around every stage call and summed after the final synchronisation
-  std::vector<cudaEvent_t> evs;
-  std::vector<int> ev_stage;
-  auto tic = [&](int stage) {
-    if (!stage_ms) return;
-    cudaEvent_t a; cudaEventCreate(&a); cudaEventRecord(a, ctx->stream); evs.push_back(a); ev_stage.push_back(stage);
-  };
-  auto toc = [&]() {
-    if (!stage_ms) return;
-    cudaEvent_t b; cudaEventCreate(&b); cudaEventRecord(b, ctx->stream); evs.push_back(b); ev_stage.push_back(-1);
-  };
-  auto cleanup = [&]() { for (auto e : evs) cudaEventDestroy(e); };
-  int rc = RPA_OK;
-  for (int b = 0; b < nblocks && !rc; b++) {  // pass 1: MTXEL + static CHI_SUM (eq. 15)
-    const int v0 = b * nvb, nb = std::min(nvb, nv - v0);
-    cplx* M = keep_all ? Mbuf + (size_t)v0 * nc * n_g : Mbuf;
-    WsAlloc s1(scratch, scratch_bytes);
-    tic(0); rc = mtxel_run(ctx, s1, psi_v + (size_t)v0 * n_pw, nb, psi_c, nc, M); toc();
+int rpa_pass1_chi0(rpa_ctx* ctx, void** chi0_out) {   // MTXEL + static CHI_SUM over all valence blocks (eq. 15)
+  int rc = pass_need(ctx, "rpa_pass1_chi0", 0);
+  if (rc) return rc;
+  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
+  rpa_ctx::PassState& ps = ctx->pass;
+  const int n_g = ctx->n_g, n_pw = ctx->n_pw;
+  for (int b = 0; b < ps.nblocks && !rc; b++) {
+    const int v0 = b * ps.nvb, nb = std::min(ps.nvb, ps.nv - v0);
+    cplx* M = ps.keep_all ? ps.Mbuf + (size_t)v0 * ps.nc * n_g : ps.Mbuf;
+    WsAlloc s1(ps.scratch, ps.scratch_bytes);
+    pass_tic(ctx, 0); rc = mtxel_run(ctx, s1, ps.psi_v + (size_t)v0 * n_pw, nb, ps.psi_c, ps.nc, M); pass_toc(ctx);
     if (rc) break;
-    WsAlloc s2(scratch, scratch_bytes);
-    tic(1); rc = do_chi0_static(ctx, s2, M, nb, nc, e_v + v0, e_c, b > 0, chi0); toc();
+    WsAlloc s2(ps.scratch, ps.scratch_bytes);
+    pass_tic(ctx, 1); rc = do_chi0_static(ctx, s2, M, nb, ps.nc, ps.e_v + v0, ps.e_c, b > 0, ps.chi0); pass_toc(ctx);
   }
-  if (!rc) {
-    WsAlloc s2(scratch, scratch_bytes);
-    tic(2); rc = basis_run(ctx, s2, chi0, n_g, n_eig, tol, C, lam, nullptr); toc();
+  if (rc) return rc;
+  ps.stage = 1;
+  if (chi0_out) *chi0_out = ps.chi0;
+  return RPA_OK;
+}
+
+int rpa_pass_basis(rpa_ctx* ctx, double tol, int compute, void** C_out, double** lambda_out) {
+  int rc = pass_need(ctx, "rpa_pass_basis", 1);
+  if (rc) return rc;
+  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
+  rpa_ctx::PassState& ps = ctx->pass;
+  if (compute) {
+    WsAlloc s2(ps.scratch, ps.scratch_bytes);
+    pass_tic(ctx, 2); rc = basis_run(ctx, s2, ps.chi0, ctx->n_g, ps.n_eig, tol, ps.C, ps.lam, nullptr); pass_toc(ctx);
+    if (rc) return rc;
   }
-  for (int b = 0; b < nblocks && !rc; b++) {  // pass 2: (MTXEL again) + projected chi_s(i w)
-    const int v0 = b * nvb, nb = std::min(nvb, nv - v0);
-    cplx* M = keep_all ? Mbuf + (size_t)v0 * nc * n_g : Mbuf;
-    if (!keep_all) {
-      WsAlloc s1(scratch, scratch_bytes);
-      tic(0); rc = mtxel_run(ctx, s1, psi_v + (size_t)v0 * n_pw, nb, psi_c, nc, M); toc();
+  ps.stage = 2;
+  if (C_out) *C_out = ps.C;
+  if (lambda_out) *lambda_out = ps.lam;
+  return RPA_OK;
+}
+
+int rpa_pass2_chis(rpa_ctx* ctx, void** chi_s_out) {   // (MTXEL again) + projected chi_s(i w) over all valence blocks
+  int rc = pass_need(ctx, "rpa_pass2_chis", 2);
+  if (rc) return rc;
+  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
+  rpa_ctx::PassState& ps = ctx->pass;
+  const int n_g = ctx->n_g, n_pw = ctx->n_pw;
+  for (int b = 0; b < ps.nblocks && !rc; b++) {
+    const int v0 = b * ps.nvb, nb = std::min(ps.nvb, ps.nv - v0);
+    cplx* M = ps.keep_all ? ps.Mbuf + (size_t)v0 * ps.nc * n_g : ps.Mbuf;
+    if (!ps.keep_all) {
+      WsAlloc s1(ps.scratch, ps.scratch_bytes);
+      pass_tic(ctx, 0); rc = mtxel_run(ctx, s1, ps.psi_v + (size_t)v0 * n_pw, nb, ps.psi_c, ps.nc, M); pass_toc(ctx);
       if (rc) break;
     }
-    WsAlloc s3(scratch, scratch_bytes);
-    tic(3); rc = do_chi_freq(ctx, s3, M, nb, nc, e_v + v0, e_c, C, n_eig, omega, n_w, b > 0, chi_s); toc();
+    WsAlloc s3(ps.scratch, ps.scratch_bytes);
+    pass_tic(ctx, 3); rc = do_chi_freq(ctx, s3, M, nb, ps.nc, ps.e_v + v0, ps.e_c, ps.C, ps.n_eig, ps.omega, ps.n_w, b > 0, ps.chi_s); pass_toc(ctx);
   }
-  if (!rc) {
-    WsAlloc s4(scratch, scratch_bytes);
-    tic(4); rc = energy_run(ctx, s4, chi_s, n_eig, weight, n_w, e_c_out, per_freq); toc();
+  if (rc) return rc;
+  ps.stage = 3;
+  if (chi_s_out) *chi_s_out = ps.chi_s;
+  return RPA_OK;
+}
+
+int rpa_pass_energy(rpa_ctx* ctx, const double* weight, double* e_c_out, double* lambda_out, double* per_freq, double* stage_ms) {
+  int rc = pass_need(ctx, "rpa_pass_energy", 3);
+  if (rc) return rc;
+  if (!weight || !e_c_out) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_pass_energy: null argument");
+  RPA_CUDA(ctx, cudaSetDevice(ctx->device));
+  rpa_ctx::PassState& ps = ctx->pass;
+  {
+    WsAlloc s4(ps.scratch, ps.scratch_bytes);
+    pass_tic(ctx, 4); rc = energy_run(ctx, s4, ps.chi_s, ps.n_eig, weight, ps.n_w, e_c_out, per_freq); pass_toc(ctx);
   }
-  if (rc) { cleanup(); return rc; }
-  if (lambda_out) RPA_CUDA(ctx, cudaMemcpyAsync(lambda_out, lam, n_eig * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+  if (rc) return rc;
+  if (lambda_out) RPA_CUDA(ctx, cudaMemcpyAsync(lambda_out, ps.lam, ps.n_eig * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
   RPA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
   if (stage_ms) {
     for (int s = 0; s < 5; s++) stage_ms[s] = 0.0;
-    for (size_t i = 0; i + 1 < evs.size(); i += 2) {
+    for (size_t i = 0; i + 1 < ps.evs.size(); i += 2) {
       float ms = 0.f;
-      cudaEventElapsedTime(&ms, evs[i], evs[i + 1]);
-      stage_ms[ev_stage[i]] += ms;
+      cudaEventElapsedTime(&ms, ps.evs[i], ps.evs[i + 1]);
+      stage_ms[ps.ev_stage[i]] += ms;
     }
   }
-  cleanup();
+  ps.stage = 4;
   return RPA_OK;
+}
+
+int rpa_pass_end(rpa_ctx* ctx) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  cudaSetDevice(ctx->device);
+  pass_reset(ctx);
+  return RPA_OK;
+}
+
+int rpa_energy_device(rpa_ctx* ctx, const void* psi_v, int nv, const void* psi_c, int nc, const double* e_v, const double* e_c,
+                      int nvb, int n_eig, double tol, const double* omega, const double* weight, int n_w, int keep_m,
+                      double* e_c_out, double* lambda_out, double* per_freq, double* stage_ms) {
+  if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
+  if (!psi_v || !psi_c || !e_v || !e_c || !omega || !weight || !e_c_out || nv < 1 || nc < 1 || n_w < 1)
+    return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_energy: invalid argument");
+  int rc = rpa_pass_begin(ctx, psi_v, nv, psi_c, nc, e_v, e_c, nvb, n_eig, omega, n_w, keep_m, stage_ms != nullptr);
+  if (!rc) rc = rpa_pass1_chi0(ctx, nullptr);
+  if (!rc) rc = rpa_pass_basis(ctx, tol, 1, nullptr, nullptr);
+  if (!rc) rc = rpa_pass2_chis(ctx, nullptr);
+  if (!rc) rc = rpa_pass_energy(ctx, weight, e_c_out, lambda_out, per_freq, stage_ms);
+  const std::string err = ctx->err;
+  rpa_pass_end(ctx);
+  if (rc) ctx->err = err;
+  return rc;
 }
 
 int rpa_energy_host(rpa_ctx* ctx, const void* psi_v, int nv, const void* psi_c, int nc, const double* e_v, const double* e_c,

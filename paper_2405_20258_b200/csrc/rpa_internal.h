@@ -54,6 +54,18 @@ struct rpa_ctx {
   // array uc_cache_src, [uc_cache_rows][n_r]
   cplx* uc_cache = nullptr; const cplx* uc_cache_src = nullptr; int uc_cache_nc = 0, uc_cache_rows = 0; bool uc_cache_filled = false;
 
+  // the two-pass loop between rpa_pass_begin and rpa_pass_end (api.cu): caller's inputs, the persistent part of the
+  // workspace (chi~0, C, lambda, chi_s, the M block or all of M) and the stage timers
+  struct PassState {
+    bool active = false, keep_all = false, timing = false;
+    int stage = 0;   // 0 begun, 1 pass 1 done, 2 basis set, 3 pass 2 done, 4 energy done
+    const cplx* psi_v = nullptr; const cplx* psi_c = nullptr; const double* e_v = nullptr; const double* e_c = nullptr; const double* omega = nullptr;
+    int nv = 0, nc = 0, nvb = 0, n_eig = 0, n_w = 0, nblocks = 0;
+    cplx* chi0 = nullptr; cplx* C = nullptr; cplx* chi_s = nullptr; cplx* Mbuf = nullptr; double* lam = nullptr;
+    char* scratch = nullptr; size_t scratch_bytes = 0;
+    std::vector<cudaEvent_t> evs; std::vector<int> ev_stage;
+  } pass;
+
   // last direct Jacobi eigen-decomposition of the basis stage: matrix size, sweeps, 0 = vector iteration / 1 = block
   int jac_n = 0, jac_sweeps = 0, jac_kind = 0;
   // what the last basis stage measured on its result: max_i ||chi0 c_i - lambda_i c_i|| / |lambda_1| and max|C C^H - 1|

@@ -3,9 +3,11 @@
 PAPER.md:104-108 eq. 9 distributes the conduction bands over ranks and PAPER.md:127-129 sums the per-rank
 contributions to chi0.  On NVLink/NVSwitch that sum is ONE all-reduce per pass (chi~0(0): 2 N_G^2 doubles, chi_s:
 2 N_w N_eig^2 doubles): every rank runs a1/a2 on its own conduction slice, the partial chi~0(0) are summed, rank 0's
-subspace basis is broadcast (the basis must be bit-identical on all ranks), every rank runs a1/a4 on its slice, the
-partial chi_s are summed, and a5 runs replicated.  All arithmetic is in the C-ABI kernels; `torch.distributed` is the
-plumbing for the two collectives.  With world size 1 (or no process group) the collectives are no-ops.
+subspace basis is broadcast (the basis must be bit-identical on all ranks: a3's split-K sums meet in an order that is
+not fixed, so it is computed once), every rank runs a1/a4 on its slice, the partial chi_s are summed, and a5 runs
+replicated.  All arithmetic AND the valence-block loop are in the C-ABI library (its pass-level calls);
+`torch.distributed` is the plumbing for the two collectives.  With world size 1 (or no process group) the collectives
+are no-ops.
 """
 from __future__ import annotations
 
@@ -45,57 +47,48 @@ class Comm:
         return t
 
 
-def rpa_energy_sharded(ctx, psi_v, psi_c_local, e_v, e_c_local, nvb, n_eig, tol, omega, weight, comm=None, keep_m=True):
+def rpa_energy_sharded(ctx, psi_v, psi_c_local, e_v, e_c_local, nvb, n_eig, tol, omega, weight, comm=None, keep_m=True,
+                       backend=None):
     """E_c with this rank's conduction slice (`psi_c_local` [nc_local][n_pw], `e_c_local`), all valence bands on every rank.
 
-    The context's workspace must hold rpa_workspace_bytes(ctx, nvb, nc_local, n_eig, n_w).  Returns the same dict as
-    rpa_energy_device (stage_ms from CUDA events on the current stream, plus 'allreduce')."""
+    Runs the library's pass-level calls (rpa_b200.h): the valence-block loop, the resident M blocks and the cached
+    real-space conduction functions are the single-GPU driver's own -- nothing is allocated per block here.  The partial
+    chi~0(0) and chi_s live in the workspace and are reduced in place.  The context's workspace must hold
+    rpa_energy_workspace_bytes(ctx, nv, nc_local, nvb, n_eig, n_w) (more lets the library keep M and u_c resident).
+    Returns the same dict as rpa_energy_device; stage_ms has an extra 'allreduce' entry (both reductions and the
+    broadcast, CUDA events on the current stream).  With one rank it is the very sequence rpa_energy_device runs.
+    `backend` (default: the ctypes binding) supplies the six rpa_pass_* calls; the CPU tests of the host logic pass a
+    stand-in, the product never does."""
     import torch
-    from . import binding as rpa
+    if backend is None:
+        from . import binding as backend
+    rpa = backend
 
     comm = comm or Comm()
-    dev = psi_v.device
-    nv, nc, ng, n_w = psi_v.shape[0], psi_c_local.shape[0], ctx_n_g(ctx, psi_v), omega.shape[0]
-    blocks = [(s, min(nv, s + nvb)) for s in range(0, nv, nvb)]
-    ms = {k: 0.0 for k in ("mtxel", "chi0_static", "basis", "chi_freq", "energy", "allreduce")}
     marks = []
 
-    def timed(stage, fn):
+    def exchange(fn):
+        if not psi_v.is_cuda:        # host-logic tests on CPU tensors: no device timers
+            return fn()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record()
-        out = fn()
+        fn()
         b.record()
-        marks.append((stage, a, b))
-        return out
+        marks.append((a, b))
 
-    chi0 = torch.zeros((ng, ng), dtype=torch.complex128, device=dev)
-    kept = []
-    for i, (s, e) in enumerate(blocks):                                   # pass 1 (PAPER.md:152 eq. 15)
-        M = torch.empty((e - s, nc, ng), dtype=torch.complex128, device=dev)
-        timed("mtxel", lambda: rpa.rpa_mtxel(ctx, psi_v[s:e].contiguous(), psi_c_local, M))
-        timed("chi0_static", lambda: rpa.rpa_chi0_static(ctx, M, e_v[s:e].contiguous(), e_c_local, i > 0, chi0))
-        if keep_m:
-            kept.append(M)
-    timed("allreduce", lambda: comm.allreduce_sum_(chi0))                 # sum over ranks (PAPER.md:127 eq. 13)
-    Cmat = torch.empty((n_eig, ng), dtype=torch.complex128, device=dev)
-    lam = torch.empty(n_eig, dtype=torch.float64, device=dev)
-    if comm.rank == 0:
-        timed("basis", lambda: rpa.rpa_subspace_basis(ctx, chi0, n_eig, tol, Cmat, lam))
-    timed("allreduce", lambda: (comm.broadcast_(Cmat), comm.broadcast_(lam)))
-    chi_s = torch.zeros((n_w, n_eig, n_eig), dtype=torch.complex128, device=dev)
-    for i, (s, e) in enumerate(blocks):                                   # pass 2 (PAPER.md:158)
-        if keep_m:
-            M = kept[i]
-        else:
-            M = torch.empty((e - s, nc, ng), dtype=torch.complex128, device=dev)
-            timed("mtxel", lambda: rpa.rpa_mtxel(ctx, psi_v[s:e].contiguous(), psi_c_local, M))
-        timed("chi_freq", lambda: rpa.rpa_chi_subspace_freq(ctx, M, e_v[s:e].contiguous(), e_c_local, Cmat, n_eig, omega, i > 0, chi_s))
-    timed("allreduce", lambda: comm.allreduce_sum_(chi_s))
-    e_c, t = timed("energy", lambda: rpa.rpa_correlation_energy(ctx, chi_s, n_eig, weight))
-    torch.cuda.synchronize(dev)
-    for stage, a, b in marks:
-        ms[stage] += a.elapsed_time(b)
-    return dict(E_c=e_c, t=t, lam=lam.cpu().numpy(), stage_ms=ms)
+    rpa.rpa_pass_begin(ctx, psi_v, psi_c_local, e_v, e_c_local, nvb, n_eig, omega, keep_m=keep_m, timing=True)
+    try:
+        chi0 = rpa.rpa_pass1_chi0(ctx)                                  # pass 1 on this rank's pairs (PAPER.md:152 eq. 15)
+        exchange(lambda: comm.allreduce_sum_(chi0))                     # sum over ranks (PAPER.md:127 eq. 13)
+        Cmat, lam = rpa.rpa_pass_basis(ctx, tol, compute=comm.rank == 0)
+        exchange(lambda: (comm.broadcast_(Cmat), comm.broadcast_(lam)))  # one basis, bit-identical on every rank
+        chi_s = rpa.rpa_pass2_chis(ctx)                                 # pass 2 (PAPER.md:158)
+        exchange(lambda: comm.allreduce_sum_(chi_s))
+        out = rpa.rpa_pass_energy(ctx, weight)                          # replicated; synchronises
+    finally:
+        rpa.rpa_pass_end(ctx)
+    out["stage_ms"]["allreduce"] = sum(a.elapsed_time(b) for a, b in marks)
+    return out
 
 
 def ctx_n_g(ctx, like):

@@ -22,6 +22,12 @@ def cfg_small_grid(fft, cell, ecw, ece, n_v=3, n_c=9, seed=5, n_eig=4, n_w=6):
     return RpaConfig("t", seed, cell, fft, ecw, ece, n_v, n_c, (-0.6, 0.0), (0.05, 3.0), n_eig, n_w)
 
 
+def rpa_energy_extra(inp, nv, nc, nvb, n_eig, n_w, keep_all=False):
+    """bytes beyond make_ctx's stage workspace that the whole-path driver needs (inputs excluded: they are device tensors)"""
+    ng = inp.n_g
+    return 16 * (ng * ng + n_eig * ng + n_w * n_eig * n_eig + (nv if keep_all else nvb) * nc * ng) + 8 * n_eig + (1 << 16)
+
+
 def check_all(inp, n_eig, nvb=None, full_basis=False):
     import paper_2405_20258_b200 as rpa
     nv, nc = inp.psi_v.shape[0], inp.psi_c.shape[0]
@@ -388,15 +394,16 @@ def test_small_config_full_against_golden():
 
 
 def test_sharded_driver_single_rank_and_emulated_two_shards():
-    """rpa_energy_sharded (the multi-GPU driver) with one rank against the oracle, and its shard arithmetic on ONE GPU:
-    the conduction bands are split with shard_range, each shard's partial chi~0(0) / chi_s comes from the stage calls one
-    after the other (no kernel waits on another), and their sums must reproduce the unsharded result."""
+    """rpa_energy_sharded (the multi-GPU driver, built on the library's pass-level calls) with one rank against the oracle
+    and against rpa_energy_device, and the shard arithmetic on ONE GPU: the conduction bands are split with shard_range,
+    each shard's partial chi~0(0) / chi_s comes from the stage calls one after the other (no kernel waits on another), and
+    their sums must reproduce the unsharded result."""
     import paper_2405_20258_b200 as rpa
     import torch
     inp = make_inputs(0)
     ref = orc.rpa_energy(inp)
     nv, nc, ng, n_eig, n_w = 8, 200, inp.n_g, inp.cfg.n_eig, len(inp.omega)
-    ctx = make_ctx(inp, 4, nc, n_eig, n_w)
+    ctx = make_ctx(inp, 4, nc, n_eig, n_w, extra_bytes=rpa_energy_extra(inp, nv, nc, 3, n_eig, n_w))
     try:
         psi_v, psi_c, e_v, e_c = dev(inp.psi_v), dev(inp.psi_c), dev(inp.e_v), dev(inp.e_c)
         omega, weight = dev(inp.omega), dev(inp.weight)
@@ -404,6 +411,19 @@ def test_sharded_driver_single_rank_and_emulated_two_shards():
             r = rpa.rpa_energy_sharded(ctx, psi_v, psi_c, e_v, e_c, 3, n_eig, 0.0, omega, weight, keep_m=keep)
             assert abs(r["E_c"] - ref["E_c"]) <= TOL_E * abs(ref["E_c"])
             assert eig_rel(r["lam"], ref["lam"]) <= TOL_LAM
+            d = rpa.rpa_energy_device(ctx, psi_v, psi_c, e_v, e_c, 3, n_eig, 0.0, omega, weight, keep_m=keep)
+            # the same sequence of launches; split-K partial sums meet through atomics, so the last bits may differ
+            assert abs(r["E_c"] - d["E_c"]) <= 1e-13 * abs(d["E_c"])
+            assert set(r["stage_ms"]) == set(d["stage_ms"]) | {"allreduce"}
+        # the pass-level calls refuse to run out of order, and the views they hand out lie in the workspace
+        with pytest.raises(rpa.RpaError):
+            rpa.rpa_pass1_chi0(ctx)
+        rpa.rpa_pass_begin(ctx, psi_v, psi_c, e_v, e_c, 3, n_eig, omega)
+        with pytest.raises(rpa.RpaError):
+            rpa.rpa_pass2_chis(ctx)
+        chi0_v = rpa.rpa_pass1_chi0(ctx)
+        assert maxnorm_rel(chi0_v.cpu().numpy(), ref["chi0"]) <= TOL_CHI
+        rpa.rpa_pass_end(ctx)
         chi0 = torch.zeros((ng, ng), dtype=torch.complex128, device="cuda")
         parts = [rpa.shard_range(nc, 3, k) for k in range(3)]
         Ms = []
@@ -456,6 +476,36 @@ def test_medium_twin_against_golden():
     mu_ref = np.array(g["chi_s_eigs_first_freq"])
     assert np.abs(mu - mu_ref).max() <= 1e-10 * np.abs(mu_ref).max()
     assert g["E_c_full"] < g["E_c"] < 0
+
+
+def test_sharded_single_rank_costs_what_the_device_driver_costs():
+    """On the configs[2] twin (1/16 of the bands, valence blocks of 8, M and u_c kept resident) the one-rank sharded
+    driver must give rpa_energy_device's E_c and take the same time: it runs the same pass-level calls and keeps the same
+    caches (the round-1 version re-transformed every conduction band for every block)."""
+    import time
+    import paper_2405_20258_b200 as rpa
+    import torch
+    inp = make_inputs(2, n_v=16, n_c=375)
+    nv, nc, n_eig, n_w = 16, 375, inp.cfg.n_eig, len(inp.omega)
+    ctx = rpa.rpa_create(inp.cell, inp.fft, inp.g_eps, inp.vcoul, inp.g_wfn)
+    try:
+        need = rpa.rpa_energy_workspace_bytes(ctx, nv, nc, 8, n_eig, n_w) + nv * nc * inp.n_g * 16 + nc * int(np.prod(inp.fft)) * 16
+        rpa.rpa_set_workspace(ctx, torch.empty(need, dtype=torch.uint8, device="cuda"))
+        a = [dev(getattr(inp, k)) for k in ("psi_v", "psi_c", "e_v", "e_c")]
+        omega, weight = dev(inp.omega), dev(inp.weight)
+        best = {}
+        for name, fn in (("device", rpa.rpa_energy_device), ("sharded", rpa.rpa_energy_sharded)):
+            for _ in range(3):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                r = fn(ctx, *a, 8, n_eig, 0.0, omega, weight, keep_m=True)
+                torch.cuda.synchronize()
+                best[name] = min(best.get(name, 1e9), time.perf_counter() - t0)
+            best[name + "_E"] = r["E_c"]
+        assert abs(best["sharded_E"] - best["device_E"]) <= 1e-13 * abs(best["device_E"])
+        assert best["sharded"] <= 1.03 * best["device"] + 2e-3, best
+    finally:
+        rpa.rpa_destroy(ctx)
 
 
 def test_medium_config_full_size_sampled_and_properties():
