@@ -28,6 +28,7 @@ struct rpa_ctx {
     int jacobi_block_min = 1024;   // RPA_JACOBI_BLOCK_MIN: smallest matrix that takes the GEMM block Jacobi
     int hetrd_mode = -1;           // RPA_HETRD_MODE=0..2: force a large-matrix variant of the tridiagonalisation kernel
     int hetrd_threads = 0;         // RPA_HETRD_THREADS: its CTA size
+    bool zgemm_3m = false;         // RPA_ZGEMM_3M=1: Hermitian updates with the 3-multiply complex product (zherk3m_kernel)
   } opt;
 
   // Kernel function attributes (dynamic shared memory > 48 KB) are per device: each launch site sets them the first time
@@ -81,7 +82,7 @@ struct rpa_ctx {
 // attr_once ids
 enum { RPA_ATTR_ZGEMM = 0 /* + 16 layout/HERM combinations */, RPA_ATTR_AXIS = 16 /* + 4 */, RPA_ATTR_FFT8 = 20 /* + 4 */,
        RPA_ATTR_ZFFT8 = 24, RPA_ATTR_POTRF = 25, RPA_ATTR_TRSM = 26, RPA_ATTR_JACOBI = 27, RPA_ATTR_PLANE_GENERIC = 28 /* + 2 */,
-       RPA_ATTR_WFN = 30 /* + 4 */ };
+       RPA_ATTR_WFN = 30 /* + 4 */, RPA_ATTR_ZHERK3M = 34 };
 
 int rpa_fail(rpa_ctx* ctx, int code, const char* fmt, ...);
 #define RPA_CUDA(ctx, call)                                                              \

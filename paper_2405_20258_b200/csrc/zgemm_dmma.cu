@@ -267,6 +267,164 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// 3M variant of the Hermitian [k][m] x [k][n] update (CHI_SUM, chi_s): the complex product with THREE real products
+// (Karatsuba) instead of four,
+//
+//   P += ar br,  Q += ai bi,  R += (ar + ai)(br - bi);      Re(a conj b) = P + Q,  Im(a conj b) = R - P + Q,
+//
+// i.e. 3 DMMAs per complex fragment MAC instead of 4 (-25 % of the tensor work) for two extra DADDs per loaded operand
+// fragment.  Three accumulator sets need 96 registers for a 32 x 16 warp tile, so the CTA is 8 warps (2 x 4) on the same
+// 64 x 64 x 16 tile and cp.async ring, one CTA per SM.  Error: the imaginary part is formed as R - P + Q, so its bound is
+// relative to sum_k |a||b| w instead of to |Im| itself -- the same max-norm bound the real part has.
+// FLOP accounting: bench.py keeps SURVEY 8(d)'s 8 FLOP per complex MAC for the ALGORITHMIC work and also reports the
+// executed 6 FLOP per complex MAC, so "fraction of the DMMA peak" is never inflated silently.
+constexpr int NTHREADS3 = 256;
+
+template <int NI>
+__device__ __forceinline__ void mma_ktile3m(const cplx* __restrict__ a_s, const cplx* __restrict__ b_s, const double* __restrict__ w_s,
+                                            int g, int q, int mb, int nb, double (&P)[4][2][2], double (&Q)[4][2][2],
+                                            double (&R)[4][2][2]) {
+#pragma unroll
+  for (int k4 = 0; k4 < BK / 4; k4++) {
+    const int k = k4 * 4 + q;
+    const double w = w_s[k];
+    double ar[NI], ai[NI], as[NI], br[2], bi[2], bd[2];
+#pragma unroll
+    for (int i = 0; i < NI; i++) {
+      const cplx a = a_s[k * LD_KM + mb + i * 8 + g];
+      ar[i] = a.x * w; ai[i] = a.y * w; as[i] = ar[i] + ai[i];
+    }
+#pragma unroll
+    for (int j = 0; j < 2; j++) {
+      const cplx b = b_s[k * LD_KM + nb + j * 8 + g];
+      br[j] = b.x; bi[j] = b.y; bd[j] = b.x - b.y;
+    }
+#pragma unroll
+    for (int i = 0; i < NI; i++)
+#pragma unroll
+      for (int j = 0; j < 2; j++) {
+        dmma(P[i][j][0], P[i][j][1], ar[i], br[j]);
+        dmma(Q[i][j][0], Q[i][j][1], ai[i], bi[j]);
+        dmma(R[i][j][0], R[i][j][1], as[i], bd[j]);
+      }
+  }
+}
+
+template <int STAGES>
+__global__ void __launch_bounds__(NTHREADS3, 1) zherk3m_kernel(KArgs p) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx* sA = reinterpret_cast<cplx*>(smem_raw);
+  cplx* sB = sA + STAGES * TILE_KM;
+  double* sW = reinterpret_cast<double*>(sB + STAGES * TILE_KM);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wm = warp >> 2, wn = warp & 3;
+  const int g = lane >> 2, q = lane & 3;
+  int tm, tn;
+  {
+    const int t = blockIdx.x;
+    tm = (int)((sqrt(8.0 * t + 1.0) - 1.0) * 0.5);
+    while ((tm + 1) * (tm + 2) / 2 <= t) tm++;
+    while (tm * (tm + 1) / 2 > t) tm--;
+    tn = t - tm * (tm + 1) / 2;
+  }
+  const int m0 = tm * BM, n0 = tn * BN;
+  const bool diag = tm == tn;
+  const int batch = blockIdx.z;
+  const cplx* A = p.A + batch * p.strideA;
+  cplx* C = p.C + batch * p.strideC;
+  const int kt0 = blockIdx.y * p.kt_per_split;
+  const int kt1 = min(p.n_kt, kt0 + p.kt_per_split);
+  const int nkt = kt1 - kt0;
+  if (nkt <= 0) return;
+  const double* wk = p.wk ? p.wk + batch * p.strideW : nullptr;
+
+  auto load_stage = [&](int stage, int kt) {
+    const int k0 = kt * BK;
+#pragma unroll
+    for (int i = 0; i < (BM * BK) / NTHREADS3; i++) {
+      const int idx = tid + i * NTHREADS3, k = idx / BM, r = idx % BM;
+      const bool kok = k0 + k < p.K;
+      const bool oka = kok && m0 + r < p.M;
+      cp_async16(sA + stage * TILE_KM + k * LD_KM + r, oka ? A + (long long)(k0 + k) * p.lda + (m0 + r) : A, oka);
+      if (!diag) {   // a diagonal tile multiplies the row panel with itself
+        const bool okb = kok && n0 + r < p.N;
+        cp_async16(sB + stage * TILE_KM + k * LD_KM + r, okb ? A + (long long)(k0 + k) * p.lda + (n0 + r) : A, okb);
+      }
+    }
+    if (tid < BK) {
+      double* dst = sW + stage * BK + tid;
+      const int kk = k0 + tid;
+      if (wk) cp_async8(dst, kk < p.K ? wk + kk : wk, kk < p.K);
+      else dst[0] = 1.0;
+    }
+  };
+
+  // ragged last tile row: rv valid fragment rows are dealt ceil(rv / 2) to each of the two warp rows
+  int ni = 4, mb = wm * 32;
+  const int nb = wn * 16;
+  if (p.M - m0 < BM - 8) { ni = (((p.M - m0 + 7) >> 3) + 1) >> 1; mb = wm * ni * 8; }
+  double P[4][2][2], Q[4][2][2], R[4][2][2];
+#pragma unroll
+  for (int i = 0; i < 4; i++)
+#pragma unroll
+    for (int j = 0; j < 2; j++)
+#pragma unroll
+      for (int e = 0; e < 2; e++) P[i][j][e] = Q[i][j][e] = R[i][j][e] = 0.0;
+
+#pragma unroll
+  for (int s = 0; s < STAGES - 1; s++) {
+    if (s < nkt) load_stage(s, kt0 + s);
+    cp_async_commit();
+  }
+  // a warp of a diagonal tile whose 32 x 16 block lies strictly above the diagonal has nothing to compute
+  const bool idle = diag && nb >= mb + ni * 8;
+  for (int it = 0; it < nkt; it++) {
+    cp_async_wait<STAGES - 2>();
+    __syncthreads();
+    {
+      const int nx = it + STAGES - 1;
+      if (nx < nkt) load_stage(nx % STAGES, kt0 + nx);
+      cp_async_commit();
+    }
+    const int st = it % STAGES;
+    const cplx* a_s = sA + st * TILE_KM;
+    const cplx* b_s = diag ? a_s : sB + st * TILE_KM;
+    const double* w_s = sW + st * BK;
+    if (idle) continue;
+    if (ni == 4) mma_ktile3m<4>(a_s, b_s, w_s, g, q, mb, nb, P, Q, R);
+    else if (ni == 3) mma_ktile3m<3>(a_s, b_s, w_s, g, q, mb, nb, P, Q, R);
+    else if (ni == 2) mma_ktile3m<2>(a_s, b_s, w_s, g, q, mb, nb, P, Q, R);
+    else mma_ktile3m<1>(a_s, b_s, w_s, g, q, mb, nb, P, Q, R);
+  }
+  cp_async_wait<0>();
+  if (idle) return;
+
+#pragma unroll
+  for (int i = 0; i < 4; i++) {
+    if (i >= ni) continue;
+    const int r = m0 + mb + i * 8 + g;
+    if (r >= p.M) continue;
+    const double sr = p.alpha * (p.rs ? p.rs[r] : 1.0);
+#pragma unroll
+    for (int j = 0; j < 2; j++) {
+#pragma unroll
+      for (int e = 0; e < 2; e++) {
+        const int c = n0 + nb + j * 8 + 2 * q + e;
+        if (c >= p.N || c > r) continue;           // the lower triangle is the truth, the upper one its mirror (R20)
+        const double sc = sr * (p.cs ? p.cs[c] : 1.0);
+        double vr = sc * (P[i][j][e] + Q[i][j][e]);
+        double vi = r == c ? 0.0 : sc * (R[i][j][e] - P[i][j][e] + Q[i][j][e]);
+        cplx* dst = C + (long long)r * p.ldc + c;
+        if (p.atomic) { atomicAdd(&dst->x, vr); atomicAdd(&dst->y, vi); continue; }
+        if (p.accumulate) { cplx o = *dst; vr += o.x; vi += o.y; }
+        *dst = make_double2(vr, vi);
+        if (c < r) C[(long long)c * p.ldc + r] = make_double2(vr, -vi);
+      }
+    }
+  }
+}
+
 // C[c][r] = conj(C[r][c]) for c > r (after a split-K Hermitian accumulation)
 __global__ void herm_mirror_kernel(cplx* C, long long ldc, long long strideC, int n) {
   cplx* c = C + blockIdx.z * strideC;
@@ -287,6 +445,16 @@ int launch_h(rpa_ctx* ctx, const KArgs& ka, dim3 grid) {
   if (ctx->attr_once(RPA_ATTR_ZGEMM + (A_KM ? 1 : 0) + (B_KN ? 2 : 0) + (CONJ_B ? 4 : 0) + (HERM ? 8 : 0)))
     RPA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   kern<<<grid, NTHREADS, smem, ctx->stream>>>(ka);
+  RPA_LAUNCH_CHECK(ctx);
+  return RPA_OK;
+}
+
+int launch_3m(rpa_ctx* ctx, const KArgs& ka, dim3 grid) {
+  constexpr int STAGES = 4;
+  constexpr size_t smem = (size_t)STAGES * 2 * TILE_KM * sizeof(cplx) + STAGES * BK * sizeof(double);
+  if (ctx->attr_once(RPA_ATTR_ZHERK3M))
+    RPA_CUDA(ctx, cudaFuncSetAttribute(zherk3m_kernel<STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  zherk3m_kernel<STAGES><<<grid, NTHREADS3, smem, ctx->stream>>>(ka);
   RPA_LAUNCH_CHECK(ctx);
   return RPA_OK;
 }
@@ -318,10 +486,12 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
   const long long tiles = p.herm ? (long long)tiles_m * (tiles_m + 1) / 2 : (long long)tiles_m * tiles_n;
   const int n_kt = (p.K + BK - 1) / BK;
   ka.n_kt = n_kt;
+  // the 3M kernel serves the Hermitian [k][m] x [k][n] updates with the same matrix on both sides (CHI_SUM, chi_s)
+  const bool use_3m = ctx->opt.zgemm_3m && p.herm && p.a_km && p.b_kn && p.conj_b && p.A == p.B && p.lda == p.ldb && p.strideA == p.strideB;
   int split = p.split_k;
   if (split <= 0) {
-    // pick the split that fills whole waves of (2 CTAs per SM): maximise CTAs / (waves * slots)
-    const long long slots = 2LL * ctx->sm_count;
+    // pick the split that fills whole waves of (2 CTAs per SM; 1 for the 3M kernel): maximise CTAs / (waves * slots)
+    const long long slots = (use_3m ? 1LL : 2LL) * ctx->sm_count;
     const long long base = tiles * p.batch;
     split = 1;
     int max_split = n_kt / 8;  // at least 8 k-tiles (128 k) per split
@@ -378,7 +548,8 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
   int rc;
   // the combinations the library uses: [k][m] x [k][n] conj (CHI_SUM, chi_s), [m][k] x [m][k] conj (projection, Gram,
   // Cholesky updates), [m][k] x [k][n] conj / plain (subspace iteration, rotations, triangular solves)
-  if (p.a_km && p.b_kn && p.conj_b) rc = launch<true, true, true>(ctx, ka, grid);
+  if (use_3m) rc = launch_3m(ctx, ka, grid);
+  else if (p.a_km && p.b_kn && p.conj_b) rc = launch<true, true, true>(ctx, ka, grid);
   else if (!p.a_km && !p.b_kn && p.conj_b) rc = launch<false, false, true>(ctx, ka, grid);
   else if (!p.a_km && p.b_kn && p.conj_b) rc = launch<false, true, true>(ctx, ka, grid);
   else if (!p.a_km && p.b_kn && !p.conj_b) rc = launch<false, true, false>(ctx, ka, grid);

@@ -8,7 +8,7 @@ BASELINE.json `configs` under the readings R1-R4, R11-R14 of SURVEY.md 8(c)
 (restated in DESIGN.md "Input recipe").
 """
 from .generate import (CONFIGS, RpaConfig, RpaInputs, make_inputs, sphere,
-                       reciprocal_lattice, coulomb, quadrature, sweep_n_eig)
+                       reciprocal_lattice, coulomb, quadrature, sweep_n_eig, SWEEP_FRACTIONS)
 
 __all__ = ["CONFIGS", "RpaConfig", "RpaInputs", "make_inputs", "sphere",
-           "reciprocal_lattice", "coulomb", "quadrature", "sweep_n_eig"]
+           "reciprocal_lattice", "coulomb", "quadrature", "sweep_n_eig", "SWEEP_FRACTIONS"]
