@@ -181,6 +181,8 @@ int rpa_pass_end(rpa_ctx* ctx);
  *                            Rayleigh-Ritz when 4 N_eig <= n_g (about), direct Jacobi otherwise
  *   RPA_JACOBI_BLOCK_MIN=n   smallest matrix for which the Jacobi solver takes its GEMM block form (default 1024)
  *   RPA_HETRD_MODE=0|1|2, RPA_HETRD_THREADS=n   force a large-matrix variant / CTA size of the tridiagonalisation kernel
+ *   RPA_ZGEMM_TMA=0          CHI_SUM / chi_s contractions stage their operands with cp.async and a block barrier per k-tile
+ *                            (the round-1 kernel) instead of TMA box loads and mbarriers
  *   RPA_VERBOSE=1            route decisions and kernel resources on stderr
  * --------------------------------------------------------------------------------------------------------------------- */
 /* Register-only FP64 peaks on the context's device.

@@ -36,7 +36,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     build_dir = os.path.join(HERE, "build")
     os.makedirs(build_dir, exist_ok=True)
     common = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
+              "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC] + os.environ.get("RPA_NVCC_FLAGS", "").split()
     procs = []
     for s in SOURCES:
         o = os.path.join(build_dir, s.replace(".cu", ".o"))

@@ -136,7 +136,7 @@ int rpa_create(rpa_ctx** out, const double cell[9], const int fft[3], int n_g, c
     ctx->opt.jacobi_block_min = std::max(2, num("RPA_JACOBI_BLOCK_MIN", 1024));
     ctx->opt.hetrd_mode = num("RPA_HETRD_MODE", -1);
     ctx->opt.hetrd_threads = num("RPA_HETRD_THREADS", 0);
-    ctx->opt.zgemm_3m = on("RPA_ZGEMM_3M");
+    { const char* e = getenv("RPA_ZGEMM_TMA"); ctx->opt.zgemm_tma = !(e && e[0] == '0'); }
   }
   auto fail = [&](int rc) { g_null_err = ctx->err; rpa_destroy(ctx); return rc; };
   if ((e = cudaSetDevice(device)) != cudaSuccess) return fail(rpa_fail(ctx, RPA_ERR_CUDA, "cudaSetDevice: %s", cudaGetErrorString(e)));

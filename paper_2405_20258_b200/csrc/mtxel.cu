@@ -30,6 +30,7 @@ struct AxisPlan {
   int* d_kpos = nullptr; // [nk] position (after the in-place passes) of each kept frequency
   int* d_kfreq = nullptr; // [nk] the kept frequencies themselves, in 0..n-1
   int max_res8 = 0;       // largest number of kept frequencies in one residue class mod 8
+  bool ends_only = false; // n = 8 R: every kept frequency k = s + 8 s2 has s2 = 0 or s2 = R - 1
   Plan fwd() const { Plan p; p.n = n; p.n_pass = n_pass; for (int i = 0; i < n_pass; i++) p.radix[i] = radix[i]; p.tw = d_tw_fwd; p.perm = d_perm; return p; }
   Plan inv() const { Plan p = fwd(); p.tw = d_tw_inv; return p; }
 };
@@ -93,6 +94,8 @@ int mtxel_plan_create(rpa_ctx* ctx, const int32_t* g_eps, const int32_t* g_wfn) 
     std::vector<int> kfreq(ap.nk);
     for (int i = 0; i < ap.nk; i++) { kfreq[i] = ((kidx[a][i] % n) + n) % n; kpos[i] = perm[kfreq[i]]; }
     { int cnt[8] = {0}; for (int i = 0; i < ap.nk; i++) ap.max_res8 = std::max(ap.max_res8, ++cnt[kfreq[i] & 7]); }
+    ap.ends_only = n % 8 == 0;
+    for (int i = 0; i < ap.nk && ap.ends_only; i++) ap.ends_only = (kfreq[i] >> 3) == 0 || (kfreq[i] >> 3) == n / 8 - 1;
     int rc;
     if ((rc = upload(ctx, (void**)&ap.d_tw_fwd, twf.data(), n * sizeof(cplx)))) return rc;
     if ((rc = upload(ctx, (void**)&ap.d_tw_inv, twi.data(), n * sizeof(cplx)))) return rc;
@@ -416,10 +419,13 @@ int launch_fft8(rpa_ctx* ctx, const cplx* u_v, const cplx* u_c, int nvb, int ncc
   const bool ring_ok = smem_ring <= 227 * 1024 && (nk2 + fft8::Geo<N>::RW - 1) / fft8::Geo<N>::RW <= fft8::Geo<N>::NWARP;
   const bool ring = ring_ok && N >= 48;
   const size_t smem = ring ? smem_ring : fft8::smem_bytes<N>(nk1, nk2);
-  auto kern = ring ? fft8::pair_plane_fft8_kernel_ring<N>
+  // N = 48: second passes that form only the two outputs the pruning keeps, when the kept sets allow it
+  const bool ends = N == 48 && mp->ax[0].ends_only && mp->ax[1].ends_only;
+  auto kern = ring ? (ends ? fft8::pair_plane_fft8_kernel_ring<N, true> : fft8::pair_plane_fft8_kernel_ring<N, false>)
                    : (fft8::Geo<N>::MAXREG > 0 ? fft8::pair_plane_fft8_kernel_r<N> : fft8::pair_plane_fft8_kernel_b<N>);
   if (ctx->attr_once(RPA_ATTR_FFT8 + (N == 24 ? 0 : N == 40 ? 1 : N == 48 ? 2 : 3))) {
-    RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_ring<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_ring<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_ring<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_r<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_b<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     if (ctx->opt.verbose) {

@@ -32,7 +32,12 @@ constexpr int up_mod8(int x, int r) { return x + (((r - x) % 8) + 8) % 8; }   //
 template <int N>
 struct Geo {
   static constexpr int R2 = N / 8;            // lanes per line in pass A
-  static constexpr int RW = 32 / R2;          // lines per warp
+#ifndef RPA_PLANE48_RW
+#define RPA_PLANE48_RW 4
+#endif
+  // lines per warp: as many as have R2 lanes each -- except N = 48, where 5 lines would leave the second pass (8 tasks
+  // per line, one lane each) with 40 tasks for 32 lanes, i.e. a second, quarter-full sweep of the most expensive code
+  static constexpr int RW = N == 48 ? RPA_PLANE48_RW : 32 / R2;
   static constexpr int NWARP = (N + RW - 1) / RW;
   // register cap (__maxnreg__) where a whole number of CTAs per SM needs one: 5 CTAs of 96 threads (N = 24), 2 of 224
   // (N = 40), 1 of 512 (N = 64); 0 = plain __launch_bounds__ (N = 48: 1 CTA of 320 threads, no cap needed)
@@ -73,6 +78,19 @@ __device__ __forceinline__ void dft_small(cplx* z) {
     z[1] = fftsm::cadd(e[1], o1);   z[4] = fftsm::csub(e[1], o1);
     z[2] = fftsm::cadd(e[2], o2);   z[5] = fftsm::csub(e[2], o2);
   }
+}
+
+// Outputs 0 and 5 only of the 6-point forward DFT: the second pass of a 48-point transform whose kept frequencies are
+// |k| <= 7 needs, of the group k = s + 8 s2, only s2 = 0 (k >= 0) and s2 = 5 (k < 0).  With w = e^{+i pi/3} (= w6^5),
+// w^3 = -1:  X5 = (z0 - z3) + w (z1 - z4) + w^2 (z2 - z5);  X0 = (z0 + z3) + (z1 + z4) + (z2 + z5).  24 FP64
+// instructions instead of the ~55 of the full butterfly.
+__device__ __forceinline__ void dft6_ends(const cplx* z, cplx& x0, cplx& x5) {
+  const double h = 0.5, s = 0.86602540378443864676;
+  const cplx a0 = fftsm::cadd(z[0], z[3]), a1 = fftsm::cadd(z[1], z[4]), a2 = fftsm::cadd(z[2], z[5]);
+  const cplx d0 = fftsm::csub(z[0], z[3]), d1 = fftsm::csub(z[1], z[4]), d2 = fftsm::csub(z[2], z[5]);
+  x0 = fftsm::cadd(fftsm::cadd(a0, a1), a2);
+  const cplx p = fftsm::csub(d1, d2), r = fftsm::cadd(d1, d2);
+  x5 = make_double2(fma(-s, r.y, fma(h, p.x, d0.x)), fma(s, r.x, fma(h, p.y, d0.y)));
 }
 
 template <int N>
@@ -243,7 +261,9 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
   } while (!ok);
 }
 
-template <int N>
+// ENDS (N = 48 only): every kept frequency of both axes has s2 = 0 or s2 = R2 - 1 (the host checks), so the second passes
+// form just those two outputs (dft6_ends) instead of the full R2-point butterfly.
+template <int N, bool ENDS>
 __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict__ u_v, const cplx* __restrict__ u_c, int nvb, int ncc,
                                                           int N3, const cplx* __restrict__ tw, const int* __restrict__ kfreq1,
                                                           const int* __restrict__ kfreq2, int nk1, int nk2, cplx* __restrict__ T) {
@@ -329,13 +349,21 @@ __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict
       cplx zz[R2];
 #pragma unroll
       for (int q = 0; q < R2; q++) zz[q] = grp[q];
-      dft_small<R2>(zz);
       const unsigned long long sl = slot1[s];
       cplx* dst = dstT + (long long)l * nk1;
+      if (ENDS && R2 == 6) {
+        cplx x0, x5;
+        dft6_ends(zz, x0, x5);
+        const int ia = (int)(sl & 0xff), ib = (int)((sl >> 40) & 0xff);
+        if (ia != 0xff) dst[ia] = x0;
+        if (ib != 0xff) dst[ib] = x5;
+      } else {
+        dft_small<R2>(zz);
 #pragma unroll
-      for (int s2 = 0; s2 < R2; s2++) {
-        const int i1 = (int)((sl >> (8 * s2)) & 0xff);
-        if (i1 != 0xff) dst[i1] = zz[s2];
+        for (int s2 = 0; s2 < R2; s2++) {
+          const int i1 = (int)((sl >> (8 * s2)) & 0xff);
+          if (i1 != 0xff) dst[i1] = zz[s2];
+        }
       }
     }
     __syncwarp();
@@ -371,13 +399,21 @@ __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict
       cplx zz[R2];
 #pragma unroll
       for (int q = 0; q < R2; q++) zz[q] = grp[q];
-      dft_small<R2>(zz);
       const unsigned long long sl = slot2[s];
       cplx* dst = cb + r0 + l;
+      if (ENDS && R2 == 6) {
+        cplx x0, x5;
+        dft6_ends(zz, x0, x5);
+        const int ia = (int)(sl & 0xff), ib = (int)((sl >> 40) & 0xff);
+        if (ia != 0xff) dst[ia * PC] = x0;
+        if (ib != 0xff) dst[ib * PC] = x5;
+      } else {
+        dft_small<R2>(zz);
 #pragma unroll
-      for (int s2 = 0; s2 < R2; s2++) {
-        const int i2 = (int)((sl >> (8 * s2)) & 0xff);
-        if (i2 != 0xff) dst[i2 * PC] = zz[s2];
+        for (int s2 = 0; s2 < R2; s2++) {
+          const int i2 = (int)((sl >> (8 * s2)) & 0xff);
+          if (i2 != 0xff) dst[i2 * PC] = zz[s2];
+        }
       }
     }
     __syncwarp();
@@ -414,9 +450,9 @@ template <int N>
 __global__ void __launch_bounds__(Geo<N>::NWARP * 32) pair_plane_fft8_kernel_b(RPA_FFT8_ARGS) {
   pair_plane_fft8_body<N>(u_v, u_c, nvb, ncc, N3, tw, kfreq1, kfreq2, nk1, nk2, T);
 }
-template <int N>
+template <int N, bool ENDS>
 __global__ void __launch_bounds__(Geo<N>::NWARP * 32) pair_plane_fft8_kernel_ring(RPA_FFT8_ARGS) {
-  pair_plane_fft8_ring_body<N>(u_v, u_c, nvb, ncc, N3, tw, kfreq1, kfreq2, nk1, nk2, T);
+  pair_plane_fft8_ring_body<N, ENDS>(u_v, u_c, nvb, ncc, N3, tw, kfreq1, kfreq2, nk1, nk2, T);
 }
 #undef RPA_FFT8_ARGS
 

@@ -28,7 +28,7 @@ struct rpa_ctx {
     int jacobi_block_min = 1024;   // RPA_JACOBI_BLOCK_MIN: smallest matrix that takes the GEMM block Jacobi
     int hetrd_mode = -1;           // RPA_HETRD_MODE=0..2: force a large-matrix variant of the tridiagonalisation kernel
     int hetrd_threads = 0;         // RPA_HETRD_THREADS: its CTA size
-    bool zgemm_3m = false;         // RPA_ZGEMM_3M=1: Hermitian updates with the 3-multiply complex product (zherk3m_kernel)
+    bool zgemm_tma = true;         // RPA_ZGEMM_TMA=0: Hermitian [k][m] updates staged by cp.async + block barrier instead of TMA + mbarriers
   } opt;
 
   // Kernel function attributes (dynamic shared memory > 48 KB) are per device: each launch site sets them the first time
@@ -36,6 +36,7 @@ struct rpa_ctx {
   unsigned long long attr_mask = 0;
   bool attr_once(int id) { const unsigned long long b = 1ull << id; if (attr_mask & b) return false; attr_mask |= b; return true; }
   int z_per_sm[3] = {0, 0, 0};     // z_fft8_scatter_kernel<40/120/160>
+  void* tma_encode = nullptr;      // cuTensorMapEncodeTiled, fetched through the runtime (no link against libcuda)
 
   // problem statement
   double cell[9];
@@ -82,7 +83,7 @@ struct rpa_ctx {
 // attr_once ids
 enum { RPA_ATTR_ZGEMM = 0 /* + 16 layout/HERM combinations */, RPA_ATTR_AXIS = 16 /* + 4 */, RPA_ATTR_FFT8 = 20 /* + 4 */,
        RPA_ATTR_ZFFT8 = 24, RPA_ATTR_POTRF = 25, RPA_ATTR_TRSM = 26, RPA_ATTR_JACOBI = 27, RPA_ATTR_PLANE_GENERIC = 28 /* + 2 */,
-       RPA_ATTR_WFN = 30 /* + 4 */, RPA_ATTR_ZHERK3M = 34 };
+       RPA_ATTR_WFN = 30 /* + 4 */, RPA_ATTR_ZHERK_TMA = 34 };
 
 int rpa_fail(rpa_ctx* ctx, int code, const char* fmt, ...);
 #define RPA_CUDA(ctx, call)                                                              \

@@ -13,6 +13,9 @@
 // 128-bit fragment loads bank-conflict free (leading dimension = 2 mod 8 elements for [k][m], 4 mod 8 for [m][k]).
 #include <algorithm>
 
+#include <cuda.h>
+#include <cudaTypedefs.h>
+
 #include "rpa_internal.h"
 
 namespace {
@@ -78,7 +81,7 @@ __device__ __forceinline__ void load_tile(cplx* s, const cplx* g, long long ld, 
 // Hermitian tile.  TRI = true: three 2 x 2 lower fragment triangles on the diagonal at 0, 24, 48 (slot [t][0] =
 // (24t, 24t), [t][1] = (24t+8, 24t), [t][2] = (24t+8, 24t+8)).  3 x 3 x 3 + TRI tile the 36 fragments on or below the
 // diagonal of a diagonal Hermitian tile, 9 per warp (see the kernel).
-template <bool A_KM, bool B_KN, bool CONJ_B, int NI, int NJ, bool TRI>
+template <bool A_KM, bool B_KN, bool CONJ_B, int NI, int NJ, bool TRI, bool BOX = false>
 __device__ __forceinline__ void mma_ktile(const cplx* __restrict__ a_s, const cplx* __restrict__ b_s,
                                           const double* __restrict__ w_s, int g, int q, int mb, int nb,
                                           double (&cre)[4][4][2], double (&cim)[4][4][2], bool skip_upper = false) {
@@ -91,13 +94,14 @@ __device__ __forceinline__ void mma_ktile(const cplx* __restrict__ a_s, const cp
 #pragma unroll
     for (int i = 0; i < NA; i++) {
       const int m = TRI ? 24 * (i >> 1) + 8 * (i & 1) + g : mb + i * 8 + g;
-      cplx a = A_KM ? a_s[k * LD_KM + m] : a_s[m * LD_MK + k];
+      // BOX: the TMA layout of a [k][m] tile, 8 boxes of [16 k][8 m] (element (k, m) at (m >> 3) 128 + 8 k + (m & 7))
+      cplx a = BOX ? a_s[((m >> 3) << 7) + k * 8 + (m & 7)] : A_KM ? a_s[k * LD_KM + m] : a_s[m * LD_MK + k];
       ar[i] = a.x * w; ai[i] = a.y * w;
     }
 #pragma unroll
     for (int j = 0; j < NB; j++) {
       const int n = TRI ? 24 * (j >> 1) + 8 * (j & 1) + g : nb + j * 8 + g;
-      cplx b = B_KN ? b_s[k * LD_KM + n] : b_s[n * LD_MK + k];
+      cplx b = BOX ? b_s[((n >> 3) << 7) + k * 8 + (n & 7)] : B_KN ? b_s[k * LD_KM + n] : b_s[n * LD_MK + k];
       br[j] = b.x; bi[j] = b.y;
     }
     // a conj(b): re += ar br + ai bi, im += ai br - ar bi;  a b: re += ar br - ai bi, im += ai br + ar bi.  The sign is
@@ -268,57 +272,48 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// 3M variant of the Hermitian [k][m] x [k][n] update (CHI_SUM, chi_s): the complex product with THREE real products
-// (Karatsuba) instead of four,
-//
-//   P += ar br,  Q += ai bi,  R += (ar + ai)(br - bi);      Re(a conj b) = P + Q,  Im(a conj b) = R - P + Q,
-//
-// i.e. 3 DMMAs per complex fragment MAC instead of 4 (-25 % of the tensor work) for two extra DADDs per loaded operand
-// fragment.  Three accumulator sets need 96 registers for a 32 x 16 warp tile, so the CTA is 8 warps (2 x 4) on the same
-// 64 x 64 x 16 tile and cp.async ring, one CTA per SM.  Error: the imaginary part is formed as R - P + Q, so its bound is
-// relative to sum_k |a||b| w instead of to |Im| itself -- the same max-norm bound the real part has.
-// FLOP accounting: bench.py keeps SURVEY 8(d)'s 8 FLOP per complex MAC for the ALGORITHMIC work and also reports the
-// executed 6 FLOP per complex MAC, so "fraction of the DMMA peak" is never inflated silently.
-constexpr int NTHREADS3 = 256;
+// TMA-staged variant of the Hermitian [k][m] x [k][n] update (CHI_SUM, chi_s): the same tile, warp shares and epilogue
+// as zgemm_dmma_kernel<1,1,1,3,1>, but the operand panels arrive by cp.async.bulk.tensor (one elected thread issues
+// 8 + 8 box loads and one weight row per k-tile) into a 3-stage ring guarded by mbarriers: full[s] (transaction bytes)
+// and empty[s] (one arrival per warp) -- no per-thread address arithmetic, no cp.async groups and no block barrier in the
+// main loop.  A [k][64] panel is loaded as 8 boxes of [16][8] complex: a warp's fragment load then reads 4 full 128-byte
+// rows, conflict-free without padding.
+constexpr int TMA_STAGES = 3;
+constexpr int TMA_TILE = BK * BM;   // 1024 complex per operand tile
 
-template <int NI>
-__device__ __forceinline__ void mma_ktile3m(const cplx* __restrict__ a_s, const cplx* __restrict__ b_s, const double* __restrict__ w_s,
-                                            int g, int q, int mb, int nb, double (&P)[4][2][2], double (&Q)[4][2][2],
-                                            double (&R)[4][2][2]) {
-#pragma unroll
-  for (int k4 = 0; k4 < BK / 4; k4++) {
-    const int k = k4 * 4 + q;
-    const double w = w_s[k];
-    double ar[NI], ai[NI], as[NI], br[2], bi[2], bd[2];
-#pragma unroll
-    for (int i = 0; i < NI; i++) {
-      const cplx a = a_s[k * LD_KM + mb + i * 8 + g];
-      ar[i] = a.x * w; ai[i] = a.y * w; as[i] = ar[i] + ai[i];
-    }
-#pragma unroll
-    for (int j = 0; j < 2; j++) {
-      const cplx b = b_s[k * LD_KM + nb + j * 8 + g];
-      br[j] = b.x; bi[j] = b.y; bd[j] = b.x - b.y;
-    }
-#pragma unroll
-    for (int i = 0; i < NI; i++)
-#pragma unroll
-      for (int j = 0; j < 2; j++) {
-        dmma(P[i][j][0], P[i][j][1], ar[i], br[j]);
-        dmma(Q[i][j][0], Q[i][j][1], ai[i], bi[j]);
-        dmma(R[i][j][0], R[i][j][1], as[i], bd[j]);
-      }
-  }
+__device__ __forceinline__ void tma_mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void tma_mbar_arrive(unsigned long long* bar) {
+  asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ void tma_mbar_expect(unsigned long long* bar, unsigned bytes) {
+  asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n}\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_mbar_wait(unsigned long long* bar, unsigned parity) {
+  const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  unsigned ok;
+  do {
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+                 : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void tma_load_2d(void* smem, const CUtensorMap* map, int x, int y, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n" ::
+               "r"((unsigned)__cvta_generic_to_shared(smem)), "l"(map), "r"(x), "r"(y), "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
 }
 
-template <int STAGES>
-__global__ void __launch_bounds__(NTHREADS3, 1) zherk3m_kernel(KArgs p) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  cplx* sA = reinterpret_cast<cplx*>(smem_raw);
-  cplx* sB = sA + STAGES * TILE_KM;
-  double* sW = reinterpret_cast<double*>(sB + STAGES * TILE_KM);
+struct TmaMaps { CUtensorMap a; CUtensorMap w; };   // operand [K][2 M doubles], weights [batch][K doubles]
+
+__global__ void __launch_bounds__(NTHREADS, 2) zherk_tma_kernel(KArgs p, const __grid_constant__ TmaMaps maps) {
+  extern __shared__ __align__(128) unsigned char smem_tma[];
+  cplx* sA = reinterpret_cast<cplx*>(smem_tma);
+  cplx* sB = sA + TMA_STAGES * TMA_TILE;
+  double* sW = reinterpret_cast<double*>(sB + TMA_STAGES * TMA_TILE);
+  unsigned long long* full = reinterpret_cast<unsigned long long*>(sW + TMA_STAGES * BK);
+  unsigned long long* empty = full + TMA_STAGES;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int wm = warp >> 2, wn = warp & 3;
+  const int wm = warp >> 1, wn = warp & 1;
   const int g = lane >> 2, q = lane & 3;
   int tm, tn;
   {
@@ -331,90 +326,91 @@ __global__ void __launch_bounds__(NTHREADS3, 1) zherk3m_kernel(KArgs p) {
   const int m0 = tm * BM, n0 = tn * BN;
   const bool diag = tm == tn;
   const int batch = blockIdx.z;
-  const cplx* A = p.A + batch * p.strideA;
   cplx* C = p.C + batch * p.strideC;
   const int kt0 = blockIdx.y * p.kt_per_split;
   const int kt1 = min(p.n_kt, kt0 + p.kt_per_split);
   const int nkt = kt1 - kt0;
   if (nkt <= 0) return;
-  const double* wk = p.wk ? p.wk + batch * p.strideW : nullptr;
-
-  auto load_stage = [&](int stage, int kt) {
+  if (tid == 0) {
+    for (int s = 0; s < TMA_STAGES; s++) { tma_mbar_init(full + s, 1); tma_mbar_init(empty + s, NTHREADS / 32); }
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  __syncthreads();
+  const unsigned stage_bytes = (unsigned)((diag ? 1 : 2) * TMA_TILE * sizeof(cplx) + BK * sizeof(double));
+  auto issue = [&](int stage, int kt) {   // one thread
     const int k0 = kt * BK;
+    tma_mbar_expect(full + stage, stage_bytes);
 #pragma unroll
-    for (int i = 0; i < (BM * BK) / NTHREADS3; i++) {
-      const int idx = tid + i * NTHREADS3, k = idx / BM, r = idx % BM;
-      const bool kok = k0 + k < p.K;
-      const bool oka = kok && m0 + r < p.M;
-      cp_async16(sA + stage * TILE_KM + k * LD_KM + r, oka ? A + (long long)(k0 + k) * p.lda + (m0 + r) : A, oka);
-      if (!diag) {   // a diagonal tile multiplies the row panel with itself
-        const bool okb = kok && n0 + r < p.N;
-        cp_async16(sB + stage * TILE_KM + k * LD_KM + r, okb ? A + (long long)(k0 + k) * p.lda + (n0 + r) : A, okb);
-      }
+    for (int b = 0; b < 8; b++) tma_load_2d(sA + stage * TMA_TILE + b * 128, &maps.a, 2 * (m0 + 8 * b), k0, full + stage);
+    if (!diag) {
+#pragma unroll
+      for (int b = 0; b < 8; b++) tma_load_2d(sB + stage * TMA_TILE + b * 128, &maps.a, 2 * (n0 + 8 * b), k0, full + stage);
     }
-    if (tid < BK) {
-      double* dst = sW + stage * BK + tid;
-      const int kk = k0 + tid;
-      if (wk) cp_async8(dst, kk < p.K ? wk + kk : wk, kk < p.K);
-      else dst[0] = 1.0;
-    }
+    tma_load_2d(sW + stage * BK, &maps.w, k0, batch, full + stage);
   };
 
-  // ragged last tile row: rv valid fragment rows are dealt ceil(rv / 2) to each of the two warp rows
-  int ni = 4, mb = wm * 32;
-  const int nb = wn * 16;
-  if (p.M - m0 < BM - 8) { ni = (((p.M - m0 + 7) >> 3) + 1) >> 1; mb = wm * ni * 8; }
-  double P[4][2][2], Q[4][2][2], R[4][2][2];
+  int mode = 0, mb = wm * 32, nb = wn * 32;
+  if (diag) {
+    if (warp == 0) { mode = 2; mb = nb = 0; }
+    else { mode = 1; mb = warp == 1 ? 16 : 40; nb = warp == 3 ? 24 : 0; }
+  }
+  int ni = mode == 0 ? 4 : 3;
+  if (mode == 0 && p.M - m0 < BM - 8) {
+    ni = (((p.M - m0 + 7) >> 3) + 1) >> 1;
+    mb = wm * ni * 8;
+  }
+  double cre[4][4][2], cim[4][4][2];
 #pragma unroll
   for (int i = 0; i < 4; i++)
 #pragma unroll
-    for (int j = 0; j < 2; j++)
-#pragma unroll
-      for (int e = 0; e < 2; e++) P[i][j][e] = Q[i][j][e] = R[i][j][e] = 0.0;
+    for (int j = 0; j < 4; j++) { cre[i][j][0] = cre[i][j][1] = 0.0; cim[i][j][0] = cim[i][j][1] = 0.0; }
 
-#pragma unroll
-  for (int s = 0; s < STAGES - 1; s++) {
-    if (s < nkt) load_stage(s, kt0 + s);
-    cp_async_commit();
-  }
-  // a warp of a diagonal tile whose 32 x 16 block lies strictly above the diagonal has nothing to compute
-  const bool idle = diag && nb >= mb + ni * 8;
+  if (tid == 0)
+    for (int s = 0; s < TMA_STAGES - 1 && s < nkt; s++) issue(s, kt0 + s);
+
   for (int it = 0; it < nkt; it++) {
-    cp_async_wait<STAGES - 2>();
-    __syncthreads();
-    {
-      const int nx = it + STAGES - 1;
-      if (nx < nkt) load_stage(nx % STAGES, kt0 + nx);
-      cp_async_commit();
+    const int st = it % TMA_STAGES;
+    if (tid == 0) {   // refill the stage all warps left one iteration ago
+      const int nx = it + TMA_STAGES - 1;
+      if (nx < nkt) {
+        const int sx = nx % TMA_STAGES;
+        if (nx >= TMA_STAGES) tma_mbar_wait(empty + sx, (unsigned)(((nx / TMA_STAGES) - 1) & 1));
+        issue(sx, kt0 + nx);
+      }
     }
-    const int st = it % STAGES;
-    const cplx* a_s = sA + st * TILE_KM;
-    const cplx* b_s = diag ? a_s : sB + st * TILE_KM;
+    __syncwarp();
+    tma_mbar_wait(full + st, (unsigned)((it / TMA_STAGES) & 1));
+    const cplx* a_s = sA + st * TMA_TILE;
+    const cplx* b_s = diag ? a_s : sB + st * TMA_TILE;
     const double* w_s = sW + st * BK;
-    if (idle) continue;
-    if (ni == 4) mma_ktile3m<4>(a_s, b_s, w_s, g, q, mb, nb, P, Q, R);
-    else if (ni == 3) mma_ktile3m<3>(a_s, b_s, w_s, g, q, mb, nb, P, Q, R);
-    else if (ni == 2) mma_ktile3m<2>(a_s, b_s, w_s, g, q, mb, nb, P, Q, R);
-    else mma_ktile3m<1>(a_s, b_s, w_s, g, q, mb, nb, P, Q, R);
+    if (mode == 0) {
+      if (ni == 4) mma_ktile<true, true, true, 4, 4, false, true>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+      else if (ni == 3) mma_ktile<true, true, true, 3, 4, false, true>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+      else if (ni == 2) mma_ktile<true, true, true, 2, 4, false, true>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+      else mma_ktile<true, true, true, 1, 4, false, true>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+    } else if (mode == 1) mma_ktile<true, true, true, 3, 3, false, true>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+    else mma_ktile<true, true, true, 3, 3, true, true>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+    __syncwarp();
+    if (lane == 0) tma_mbar_arrive(empty + st);
   }
-  cp_async_wait<0>();
-  if (idle) return;
 
 #pragma unroll
   for (int i = 0; i < 4; i++) {
-    if (i >= ni) continue;
-    const int r = m0 + mb + i * 8 + g;
-    if (r >= p.M) continue;
-    const double sr = p.alpha * (p.rs ? p.rs[r] : 1.0);
 #pragma unroll
-    for (int j = 0; j < 2; j++) {
+    for (int j = 0; j < 4; j++) {
+      if (i >= ni || (mode != 0 && j == 3)) continue;
+      const int ro = mode == 2 ? 24 * i + (j >= 1 ? 8 : 0) : mb + i * 8;
+      const int co = mode == 2 ? 24 * i + (j == 2 ? 8 : 0) : nb + j * 8;
+      const int r = m0 + ro + g;
+      if (r >= p.M) continue;
+      const double sr = p.alpha * (p.rs ? p.rs[r] : 1.0);
 #pragma unroll
       for (int e = 0; e < 2; e++) {
-        const int c = n0 + nb + j * 8 + 2 * q + e;
-        if (c >= p.N || c > r) continue;           // the lower triangle is the truth, the upper one its mirror (R20)
+        const int c = n0 + co + 2 * q + e;
+        if (c >= p.N || c > r) continue;
         const double sc = sr * (p.cs ? p.cs[c] : 1.0);
-        double vr = sc * (P[i][j][e] + Q[i][j][e]);
-        double vi = r == c ? 0.0 : sc * (R[i][j][e] - P[i][j][e] + Q[i][j][e]);
+        double vr = sc * cre[i][j][e], vi = sc * cim[i][j][e];
+        if (r == c) vi = 0.0;
         cplx* dst = C + (long long)r * p.ldc + c;
         if (p.atomic) { atomicAdd(&dst->x, vr); atomicAdd(&dst->y, vi); continue; }
         if (p.accumulate) { cplx o = *dst; vr += o.x; vi += o.y; }
@@ -449,13 +445,41 @@ int launch_h(rpa_ctx* ctx, const KArgs& ka, dim3 grid) {
   return RPA_OK;
 }
 
-int launch_3m(rpa_ctx* ctx, const KArgs& ka, dim3 grid) {
-  constexpr int STAGES = 4;
-  constexpr size_t smem = (size_t)STAGES * 2 * TILE_KM * sizeof(cplx) + STAGES * BK * sizeof(double);
-  if (ctx->attr_once(RPA_ATTR_ZHERK3M))
-    RPA_CUDA(ctx, cudaFuncSetAttribute(zherk3m_kernel<STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  zherk3m_kernel<STAGES><<<grid, NTHREADS3, smem, ctx->stream>>>(ka);
+// Tensor maps for zherk_tma_kernel.  Returns RPA_OK and sets *ok = false when the operands do not meet TMA's alignment
+// rules (the caller then takes the cp.async kernel).
+int launch_tma(rpa_ctx* ctx, const KArgs& ka, dim3 grid, int batch, bool* ok) {
+  *ok = false;
+  if (!ctx->tma_encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) { (void)cudaGetLastError(); return RPA_OK; }
+    ctx->tma_encode = fn;
+  }
+  auto encode = reinterpret_cast<PFN_cuTensorMapEncodeTiled>(ctx->tma_encode);
+  if (!ka.wk || ((uintptr_t)ka.A & 15) || ((uintptr_t)ka.wk & 15) || (ka.strideW * 8) % 16 != 0 || (batch > 1 && ka.strideA != 0)) return RPA_OK;
+  TmaMaps maps;
+  {
+    cuuint64_t dims[2] = {(cuuint64_t)2 * ka.M, (cuuint64_t)ka.K};
+    cuuint64_t strides[1] = {(cuuint64_t)ka.lda * sizeof(cplx)};
+    cuuint32_t box[2] = {16, (cuuint32_t)BK};
+    cuuint32_t es[2] = {1, 1};
+    if (encode(&maps.a, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void*)ka.A, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return RPA_OK;
+  }
+  {
+    cuuint64_t dims[2] = {(cuuint64_t)ka.K, (cuuint64_t)batch};
+    cuuint64_t strides[1] = {(cuuint64_t)(batch > 1 ? ka.strideW : ka.K + (ka.K & 1)) * sizeof(double)};
+    cuuint32_t box[2] = {(cuuint32_t)BK, 1};
+    cuuint32_t es[2] = {1, 1};
+    if (encode(&maps.w, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void*)ka.wk, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return RPA_OK;
+  }
+  constexpr size_t smem = (size_t)TMA_STAGES * 2 * TMA_TILE * sizeof(cplx) + TMA_STAGES * BK * sizeof(double) + 2 * TMA_STAGES * sizeof(unsigned long long) + 128;
+  if (ctx->attr_once(RPA_ATTR_ZHERK_TMA))
+    RPA_CUDA(ctx, cudaFuncSetAttribute(zherk_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  zherk_tma_kernel<<<grid, NTHREADS, smem, ctx->stream>>>(ka, maps);
   RPA_LAUNCH_CHECK(ctx);
+  *ok = true;
   return RPA_OK;
 }
 
@@ -486,12 +510,10 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
   const long long tiles = p.herm ? (long long)tiles_m * (tiles_m + 1) / 2 : (long long)tiles_m * tiles_n;
   const int n_kt = (p.K + BK - 1) / BK;
   ka.n_kt = n_kt;
-  // the 3M kernel serves the Hermitian [k][m] x [k][n] updates with the same matrix on both sides (CHI_SUM, chi_s)
-  const bool use_3m = ctx->opt.zgemm_3m && p.herm && p.a_km && p.b_kn && p.conj_b && p.A == p.B && p.lda == p.ldb && p.strideA == p.strideB;
   int split = p.split_k;
   if (split <= 0) {
-    // pick the split that fills whole waves of (2 CTAs per SM; 1 for the 3M kernel): maximise CTAs / (waves * slots)
-    const long long slots = (use_3m ? 1LL : 2LL) * ctx->sm_count;
+    // pick the split that fills whole waves of (2 CTAs per SM): maximise CTAs / (waves * slots)
+    const long long slots = 2LL * ctx->sm_count;
     const long long base = tiles * p.batch;
     split = 1;
     int max_split = n_kt / 8;  // at least 8 k-tiles (128 k) per split
@@ -548,7 +570,11 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
   int rc;
   // the combinations the library uses: [k][m] x [k][n] conj (CHI_SUM, chi_s), [m][k] x [m][k] conj (projection, Gram,
   // Cholesky updates), [m][k] x [k][n] conj / plain (subspace iteration, rotations, triangular solves)
-  if (use_3m) rc = launch_3m(ctx, ka, grid);
+  bool tma_done = false;
+  if (ctx->opt.zgemm_tma && p.herm && p.a_km && p.b_kn && p.conj_b && p.A == p.B && p.lda == p.ldb && p.strideA == p.strideB) {
+    if ((rc = launch_tma(ctx, ka, grid, p.batch, &tma_done))) return rc;
+  }
+  if (tma_done) rc = RPA_OK;
   else if (p.a_km && p.b_kn && p.conj_b) rc = launch<true, true, true>(ctx, ka, grid);
   else if (!p.a_km && !p.b_kn && p.conj_b) rc = launch<false, false, true>(ctx, ka, grid);
   else if (!p.a_km && p.b_kn && p.conj_b) rc = launch<false, true, true>(ctx, ka, grid);
