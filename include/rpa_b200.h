@@ -186,8 +186,9 @@ int rpa_pass_end(rpa_ctx* ctx);
  *   RPA_VERBOSE=1            route decisions and kernel resources on stderr
  * --------------------------------------------------------------------------------------------------------------------- */
 /* Register-only FP64 peaks on the context's device.
- *   kind 0: mma.sync m8n8k4 f64 (DMMA), kind 1: DFMA.  Returns TFLOP/s in *tflops; runs `iters`
- *   launches of a fixed-size kernel on the context stream and synchronises.                      */
+ *   kind 0: mma.sync m8n8k4 f64 (DMMA), kind 1: DFMA, kind 2: DMMA throughput when every 24 DMMAs are interleaved with 14
+ *   independent DADDs (plain FP64 instructions share the pipe).  Returns TFLOP/s in *tflops; runs `iters` launches of a
+ *   fixed-size kernel on the context stream and synchronises.                                    */
 int rpa_fp64_peak(rpa_ctx* ctx, int kind, int iters, double* tflops);
 /* Per-kernel-class device times (bench.py's roofline of the dominant kernel).  Between rpa_profile_begin and
  * rpa_profile_end every launch of the classes below is bracketed by a pair of CUDA events on the context stream;

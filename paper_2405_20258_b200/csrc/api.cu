@@ -334,7 +334,7 @@ int rpa_epsilon_inverse(rpa_ctx* ctx, const void* chi_s, int n_eig, int n_w, voi
 
 int rpa_fp64_peak(rpa_ctx* ctx, int kind, int iters, double* tflops) {
   if (bad_ctx(ctx)) return rpa_fail(nullptr, RPA_ERR_INVALID, "null context");
-  if (!tflops || kind < 0 || kind > 1) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_fp64_peak: invalid argument");
+  if (!tflops || kind < 0 || kind > 2) return rpa_fail(ctx, RPA_ERR_INVALID, "rpa_fp64_peak: invalid argument");
   RPA_CUDA(ctx, cudaSetDevice(ctx->device));
   return fp64_peak_kernel(ctx, kind, iters, tflops);
 }

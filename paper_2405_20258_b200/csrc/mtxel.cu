@@ -356,6 +356,19 @@ MtxelSizes mtxel_sizes(const rpa_ctx* ctx, int nvb, int nc) {
   size_t budget = (size_t)1536 << 20;  // chunk the conduction bands so that u_c + T stay near 1.5 GB
   int ncc = (int)std::max<size_t>(16, budget / per_c);
   if (ncc > nc) ncc = nc;
+  else {
+    // the plane kernel launches one CTA per (conduction band or pair of bands, plane) and one CTA per SM is resident: take
+    // the chunk, not more than a quarter below the budget, whose CTAs come closest to whole waves
+    const int per_cta = (ctx->fft[0] == 48 && ctx->fft[1] == 48) ? 2 : 1;
+    double best = -1.0; int best_ncc = ncc;
+    for (int cand = ncc; cand >= std::max(16, ncc - ncc / 4); cand--) {
+      const long long ctas = (long long)((cand + per_cta - 1) / per_cta) * ctx->fft[2];
+      const long long waves = (ctas + ctx->sm_count - 1) / ctx->sm_count;
+      const double eff = (double)ctas / (double)(waves * ctx->sm_count);
+      if (eff > best + 1e-9) { best = eff; best_ncc = cand; }
+    }
+    ncc = best_ncc;
+  }
   MtxelSizes s;
   s.ncc = ncc;
   s.u_v = ws_round((size_t)nvb * n_r * sizeof(cplx));
@@ -418,14 +431,20 @@ int launch_fft8(rpa_ctx* ctx, const cplx* u_v, const cplx* u_c, int nvb, int ncc
   const size_t smem_ring = fft8::smem_bytes_ring<N>(nk2);
   const bool ring_ok = smem_ring <= 227 * 1024 && (nk2 + fft8::Geo<N>::RW - 1) / fft8::Geo<N>::RW <= fft8::Geo<N>::NWARP;
   const bool ring = ring_ok && N >= 48;
-  const size_t smem = ring ? smem_ring : fft8::smem_bytes<N>(nk1, nk2);
-  // N = 48: second passes that form only the two outputs the pruning keeps, when the kept sets allow it
+  // N = 48: second passes that form only the two outputs the pruning keeps, when the kept sets allow it; and two
+  // conduction bands per CTA (two u_c planes fit next to the ring), which halves the u_v traffic from L2
   const bool ends = N == 48 && mp->ax[0].ends_only && mp->ax[1].ends_only;
-  auto kern = ring ? (ends ? fft8::pair_plane_fft8_kernel_ring<N, true> : fft8::pair_plane_fft8_kernel_ring<N, false>)
+  const bool two = N == 48 && ring && fft8::smem_bytes_ring<N>(nk2, 2) <= 227 * 1024 && ncc >= 2;
+  const size_t smem = ring ? fft8::smem_bytes_ring<N>(nk2, two ? 2 : 1) : fft8::smem_bytes<N>(nk1, nk2);
+  constexpr int CB2 = N == 48 ? 2 : 1;   // the two-band form is compiled for N = 48 only
+  auto kern = ring ? (two ? (ends ? fft8::pair_plane_fft8_kernel_ring<N, true, CB2> : fft8::pair_plane_fft8_kernel_ring<N, false, CB2>)
+                          : (ends ? fft8::pair_plane_fft8_kernel_ring<N, true, 1> : fft8::pair_plane_fft8_kernel_ring<N, false, 1>))
                    : (fft8::Geo<N>::MAXREG > 0 ? fft8::pair_plane_fft8_kernel_r<N> : fft8::pair_plane_fft8_kernel_b<N>);
   if (ctx->attr_once(RPA_ATTR_FFT8 + (N == 24 ? 0 : N == 40 ? 1 : N == 48 ? 2 : 3))) {
-    RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_ring<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-    RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_ring<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_ring<N, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_ring<N, true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_ring<N, false, CB2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_ring<N, true, CB2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_r<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     RPA_CUDA(ctx, cudaFuncSetAttribute(fft8::pair_plane_fft8_kernel_b<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
     if (ctx->opt.verbose) {
@@ -435,8 +454,9 @@ int launch_fft8(rpa_ctx* ctx, const cplx* u_v, const cplx* u_c, int nvb, int ncc
               fa.numRegs, fa.maxThreadsPerBlock, fft8::Geo<N>::NWARP * 32, smem);
     }
   }
-  kern<<<(unsigned)(ncc * N3), fft8::Geo<N>::NWARP * 32, smem, ctx->stream>>>(u_v, u_c, nvb, ncc, N3, mp->ax[0].d_tw_fwd,
-                                                                             mp->ax[0].d_kfreq, mp->ax[1].d_kfreq, nk1, nk2, T);
+  const int ctas_c = two ? (ncc + 1) / 2 : ncc;
+  kern<<<(unsigned)(ctas_c * N3), fft8::Geo<N>::NWARP * 32, smem, ctx->stream>>>(u_v, u_c, nvb, ncc, N3, mp->ax[0].d_tw_fwd,
+                                                                                mp->ax[0].d_kfreq, mp->ax[1].d_kfreq, nk1, nk2, T);
   RPA_LAUNCH_CHECK(ctx);
   return RPA_OK;
 }

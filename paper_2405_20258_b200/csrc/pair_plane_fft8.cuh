@@ -58,7 +58,11 @@ struct Geo {
   // 128-bit pass-A accesses are conflict free; an odd pitch makes the transposed stores of pass B conflict free.
   static constexpr int PS = up_mod8(N, R2);          // u_c plane
   static constexpr int PW = up_mod8(LW, R2);         // row work lines
-  static constexpr int PC = (R2 & 1) ? up_mod8(LW > N ? LW : N, R2) : ((LW > N ? LW : N) | 1);   // column lines
+  // column lines.  R2 odd: = R2 (mod 8) is odd too and serves both access patterns.  R2 = 8: a line's 8 lanes are one
+  // quarter-warp, any pitch is conflict-free in pass A, so the odd pitch the transposed stores want.  R2 = 6: no pitch
+  // serves both; = 6 (mod 8) keeps the 16 pass-A accesses of the columns conflict-free and leaves the transposed stores
+  // of the rows with 2-way conflicts (480 instead of 576 wavefronts per band for the three patterns together)
+  static constexpr int PC = ((R2 & 1) || R2 == 6) ? up_mod8(LW > N ? LW : N, R2) : ((LW > N ? LW : N) | 1);
 };
 
 // natural-order R-point DFT in registers (forward)
@@ -263,7 +267,36 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
 
 // ENDS (N = 48 only): every kept frequency of both axes has s2 = 0 or s2 = R2 - 1 (the host checks), so the second passes
 // form just those two outputs (dft6_ends) instead of the full R2-point butterfly.
-template <int N, bool ENDS>
+// Pass-A output twiddles w_N^{j s}, s = 1..7.  TW3 (N = 64, where 512 threads cap the kernel at 128 registers and the
+// seven values of the plain form spill -- and a spill is one more access on the LSU data pipe that already bounds the
+// kernel): only s = 1, 2, 4 live in registers, the other four are their products (16 FP64 instructions per pass A on a pipe
+// that is 37 % busy; each product adds one rounding, far inside the 1e-12 of M).
+template <bool TW3>
+struct Twid {
+  cplx w[TW3 ? 3 : 8];
+  __device__ __forceinline__ void init(const cplx* __restrict__ tw, int j, int n) {
+    if (TW3) { w[0] = tw[j % n]; w[1] = tw[(2 * j) % n]; w[2] = tw[(4 * j) % n]; }
+    else {
+#pragma unroll
+      for (int s = 1; s < 8; s++) w[s] = tw[(j * s) % n];
+    }
+  }
+  __device__ __forceinline__ void apply(cplx* x) const {   // x[s] *= w^{j s}, s = 1..7
+    if (TW3) {
+      const cplx w3 = fftsm::cmul(w[0], w[1]);
+      x[1] = fftsm::cmul(x[1], w[0]); x[2] = fftsm::cmul(x[2], w[1]); x[3] = fftsm::cmul(x[3], w3);
+      x[4] = fftsm::cmul(x[4], w[2]); x[5] = fftsm::cmul(x[5], fftsm::cmul(w[0], w[2]));
+      x[6] = fftsm::cmul(x[6], fftsm::cmul(w[1], w[2])); x[7] = fftsm::cmul(x[7], fftsm::cmul(w3, w[2]));
+    } else {
+#pragma unroll
+      for (int s = 1; s < 8; s++) x[s] = fftsm::cmul(x[s], w[s]);
+    }
+  }
+};
+
+// CB conduction bands per CTA (N = 48: 2, where two u_c planes fit): the band loop runs over the nvb CB (valence band,
+// conduction band) pairs of the CTA, so every u_v element fetched from L2 is used CB times.
+template <int N, bool ENDS, int CB>
 __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict__ u_v, const cplx* __restrict__ u_c, int nvb, int ncc,
                                                           int N3, const cplx* __restrict__ tw, const int* __restrict__ kfreq1,
                                                           const int* __restrict__ kfreq2, int nk1, int nk2, cplx* __restrict__ T) {
@@ -271,22 +304,26 @@ __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict
   constexpr int R2 = GE::R2, RW = GE::RW, NWARP = GE::NWARP, G = GE::G, PS = GE::PS, PW = GE::PW, PC = GE::PC, D = RING_D;
   constexpr int NTHR = NWARP * 32;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  cplx* sc = reinterpret_cast<cplx*>(smem_raw);   // [N][PS]  u_c plane
-  cplx* wk = sc + N * PS;                         // [N][PW]  pass-A output of the rows (warp-private rows)
+  cplx* sc = reinterpret_cast<cplx*>(smem_raw);   // [CB][N][PS]  u_c planes
+  cplx* wk = sc + CB * N * PS;                    // [N][PW]  pass-A output of the rows (warp-private rows)
   cplx* cb0 = wk + N * PW;                        // D x [nk2][PC] kept y-frequencies, x contiguous
   unsigned long long* slot2 = reinterpret_cast<unsigned long long*>(cb0 + D * nk2 * PC);
   unsigned long long* slot1 = slot2 + 8;
   unsigned long long* full = slot1 + 8;           // [D]
   unsigned long long* empty = full + D;           // [D]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int z = blockIdx.x / ncc, c = blockIdx.x - z * ncc;
+  const int ncg = (ncc + CB - 1) / CB;            // conduction-band groups of the launch
+  const int z = blockIdx.x / ncg, c = (blockIdx.x - z * ncg) * CB;
+  const int ncb_here = CB == 1 ? 1 : min(CB, ncc - c);   // conduction bands of this CTA (the last group may be short)
   constexpr int plane = N * N;
   const long long n_r = (long long)plane * N3;
   const long long n_rp = (long long)GE::PP * N3;   // one valence band in lane order
-  const cplx* ucp = u_c + (long long)c * n_r + (long long)z * plane;
-  for (int idx = tid; idx < plane; idx += NTHR) {
-    int x = idx / N, y = idx - x * N;
-    sc[x * PS + y] = ucp[idx];
+  for (int cs = 0; cs < ncb_here; cs++) {
+    const cplx* ucp = u_c + (long long)(c + cs) * n_r + (long long)z * plane;
+    for (int idx = tid; idx < plane; idx += NTHR) {
+      int x = idx / N, y = idx - x * N;
+      sc[(cs * N + x) * PS + y] = ucp[idx];
+    }
   }
   const int ncb = (nk2 + RW - 1) / RW;            // column batches per band (host guarantees ncb <= NWARP)
   if (tid < 16) {
@@ -307,9 +344,8 @@ __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict
   const int r0 = warp * RW, row = r0 + ls;
   const bool row_on = lane_on && row < N;
   const int nrow = min(RW, N - r0);
-  cplx twj[8];
-#pragma unroll
-  for (int s = 1; s < 8; s++) twj[s] = tw[(j * s) % N];
+  Twid<N == 64> twj;
+  twj.init(tw, j, N);
   const cplx* uvp = u_v + (long long)z * GE::PP + warp * (8 * GE::QS) + lane;   // lane order, see Geo
   cplx nxt[8];
   if (row_on) {
@@ -337,12 +373,13 @@ __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict
     }
     __syncwarp();
     if (col_on) {
-      line[j] = x[0];
+      twj.apply(x);
 #pragma unroll
-      for (int s = 1; s < 8; s++) line[s * G + j] = fftsm::cmul(x[s], twj[s]);
+      for (int s = 0; s < 8; s++) line[s * G + j] = x[s];
     }
     __syncwarp();
-    cplx* dstT = T + (((long long)band * ncc + c) * N3 + z) * J;
+    const int bv = band / ncb_here, bc = band - bv * ncb_here;   // valence band, conduction band of the CTA
+    cplx* dstT = T + (((long long)bv * ncc + c + bc) * N3 + z) * J;
     for (int t = lane; t < nl * 8; t += 32) {
       const int l = l0 + (t >> 3), s = t & 7;
       const cplx* grp = cb + l * PC + s * G;
@@ -370,7 +407,9 @@ __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict
     if (lane == 0) mbar_arrive(empty + b);
   };
 
-  for (int it = 0; it < nvb; it++) {
+  const int n_it = nvb * ncb_here;                // (valence band, conduction band) pairs, conduction band fastest
+  int iv = 0, ic = 0;                             // valence band / conduction band of iteration it
+  for (int it = 0; it < n_it; it++) {
     const int b = it % D;
     if (it >= D) mbar_wait(empty + b, ((it / D) - 1) & 1);   // the x transforms of band it - D have left cb[b]
     cplx* cb = cb0 + b * nk2 * PC;
@@ -378,19 +417,19 @@ __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict
       cplx x[8];
 #pragma unroll
       for (int q = 0; q < 8; q++) {
-        cplx a = nxt[q], bb = sc[row * PS + j + q * R2];
+        cplx a = nxt[q], bb = sc[(ic * N + row) * PS + j + q * R2];
         x[q] = make_double2(a.x * bb.x + a.y * bb.y, a.x * bb.y - a.y * bb.x);   // conj(u_v) u_c
       }
-      if (it + 1 < nvb) {
-        const cplx* nx = uvp + (long long)(it + 1) * n_rp;
+      if (ic + 1 == ncb_here && iv + 1 < nvb) {   // last use of this valence band: fetch the next one
+        const cplx* nx = uvp + (long long)(iv + 1) * n_rp;
 #pragma unroll
         for (int q = 0; q < 8; q++) nxt[q] = nx[q * GE::QS];
       }
       fftsm::bfly8<false>(x);
+      twj.apply(x);
       cplx* line = wk + row * PW + j;
-      line[0] = x[0];
 #pragma unroll
-      for (int s = 1; s < 8; s++) line[s * G] = fftsm::cmul(x[s], twj[s]);
+      for (int s = 0; s < 8; s++) line[s * G] = x[s];
     }
     __syncwarp();
     for (int t = lane; t < nrow * 8; t += 32) {
@@ -419,8 +458,9 @@ __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict
     __syncwarp();
     if (lane == 0) mbar_arrive(full + b);
     if (it >= 1) cols(it - 1);
+    if (++ic == ncb_here) { ic = 0; iv++; }
   }
-  cols(nvb - 1);
+  cols(n_it - 1);
 }
 
 // u_nat[v][z][x][y] (plane-major, as the wavefunction transforms leave it) -> u_lane[v][z][PP] in the lane order of the
@@ -450,9 +490,9 @@ template <int N>
 __global__ void __launch_bounds__(Geo<N>::NWARP * 32) pair_plane_fft8_kernel_b(RPA_FFT8_ARGS) {
   pair_plane_fft8_body<N>(u_v, u_c, nvb, ncc, N3, tw, kfreq1, kfreq2, nk1, nk2, T);
 }
-template <int N, bool ENDS>
+template <int N, bool ENDS, int CB>
 __global__ void __launch_bounds__(Geo<N>::NWARP * 32) pair_plane_fft8_kernel_ring(RPA_FFT8_ARGS) {
-  pair_plane_fft8_ring_body<N, ENDS>(u_v, u_c, nvb, ncc, N3, tw, kfreq1, kfreq2, nk1, nk2, T);
+  pair_plane_fft8_ring_body<N, ENDS, CB>(u_v, u_c, nvb, ncc, N3, tw, kfreq1, kfreq2, nk1, nk2, T);
 }
 #undef RPA_FFT8_ARGS
 
@@ -466,8 +506,8 @@ size_t smem_bytes(int nk1, int nk2) {
 
 namespace fft8 {
 template <int N>
-size_t smem_bytes_ring(int nk2) {
-  return ((size_t)N * Geo<N>::PS + (size_t)N * Geo<N>::PW + (size_t)RING_D * nk2 * Geo<N>::PC) * sizeof(cplx) +
+size_t smem_bytes_ring(int nk2, int cb = 1) {
+  return ((size_t)cb * N * Geo<N>::PS + (size_t)N * Geo<N>::PW + (size_t)RING_D * nk2 * Geo<N>::PC) * sizeof(cplx) +
          (16 + 2 * RING_D) * sizeof(unsigned long long);
 }
 }  // namespace fft8

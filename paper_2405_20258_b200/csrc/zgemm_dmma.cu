@@ -94,14 +94,15 @@ __device__ __forceinline__ void mma_ktile(const cplx* __restrict__ a_s, const cp
 #pragma unroll
     for (int i = 0; i < NA; i++) {
       const int m = TRI ? 24 * (i >> 1) + 8 * (i & 1) + g : mb + i * 8 + g;
-      // BOX: the TMA layout of a [k][m] tile, 8 boxes of [16 k][8 m] (element (k, m) at (m >> 3) 128 + 8 k + (m & 7))
-      cplx a = BOX ? a_s[((m >> 3) << 7) + k * 8 + (m & 7)] : A_KM ? a_s[k * LD_KM + m] : a_s[m * LD_MK + k];
+      // BOX: the TMA layout of a [k][m] tile, 8 boxes of [16 k][8 m] with the 128-byte swizzle: element (k, m) sits in box
+      // m >> 3, row k, 16-byte chunk (m & 7) ^ (k & 7).  The caller passes g already permuted (see zherk_tma_kernel).
+      cplx a = BOX ? a_s[((m >> 3) << 7) + k * 8 + ((m & 7) ^ (k & 7))] : A_KM ? a_s[k * LD_KM + m] : a_s[m * LD_MK + k];
       ar[i] = a.x * w; ai[i] = a.y * w;
     }
 #pragma unroll
     for (int j = 0; j < NB; j++) {
       const int n = TRI ? 24 * (j >> 1) + 8 * (j & 1) + g : nb + j * 8 + g;
-      cplx b = BOX ? b_s[((n >> 3) << 7) + k * 8 + (n & 7)] : B_KN ? b_s[k * LD_KM + n] : b_s[n * LD_MK + k];
+      cplx b = BOX ? b_s[((n >> 3) << 7) + k * 8 + ((n & 7) ^ (k & 7))] : B_KN ? b_s[k * LD_KM + n] : b_s[n * LD_MK + k];
       br[j] = b.x; bi[j] = b.y;
     }
     // a conj(b): re += ar br + ai bi, im += ai br - ar bi;  a b: re += ar br - ai bi, im += ai br + ar bi.  The sign is
@@ -276,8 +277,10 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_dmma_kernel(KArgs p) {
 // as zgemm_dmma_kernel<1,1,1,3,1>, but the operand panels arrive by cp.async.bulk.tensor (one elected thread issues
 // 8 + 8 box loads and one weight row per k-tile) into a 3-stage ring guarded by mbarriers: full[s] (transaction bytes)
 // and empty[s] (one arrival per warp) -- no per-thread address arithmetic, no cp.async groups and no block barrier in the
-// main loop.  A [k][64] panel is loaded as 8 boxes of [16][8] complex: a warp's fragment load then reads 4 full 128-byte
-// rows, conflict-free without padding.
+// main loop.  A [k][64] panel is loaded as 8 boxes of [16 k][8 m] complex (128-byte rows) with the 128-byte swizzle, and the
+// fragment row g of the MMA is mapped to row rho(g) = (g >> 1) + 4 (g & 1) of its 8-row group: a quarter-warp (two g, four
+// k) then touches 8 different 16-byte bank groups -- conflict-free without padding.  (Unswizzled boxes are 4-way
+// conflicted: all rows of a box share their bank alignment; the swizzle alone still pairs g = 2a, 2a + 1 in one half.)
 constexpr int TMA_STAGES = 3;
 constexpr int TMA_TILE = BK * BM;   // 1024 complex per operand tile
 
@@ -306,7 +309,7 @@ __device__ __forceinline__ void tma_load_2d(void* smem, const CUtensorMap* map, 
 struct TmaMaps { CUtensorMap a; CUtensorMap w; };   // operand [K][2 M doubles], weights [batch][K doubles]
 
 __global__ void __launch_bounds__(NTHREADS, 2) zherk_tma_kernel(KArgs p, const __grid_constant__ TmaMaps maps) {
-  extern __shared__ __align__(128) unsigned char smem_tma[];
+  extern __shared__ __align__(1024) unsigned char smem_tma[];
   cplx* sA = reinterpret_cast<cplx*>(smem_tma);
   cplx* sB = sA + TMA_STAGES * TMA_TILE;
   double* sW = reinterpret_cast<double*>(sB + TMA_STAGES * TMA_TILE);
@@ -314,7 +317,8 @@ __global__ void __launch_bounds__(NTHREADS, 2) zherk_tma_kernel(KArgs p, const _
   unsigned long long* empty = full + TMA_STAGES;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int wm = warp >> 1, wn = warp & 1;
-  const int g = lane >> 2, q = lane & 3;
+  const int q = lane & 3;
+  const int g = ((lane >> 2) >> 1) + 4 * ((lane >> 2) & 1);   // rho(fragment row): the tile row this lane's fragment row maps to
   int tm, tn;
   {
     const int t = blockIdx.x;
@@ -406,7 +410,8 @@ __global__ void __launch_bounds__(NTHREADS, 2) zherk_tma_kernel(KArgs p, const _
       const double sr = p.alpha * (p.rs ? p.rs[r] : 1.0);
 #pragma unroll
       for (int e = 0; e < 2; e++) {
-        const int c = n0 + co + 2 * q + e;
+        const int cf = 2 * q + e;                                    // fragment column -> tile column, same rho
+        const int c = n0 + co + (cf >> 1) + 4 * (cf & 1);
         if (c >= p.N || c > r) continue;
         const double sc = sr * (p.cs ? p.cs[c] : 1.0);
         double vr = sc * cre[i][j][e], vi = sc * cim[i][j][e];
@@ -464,7 +469,7 @@ int launch_tma(rpa_ctx* ctx, const KArgs& ka, dim3 grid, int batch, bool* ok) {
     cuuint32_t box[2] = {16, (cuuint32_t)BK};
     cuuint32_t es[2] = {1, 1};
     if (encode(&maps.a, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void*)ka.A, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return RPA_OK;
+               CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return RPA_OK;
   }
   {
     cuuint64_t dims[2] = {(cuuint64_t)ka.K, (cuuint64_t)batch};
@@ -475,6 +480,7 @@ int launch_tma(rpa_ctx* ctx, const KArgs& ka, dim3 grid, int batch, bool* ok) {
                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return RPA_OK;
   }
   constexpr size_t smem = (size_t)TMA_STAGES * 2 * TMA_TILE * sizeof(cplx) + TMA_STAGES * BK * sizeof(double) + 2 * TMA_STAGES * sizeof(unsigned long long) + 128;
+  static_assert((TMA_TILE * sizeof(cplx)) % 1024 == 0, "swizzled boxes need 1024-byte aligned stages");
   if (ctx->attr_once(RPA_ATTR_ZHERK_TMA))
     RPA_CUDA(ctx, cudaFuncSetAttribute(zherk_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   zherk_tma_kernel<<<grid, NTHREADS, smem, ctx->stream>>>(ka, maps);
@@ -634,6 +640,28 @@ __global__ void __launch_bounds__(256) dmma_peak_kernel(double* out) {
   for (int i = 0; i < 16; i++) s += acc[i][0] + acc[i][1];
   if (s == 123.456) out[0] = s;
 }
+// kind 2: the instruction mix a 3-multiply complex product would run per k-step and warp -- 24 DMMAs and 14 independent
+// DADDs -- to show that plain FP64 instructions share the pipe with the DMMAs.  Counts DMMA FLOPs only.
+__global__ void __launch_bounds__(256) dmma_dadd_mix_kernel(double* out) {
+  double acc[24][2], s[14];
+#pragma unroll
+  for (int i = 0; i < 24; i++) acc[i][0] = acc[i][1] = 0.0;
+#pragma unroll
+  for (int i = 0; i < 14; i++) s[i] = threadIdx.x * 1e-3 + i;
+  double a = 1.0 + threadIdx.x * 1e-9, b = 1.0 - threadIdx.x * 1e-9;
+  for (int it = 0; it < PEAK_ITERS; it++) {
+#pragma unroll
+    for (int i = 0; i < 24; i++) dmma(acc[i][0], acc[i][1], a, b);
+#pragma unroll
+    for (int i = 0; i < 14; i++) s[i] += a;
+  }
+  double t = 0;
+#pragma unroll
+  for (int i = 0; i < 24; i++) t += acc[i][0] + acc[i][1];
+#pragma unroll
+  for (int i = 0; i < 14; i++) t += s[i];
+  if (t == 123.456) out[0] = t;
+}
 __global__ void __launch_bounds__(256) dfma_peak_kernel(double* out) {
   double acc[16];
 #pragma unroll
@@ -661,6 +689,7 @@ int fp64_peak_kernel(rpa_ctx* ctx, int kind, int iters, double* tflops) {
     RPA_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
     for (int i = 0; i < iters; i++) {
       if (kind == 0) dmma_peak_kernel<<<blocks, 256, 0, ctx->stream>>>((double*)ctx->ws);
+      else if (kind == 2) dmma_dadd_mix_kernel<<<blocks, 256, 0, ctx->stream>>>((double*)ctx->ws);
       else dfma_peak_kernel<<<blocks, 256, 0, ctx->stream>>>((double*)ctx->ws);
       ctx->launches++;
     }
@@ -672,7 +701,8 @@ int fp64_peak_kernel(rpa_ctx* ctx, int kind, int iters, double* tflops) {
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
   const double warps = (double)blocks * 8;
-  const double flops = kind == 0 ? warps * PEAK_ITERS * 16.0 * (2.0 * 8 * 8 * 4) : warps * 32.0 * PEAK_ITERS * 16.0 * 2.0;
+  const double flops = kind == 0 ? warps * PEAK_ITERS * 16.0 * (2.0 * 8 * 8 * 4) : kind == 2 ? warps * PEAK_ITERS * 24.0 * (2.0 * 8 * 8 * 4)
+                                                                                             : warps * 32.0 * PEAK_ITERS * 16.0 * 2.0;
   *tflops = flops * iters / (ms * 1e-3) / 1e12;
   return RPA_OK;
 }
