@@ -436,6 +436,8 @@ def main():
             out["traffic_source"] = f"{ne.get('source')} (commit {prof_tab.get('commit')})"
             if unit == "B" and out["traffic"]:
                 out["traffic_over_algorithmic"] = out["traffic"] / per_launch
+            if "units" in ne:          # pipe utilisation of that launch as ncu measured it
+                out["ncu_units"] = ne["units"]
             if "binding_unit" in ne:   # where DRAM traffic is far below the algorithmic bytes the roof is elsewhere: say which unit
                 out["binding_unit"] = ne["binding_unit"]
         return out
