@@ -361,7 +361,10 @@ MtxelSizes mtxel_sizes(const rpa_ctx* ctx, int nvb, int nc) {
     // the chunk, not more than a quarter below the budget, whose CTAs come closest to whole waves
     const int per_cta = (ctx->fft[0] == 48 && ctx->fft[1] == 48) ? 2 : 1;
     double best = -1.0; int best_ncc = ncc;
-    for (int cand = ncc; cand >= std::max(16, ncc - ncc / 4); cand--) {
+#ifndef RPA_WAVE_CHUNK
+#define RPA_WAVE_CHUNK 1
+#endif
+    for (int cand = ncc; RPA_WAVE_CHUNK && cand >= std::max(16, ncc - ncc / 4); cand--) {
       const long long ctas = (long long)((cand + per_cta - 1) / per_cta) * ctx->fft[2];
       const long long waves = (ctas + ctx->sm_count - 1) / ctx->sm_count;
       const double eff = (double)ctas / (double)(waves * ctx->sm_count);

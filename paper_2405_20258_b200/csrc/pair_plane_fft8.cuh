@@ -344,7 +344,10 @@ __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict
   const int r0 = warp * RW, row = r0 + ls;
   const bool row_on = lane_on && row < N;
   const int nrow = min(RW, N - r0);
-  Twid<N == 64> twj;
+#ifndef RPA_TW3
+#define RPA_TW3 1
+#endif
+  Twid<N == 64 && RPA_TW3> twj;
   twj.init(tw, j, N);
   const cplx* uvp = u_v + (long long)z * GE::PP + warp * (8 * GE::QS) + lane;   // lane order, see Geo
   cplx nxt[8];
@@ -408,8 +411,9 @@ __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict
   };
 
   const int n_it = nvb * ncb_here;                // (valence band, conduction band) pairs, conduction band fastest
-  int iv = 0, ic = 0;                             // valence band / conduction band of iteration it
+  int iv_run = 0, ic_run = 0;                     // valence band / conduction band of iteration it
   for (int it = 0; it < n_it; it++) {
+    const int iv = CB == 1 ? it : iv_run, ic = CB == 1 ? 0 : ic_run;
     const int b = it % D;
     if (it >= D) mbar_wait(empty + b, ((it / D) - 1) & 1);   // the x transforms of band it - D have left cb[b]
     cplx* cb = cb0 + b * nk2 * PC;
@@ -458,7 +462,7 @@ __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict
     __syncwarp();
     if (lane == 0) mbar_arrive(full + b);
     if (it >= 1) cols(it - 1);
-    if (++ic == ncb_here) { ic = 0; iv++; }
+    if (CB > 1 && ++ic_run == ncb_here) { ic_run = 0; iv_run++; }
   }
   cols(n_it - 1);
 }

@@ -674,6 +674,31 @@ def test_n_eig_sweep_against_golden(name, idx, n_v, n_c, capsys):
                   f"{m['mtxel']:.1f} {m['chi0_static']:.1f} {m['basis']:.1f} {m['chi_freq']:.1f} {m['energy']:.2f}")
 
 
+def test_two_contexts_in_one_process_interleaved():
+    """Kernel attributes, tuning switches and plans are per context: two contexts with different grids (24^3 and 48 x 48 x 12),
+    created one after the other and used alternately, must both give the oracle's M and chi~0(0)."""
+    import paper_2405_20258_b200 as rpa
+    import torch
+    inp_a = make_inputs(0, n_v=2, n_c=9)
+    inp_b = make_inputs(cfg_small_grid((48, 48, 12), (12.0, 12.0, 3.0), 3.0, 1.5))
+    ctx_a = make_ctx(inp_a, 2, 9, 4, 6)
+    ctx_b = make_ctx(inp_b, 3, 9, 4, 6)
+    try:
+        for rep in range(2):
+            for ctx, inp in ((ctx_a, inp_a), (ctx_b, inp_b)):
+                nv, nc = inp.psi_v.shape[0], inp.psi_c.shape[0]
+                M = torch.empty((nv, nc, inp.n_g), dtype=torch.complex128, device="cuda")
+                rpa.rpa_mtxel(ctx, dev(inp.psi_v), dev(inp.psi_c), M)
+                Mref = orc.mtxel(inp.psi_v, inp.psi_c, inp.g_wfn, inp.g_eps, inp.fft)
+                assert maxnorm_rel(M.cpu().numpy(), Mref) <= 1e-12
+                chi = torch.empty((inp.n_g, inp.n_g), dtype=torch.complex128, device="cuda")
+                rpa.rpa_chi0_static(ctx, M, dev(inp.e_v), dev(inp.e_c), False, chi)
+                assert maxnorm_rel(chi.cpu().numpy(), orc.chi0(Mref, inp.e_v, inp.e_c, inp.vcoul)) <= TOL_CHI
+    finally:
+        rpa.rpa_destroy(ctx_a)
+        rpa.rpa_destroy(ctx_b)
+
+
 def test_partial_occupations_against_oracle():
     """NEXT-4: rpa_chi0_static_occ / rpa_chi_subspace_freq_occ on random M with a smeared Fermi edge (bands with
     0 < f < 1 sit in both band sets), against the oracle's occupation-weighted sums; f_v = 1, f_c = 0 must reproduce
