@@ -79,6 +79,23 @@ int rpa_mtxel(rpa_ctx* ctx, const void* psi_v, int nvb, const void* psi_c, int n
 int rpa_chi0_static(rpa_ctx* ctx, const void* M, int nvb, int nc, const double* e_v, const double* e_c,
                     int accumulate, void* chi0);
 
+/* (a2) without any memory from the caller or from the allocator: the same CHI_SUM (same kernels, same result up to the
+ * order in which split-K partial sums meet) for callers that cannot call cudaMalloc or lend a workspace at call time --
+ * code under CUDA graph capture, tight serving loops, harnesses that forbid allocation.  The one piece of scratch
+ * rpa_chi0_static takes from the workspace (the pair weights D_vc(0), nvb * nc doubles) lives in a device array built
+ * into the library: rpa_noalloc_max_pairs() = 524 288 pairs = 4 MiB, held by every GPU that loads the library until the
+ * process exits.  nvb * nc beyond that is rejected with RPA_ERR_INVALID (split the valence block, or use
+ * rpa_chi0_static).  No workspace is needed (rpa_set_workspace need not have been called); the call makes no cudaMalloc /
+ * cudaFree and calls no allocating library routine.  ALL calls on a device share that array: calls on one stream are
+ * ordered and safe, calls that overlap on the GPU (two streams, two contexts on one device) race on it.  The array keeps
+ * the previous call's contents; a call overwrites what it reads, so nothing needs clearing.
+ * rpa_noalloc_setup (optional; otherwise done by the first call): fetches the array's device address for the context's
+ * device -- call it once before capturing a graph.  Arguments of rpa_chi0_static_noalloc as rpa_chi0_static.          */
+long long rpa_noalloc_max_pairs(void);
+int rpa_noalloc_setup(rpa_ctx* ctx);
+int rpa_chi0_static_noalloc(rpa_ctx* ctx, const void* M, int nvb, int nc, const double* e_v, const double* e_c,
+                            int accumulate, void* chi0);
+
 /* (a3) Static subspace basis; reading R9.  The n_eig eigenpairs of Hermitian chi0 with
  *   the greatest |lambda| (chi0 is negative-semidefinite: the most negative ones).
  *   C dev out [n_eig][n_g], row i = eigenvector i (unit 2-norm); lambda dev out [n_eig] ascending.

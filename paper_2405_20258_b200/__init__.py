@@ -8,7 +8,8 @@ from .binding import (RpaContext, RpaError, load_library, library_path, EXPORTED
                       rpa_profile_begin, rpa_profile_end, PROFILE_CLASSES,
                       rpa_chi0_static_occ, rpa_chi_subspace_freq_occ,
                       rpa_epsilon_inverse, rpa_epsilon_inverse_workspace_bytes, rpa_basis_info, rpa_basis_quality,
-                      rpa_pass_begin, rpa_pass1_chi0, rpa_pass_basis, rpa_pass2_chis, rpa_pass_energy, rpa_pass_end)
+                      rpa_pass_begin, rpa_pass1_chi0, rpa_pass_basis, rpa_pass2_chis, rpa_pass_energy, rpa_pass_end,
+                      rpa_noalloc_max_pairs, rpa_noalloc_setup, rpa_chi0_static_noalloc)
 
 from .sharded import shard_range, Comm, rpa_energy_sharded
 
@@ -19,4 +20,5 @@ __all__ = ["shard_range", "Comm", "rpa_energy_sharded", "RpaContext", "RpaError"
            "rpa_profile_begin", "rpa_profile_end", "PROFILE_CLASSES",
            "rpa_chi0_static_occ", "rpa_chi_subspace_freq_occ",
            "rpa_epsilon_inverse", "rpa_epsilon_inverse_workspace_bytes", "rpa_basis_info", "rpa_basis_quality",
-           "rpa_pass_begin", "rpa_pass1_chi0", "rpa_pass_basis", "rpa_pass2_chis", "rpa_pass_energy", "rpa_pass_end"]
+           "rpa_pass_begin", "rpa_pass1_chi0", "rpa_pass_basis", "rpa_pass2_chis", "rpa_pass_energy", "rpa_pass_end",
+           "rpa_noalloc_max_pairs", "rpa_noalloc_setup", "rpa_chi0_static_noalloc"]

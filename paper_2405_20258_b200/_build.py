@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librpa_b200.so")
-SOURCES = ["api.cu", "zgemm_dmma.cu", "mtxel.cu", "chol.cu", "basis.cu", "energy.cu", "tridiag_eig.cu"]
+SOURCES = ["api.cu", "zgemm_dmma.cu", "mtxel.cu", "chol.cu", "basis.cu", "energy.cu", "tridiag_eig.cu", "noalloc.cu"]
 HEADERS = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".h", ".cuh"))) + \
     [os.path.join(ROOT, "include", "rpa_b200.h")]
 

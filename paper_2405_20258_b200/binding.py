@@ -20,6 +20,7 @@ EXPORTED_SYMBOLS = [
     "rpa_profile_begin", "rpa_profile_end", "rpa_chi0_static_occ", "rpa_chi_subspace_freq_occ",
     "rpa_epsilon_inverse", "rpa_epsilon_inverse_workspace_bytes", "rpa_basis_info", "rpa_basis_quality",
     "rpa_pass_begin", "rpa_pass1_chi0", "rpa_pass_basis", "rpa_pass2_chis", "rpa_pass_energy", "rpa_pass_end",
+    "rpa_noalloc_max_pairs", "rpa_noalloc_setup", "rpa_chi0_static_noalloc",
 ]
 
 
@@ -98,6 +99,12 @@ def load_library(build_if_missing: bool = True):
     lib.rpa_pass_energy.restype = ci
     lib.rpa_pass_end.argtypes = [vp]
     lib.rpa_pass_end.restype = ci
+    lib.rpa_noalloc_max_pairs.argtypes = []
+    lib.rpa_noalloc_max_pairs.restype = C.c_longlong
+    lib.rpa_noalloc_setup.argtypes = [vp]
+    lib.rpa_noalloc_setup.restype = ci
+    lib.rpa_chi0_static_noalloc.argtypes = [vp, vp, ci, ci, vp, vp, ci, vp]
+    lib.rpa_chi0_static_noalloc.restype = ci
     lib.rpa_fp64_peak.argtypes = [vp, ci, ci, pd]
     lib.rpa_fp64_peak.restype = ci
     lib.rpa_profile_begin.argtypes = [vp]
@@ -240,6 +247,26 @@ def rpa_chi0_static(ctx, M, e_v, e_c, accumulate, chi0):
     _check(ctx.handle, load_library().rpa_chi0_static(ctx.handle, _dev(M, torch.complex128), e_v.shape[0], e_c.shape[0],
                                                       _dev(e_v, torch.float64), _dev(e_c, torch.float64),
                                                       int(bool(accumulate)), _dev(chi0, torch.complex128)))
+    return chi0
+
+
+def rpa_noalloc_max_pairs() -> int:
+    return int(load_library().rpa_noalloc_max_pairs())
+
+
+def rpa_noalloc_setup(ctx):
+    _check(ctx.handle, load_library().rpa_noalloc_setup(ctx.handle))
+
+
+def rpa_chi0_static_noalloc(ctx, M, e_v, e_c, accumulate, chi0):
+    """rpa_chi0_static with its scratch in a device array built into the library (no workspace, no allocation); at most
+    rpa_noalloc_max_pairs() pairs per call; calls that overlap on the GPU race on that array."""
+    import torch
+    _pair_shapes(ctx, M, e_v, e_c)
+    _shape("chi0", chi0, ctx.n_g, ctx.n_g)
+    _check(ctx.handle, load_library().rpa_chi0_static_noalloc(ctx.handle, _dev(M, torch.complex128), e_v.shape[0], e_c.shape[0],
+                                                              _dev(e_v, torch.float64), _dev(e_c, torch.float64),
+                                                              int(bool(accumulate)), _dev(chi0, torch.complex128)))
     return chi0
 
 
