@@ -57,6 +57,7 @@ struct KArgs {
   const double* wk; long long strideW;
   long long strideA, strideB, strideC;
   int tiles_n, kt_per_split, n_kt;
+  int batch_fastest;   // zherk_tma_kernel only: grid = (batch, tiles, split) instead of (tiles, split, batch)
 };
 
 template <bool KM>
@@ -321,7 +322,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) zherk_tma_kernel(KArgs p, const _
   const int g = ((lane >> 2) >> 1) + 4 * ((lane >> 2) & 1);   // rho(fragment row): the tile row this lane's fragment row maps to
   int tm, tn;
   {
-    const int t = blockIdx.x;
+    const int t = p.batch_fastest ? blockIdx.y : blockIdx.x;
     tm = (int)((sqrt(8.0 * t + 1.0) - 1.0) * 0.5);
     while ((tm + 1) * (tm + 2) / 2 <= t) tm++;
     while (tm * (tm + 1) / 2 > t) tm--;
@@ -329,9 +330,11 @@ __global__ void __launch_bounds__(NTHREADS, 2) zherk_tma_kernel(KArgs p, const _
   }
   const int m0 = tm * BM, n0 = tn * BN;
   const bool diag = tm == tn;
-  const int batch = blockIdx.z;
+  // batch_fastest (chi_s: one operand, n_w weight rows): the CTAs of one tile and all frequencies are neighbours in the
+  // launch order, so the CTAs resident together read the SAME operand panels at the same pace -- L2 serves 15 of 16
+  const int batch = p.batch_fastest ? blockIdx.x : blockIdx.z;
   cplx* C = p.C + batch * p.strideC;
-  const int kt0 = blockIdx.y * p.kt_per_split;
+  const int kt0 = (p.batch_fastest ? blockIdx.z : blockIdx.y) * p.kt_per_split;
   const int kt1 = min(p.n_kt, kt0 + p.kt_per_split);
   const int nkt = kt1 - kt0;
   if (nkt <= 0) return;
@@ -483,7 +486,10 @@ int launch_tma(rpa_ctx* ctx, const KArgs& ka, dim3 grid, int batch, bool* ok) {
   static_assert((TMA_TILE * sizeof(cplx)) % 1024 == 0, "swizzled boxes need 1024-byte aligned stages");
   if (ctx->attr_once(RPA_ATTR_ZHERK_TMA))
     RPA_CUDA(ctx, cudaFuncSetAttribute(zherk_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  zherk_tma_kernel<<<grid, NTHREADS, smem, ctx->stream>>>(ka, maps);
+  KArgs kb = ka;
+  kb.batch_fastest = batch > 1 && ka.strideA == 0 && grid.x <= 65535 ? 1 : 0;
+  if (kb.batch_fastest) grid = dim3(grid.z, grid.x, grid.y);
+  zherk_tma_kernel<<<grid, NTHREADS, smem, ctx->stream>>>(kb, maps);
   RPA_LAUNCH_CHECK(ctx);
   *ok = true;
   return RPA_OK;
@@ -511,6 +517,7 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
   ka.alpha = p.alpha; ka.rs = p.rs; ka.cs = p.cs;
   ka.wk = p.wk; ka.strideW = p.strideW;
   ka.strideA = p.strideA; ka.strideB = p.strideB; ka.strideC = p.strideC;
+  ka.batch_fastest = 0;
   const int tiles_m = (p.M + BM - 1) / BM, tiles_n = (p.N + BN - 1) / BN;
   ka.tiles_n = tiles_n;
   const long long tiles = p.herm ? (long long)tiles_m * (tiles_m + 1) / 2 : (long long)tiles_m * tiles_n;
