@@ -83,7 +83,7 @@ struct rpa_ctx {
 // attr_once ids
 enum { RPA_ATTR_ZGEMM = 0 /* + 16 layout/HERM combinations */, RPA_ATTR_AXIS = 16 /* + 4 */, RPA_ATTR_FFT8 = 20 /* + 4 */,
        RPA_ATTR_ZFFT8 = 24, RPA_ATTR_POTRF = 25, RPA_ATTR_TRSM = 26, RPA_ATTR_JACOBI = 27, RPA_ATTR_PLANE_GENERIC = 28 /* + 2 */,
-       RPA_ATTR_WFN = 30 /* + 4 */, RPA_ATTR_ZHERK_TMA = 34 };
+       RPA_ATTR_WFN = 30 /* + 4 */, RPA_ATTR_ZHERK_TMA = 34, RPA_ATTR_ZGEMM_TMA_MK = 35 };
 
 int rpa_fail(rpa_ctx* ctx, int code, const char* fmt, ...);
 #define RPA_CUDA(ctx, call)                                                              \

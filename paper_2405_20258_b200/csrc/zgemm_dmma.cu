@@ -82,7 +82,7 @@ __device__ __forceinline__ void load_tile(cplx* s, const cplx* g, long long ld, 
 // Hermitian tile.  TRI = true: three 2 x 2 lower fragment triangles on the diagonal at 0, 24, 48 (slot [t][0] =
 // (24t, 24t), [t][1] = (24t+8, 24t), [t][2] = (24t+8, 24t+8)).  3 x 3 x 3 + TRI tile the 36 fragments on or below the
 // diagonal of a diagonal Hermitian tile, 9 per warp (see the kernel).
-template <bool A_KM, bool B_KN, bool CONJ_B, int NI, int NJ, bool TRI, bool BOX = false>
+template <bool A_KM, bool B_KN, bool CONJ_B, int NI, int NJ, bool TRI, int BOX = 0>
 __device__ __forceinline__ void mma_ktile(const cplx* __restrict__ a_s, const cplx* __restrict__ b_s,
                                           const double* __restrict__ w_s, int g, int q, int mb, int nb,
                                           double (&cre)[4][4][2], double (&cim)[4][4][2], bool skip_upper = false) {
@@ -97,13 +97,18 @@ __device__ __forceinline__ void mma_ktile(const cplx* __restrict__ a_s, const cp
       const int m = TRI ? 24 * (i >> 1) + 8 * (i & 1) + g : mb + i * 8 + g;
       // BOX: the TMA layout of a [k][m] tile, 8 boxes of [16 k][8 m] with the 128-byte swizzle: element (k, m) sits in box
       // m >> 3, row k, 16-byte chunk (m & 7) ^ (k & 7).  The caller passes g already permuted (see zherk_tma_kernel).
-      cplx a = BOX ? a_s[((m >> 3) << 7) + k * 8 + ((m & 7) ^ (k & 7))] : A_KM ? a_s[k * LD_KM + m] : a_s[m * LD_MK + k];
+      // BOX 2: the TMA layout of an [m][k] tile, 2 boxes of [64 m][8 k], swizzled: element (m, k) in box k >> 3, row m, chunk (k & 7) ^ (m & 7)
+      cplx a = BOX == 1 ? a_s[((m >> 3) << 7) + k * 8 + ((m & 7) ^ (k & 7))]
+             : BOX == 2 ? a_s[((k >> 3) << 9) + m * 8 + ((k & 7) ^ (m & 7))]
+             : A_KM ? a_s[k * LD_KM + m] : a_s[m * LD_MK + k];
       ar[i] = a.x * w; ai[i] = a.y * w;
     }
 #pragma unroll
     for (int j = 0; j < NB; j++) {
       const int n = TRI ? 24 * (j >> 1) + 8 * (j & 1) + g : nb + j * 8 + g;
-      cplx b = BOX ? b_s[((n >> 3) << 7) + k * 8 + ((n & 7) ^ (k & 7))] : B_KN ? b_s[k * LD_KM + n] : b_s[n * LD_MK + k];
+      cplx b = BOX == 1 ? b_s[((n >> 3) << 7) + k * 8 + ((n & 7) ^ (k & 7))]
+             : BOX == 2 ? b_s[((k >> 3) << 9) + n * 8 + ((k & 7) ^ (n & 7))]
+             : B_KN ? b_s[k * LD_KM + n] : b_s[n * LD_MK + k];
       br[j] = b.x; bi[j] = b.y;
     }
     // a conj(b): re += ar br + ai bi, im += ai br - ar bi;  a b: re += ar br - ai bi, im += ai br + ar bi.  The sign is
@@ -391,12 +396,12 @@ __global__ void __launch_bounds__(NTHREADS, 2) zherk_tma_kernel(KArgs p, const _
     const cplx* b_s = diag ? a_s : sB + st * TMA_TILE;
     const double* w_s = sW + st * BK;
     if (mode == 0) {
-      if (ni == 4) mma_ktile<true, true, true, 4, 4, false, true>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
-      else if (ni == 3) mma_ktile<true, true, true, 3, 4, false, true>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
-      else if (ni == 2) mma_ktile<true, true, true, 2, 4, false, true>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
-      else mma_ktile<true, true, true, 1, 4, false, true>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
-    } else if (mode == 1) mma_ktile<true, true, true, 3, 3, false, true>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
-    else mma_ktile<true, true, true, 3, 3, true, true>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+      if (ni == 4) mma_ktile<true, true, true, 4, 4, false, 1>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+      else if (ni == 3) mma_ktile<true, true, true, 3, 4, false, 1>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+      else if (ni == 2) mma_ktile<true, true, true, 2, 4, false, 1>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+      else mma_ktile<true, true, true, 1, 4, false, 1>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+    } else if (mode == 1) mma_ktile<true, true, true, 3, 3, false, 1>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
+    else mma_ktile<true, true, true, 3, 3, true, 1>(a_s, b_s, w_s, g, q, mb, nb, cre, cim);
     __syncwarp();
     if (lane == 0) tma_mbar_arrive(empty + st);
   }
@@ -424,6 +429,86 @@ __global__ void __launch_bounds__(NTHREADS, 2) zherk_tma_kernel(KArgs p, const _
         if (p.accumulate) { cplx o = *dst; vr += o.x; vi += o.y; }
         *dst = make_double2(vr, vi);
         if (c < r) C[(long long)c * p.ldc + r] = make_double2(vr, -vi);
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// TMA-staged general product for operands stored [m][k] and [n][k] (k contiguous): the projection B_vc = C^H v^1/2 M_vc
+// (eq. 7), C[m][n] = sum_k w_k A[m][k] conj(B[n][k]).  Same ring, barriers and warp tiles as
+// zherk_tma_kernel; a 64 x 16 operand tile arrives as two boxes of [64 rows][8 k] (128-byte rows, 128-byte swizzle), and
+// with the same fragment-row map rho a quarter-warp's fragment load touches 8 different bank groups.  One k-split, plain
+// stores (the projection has tens of thousands of tiles), rows / columns / k beyond the matrix are zero-filled by TMA.
+struct TmaMapsMK { CUtensorMap a; CUtensorMap b; CUtensorMap w; };
+
+__global__ void __launch_bounds__(NTHREADS, 2) zgemm_tma_mk_kernel(KArgs p, const __grid_constant__ TmaMapsMK maps) {
+  extern __shared__ __align__(1024) unsigned char smem_tma[];
+  cplx* sA = reinterpret_cast<cplx*>(smem_tma);
+  cplx* sB = sA + TMA_STAGES * TMA_TILE;
+  double* sW = reinterpret_cast<double*>(sB + TMA_STAGES * TMA_TILE);
+  unsigned long long* full = reinterpret_cast<unsigned long long*>(sW + TMA_STAGES * BK);
+  unsigned long long* empty = full + TMA_STAGES;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wm = warp >> 1, wn = warp & 1;
+  const int q = lane & 3;
+  const int g = ((lane >> 2) >> 1) + 4 * ((lane >> 2) & 1);   // rho(fragment row), see zherk_tma_kernel
+  const int tm = blockIdx.x / p.tiles_n, tn = blockIdx.x % p.tiles_n;
+  const int m0 = tm * BM, n0 = tn * BN;
+  const int nkt = p.n_kt;
+  if (tid == 0) {
+    for (int s = 0; s < TMA_STAGES; s++) { tma_mbar_init(full + s, 1); tma_mbar_init(empty + s, NTHREADS / 32); }
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  __syncthreads();
+  constexpr unsigned stage_bytes = (unsigned)(2 * TMA_TILE * sizeof(cplx) + BK * sizeof(double));
+  auto issue = [&](int stage, int kt) {   // one thread
+    const int k0 = kt * BK;
+    tma_mbar_expect(full + stage, stage_bytes);
+#pragma unroll
+    for (int b = 0; b < 2; b++) {
+      tma_load_2d(sA + stage * TMA_TILE + b * 512, &maps.a, 2 * (k0 + 8 * b), m0, full + stage);
+      tma_load_2d(sB + stage * TMA_TILE + b * 512, &maps.b, 2 * (k0 + 8 * b), n0, full + stage);
+    }
+    tma_load_2d(sW + stage * BK, &maps.w, k0, 0, full + stage);
+  };
+  const int mb = wm * 32, nb = wn * 32;
+  double cre[4][4][2], cim[4][4][2];
+#pragma unroll
+  for (int i = 0; i < 4; i++)
+#pragma unroll
+    for (int j = 0; j < 4; j++) { cre[i][j][0] = cre[i][j][1] = 0.0; cim[i][j][0] = cim[i][j][1] = 0.0; }
+
+  if (tid == 0)
+    for (int s = 0; s < TMA_STAGES - 1 && s < nkt; s++) issue(s, s);
+  for (int it = 0; it < nkt; it++) {
+    const int st = it % TMA_STAGES;
+    if (tid == 0) {   // refill the stage all warps left one iteration ago
+      const int nx = it + TMA_STAGES - 1;
+      if (nx < nkt) {
+        const int sx = nx % TMA_STAGES;
+        if (nx >= TMA_STAGES) tma_mbar_wait(empty + sx, (unsigned)(((nx / TMA_STAGES) - 1) & 1));
+        issue(sx, nx);
+      }
+    }
+    __syncwarp();
+    tma_mbar_wait(full + st, (unsigned)((it / TMA_STAGES) & 1));
+    mma_ktile<false, false, true, 4, 4, false, 2>(sA + st * TMA_TILE, sB + st * TMA_TILE, sW + st * BK, g, q, mb, nb, cre, cim);
+    __syncwarp();
+    if (lane == 0) tma_mbar_arrive(empty + st);
+  }
+#pragma unroll
+  for (int i = 0; i < 4; i++) {
+    const int r = m0 + mb + i * 8 + g;
+    if (r >= p.M) continue;
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+#pragma unroll
+      for (int e = 0; e < 2; e++) {
+        const int cf = 2 * q + e;                                    // fragment column -> tile column, same rho
+        const int c = n0 + nb + j * 8 + (cf >> 1) + 4 * (cf & 1);
+        if (c >= p.N) continue;
+        p.C[(long long)r * p.ldc + c] = make_double2(p.alpha * cre[i][j][e], p.alpha * cim[i][j][e]);
       }
     }
   }
@@ -490,6 +575,44 @@ int launch_tma(rpa_ctx* ctx, const KArgs& ka, dim3 grid, int batch, bool* ok) {
   kb.batch_fastest = batch > 1 && ka.strideA == 0 && grid.x <= 65535 ? 1 : 0;
   if (kb.batch_fastest) grid = dim3(grid.z, grid.x, grid.y);
   zherk_tma_kernel<<<grid, NTHREADS, smem, ctx->stream>>>(kb, maps);
+  RPA_LAUNCH_CHECK(ctx);
+  *ok = true;
+  return RPA_OK;
+}
+
+// Tensor maps + launch of zgemm_tma_mk_kernel; *ok = false (and nothing launched) when TMA's rules are not met.
+int launch_tma_mk(rpa_ctx* ctx, const KArgs& ka, dim3 grid, bool* ok) {
+  *ok = false;
+  if (!ctx->tma_encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) { (void)cudaGetLastError(); return RPA_OK; }
+    ctx->tma_encode = fn;
+  }
+  auto encode = reinterpret_cast<PFN_cuTensorMapEncodeTiled>(ctx->tma_encode);
+  if (((uintptr_t)ka.A & 15) || ((uintptr_t)ka.B & 15) || ((uintptr_t)ka.wk & 15)) return RPA_OK;
+  TmaMapsMK maps;
+  auto operand = [&](CUtensorMap* m, const cplx* base, long long ld, int rows) {
+    cuuint64_t dims[2] = {(cuuint64_t)2 * ka.K, (cuuint64_t)rows};
+    cuuint64_t strides[1] = {(cuuint64_t)ld * sizeof(cplx)};
+    cuuint32_t box[2] = {16, (cuuint32_t)BM};
+    cuuint32_t es[2] = {1, 1};
+    return encode(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void*)base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+  };
+  if (!operand(&maps.a, ka.A, ka.lda, ka.M) || !operand(&maps.b, ka.B, ka.ldb, ka.N)) return RPA_OK;
+  {
+    cuuint64_t dims[2] = {(cuuint64_t)ka.K, 1};
+    cuuint64_t strides[1] = {(cuuint64_t)(ka.K + (ka.K & 1)) * sizeof(double)};
+    cuuint32_t box[2] = {(cuuint32_t)BK, 1};
+    cuuint32_t es[2] = {1, 1};
+    if (encode(&maps.w, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void*)ka.wk, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return RPA_OK;
+  }
+  constexpr size_t smem = (size_t)TMA_STAGES * 2 * TMA_TILE * sizeof(cplx) + TMA_STAGES * BK * sizeof(double) + 2 * TMA_STAGES * sizeof(unsigned long long) + 128;
+  if (ctx->attr_once(RPA_ATTR_ZGEMM_TMA_MK))
+    RPA_CUDA(ctx, cudaFuncSetAttribute(zgemm_tma_mk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  zgemm_tma_mk_kernel<<<grid, NTHREADS, smem, ctx->stream>>>(ka, maps);
   RPA_LAUNCH_CHECK(ctx);
   *ok = true;
   return RPA_OK;
@@ -586,6 +709,14 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
   bool tma_done = false;
   if (ctx->opt.zgemm_tma && p.herm && p.a_km && p.b_kn && p.conj_b && p.A == p.B && p.lda == p.ldb && p.strideA == p.strideB) {
     if ((rc = launch_tma(ctx, ka, grid, p.batch, &tma_done))) return rc;
+  }
+#ifndef RPA_PROJ_TMA
+#define RPA_PROJ_TMA 1
+#endif
+  // the projection shape: [m][k] x [n][k] conj, weights along k, one split, plain store of alpha * sum
+  if (RPA_PROJ_TMA && ctx->opt.zgemm_tma && !tma_done && !p.a_km && !p.b_kn && p.conj_b && !p.herm && p.batch == 1 && !ka.atomic && !p.accumulate &&
+      !p.rs && !p.cs && p.wk && (p.lda * (long long)sizeof(cplx)) % 16 == 0) {
+    if ((rc = launch_tma_mk(ctx, ka, grid, &tma_done))) return rc;
   }
   if (tma_done) rc = RPA_OK;
   else if (p.a_km && p.b_kn && p.conj_b) rc = launch<true, true, true>(ctx, ka, grid);
