@@ -674,6 +674,40 @@ def test_n_eig_sweep_against_golden(name, idx, n_v, n_c, capsys):
                   f"{m['mtxel']:.1f} {m['chi0_static']:.1f} {m['basis']:.1f} {m['chi_freq']:.1f} {m['energy']:.2f}")
 
 
+def test_degenerate_zero_response_is_handled():
+    """The degenerate input of the method: no response at all (M = 0, e.g. bands without overlap).  chi~0 = 0 exactly,
+    chi_s = 0, E_c = 0; the basis of the zero matrix is any orthonormal set with lambda = 0 -- the library must either
+    return that or refuse with a clean error, never hang or return NaN."""
+    import paper_2405_20258_b200 as rpa
+    import torch
+    inp = make_inputs(0)
+    ng, nv, nc, n_eig = inp.n_g, 2, 19, 12
+    ctx = make_ctx(inp, nv, nc, n_eig, len(inp.omega))
+    try:
+        M = torch.zeros((nv, nc, ng), dtype=torch.complex128, device="cuda")
+        chi = torch.full((ng, ng), 3.0, dtype=torch.complex128, device="cuda")
+        rpa.rpa_chi0_static(ctx, M, dev(inp.e_v[:nv]), dev(inp.e_c[:nc]), False, chi)
+        assert float(chi.abs().max()) == 0.0
+        Cm = torch.empty((n_eig, ng), dtype=torch.complex128, device="cuda")
+        lam = torch.empty(n_eig, dtype=torch.float64, device="cuda")
+        try:
+            rpa.rpa_subspace_basis(ctx, chi, n_eig, 0.0, Cm, lam)
+            Cg, lg = Cm.cpu().numpy(), lam.cpu().numpy()
+            assert np.all(np.isfinite(Cg)) and np.all(lg == 0.0)
+            assert np.abs(Cg.conj() @ Cg.T - np.eye(n_eig)).max() <= 1e-11
+        except rpa.RpaError as e:                                 # a refusal is acceptable, with the documented code
+            assert e.code in (-5, -1)
+            q, _ = np.linalg.qr(np.random.default_rng(0).standard_normal((ng, n_eig)) + 0j)
+            Cm = dev(np.ascontiguousarray(q.T))
+        chis = torch.full((len(inp.omega), n_eig, n_eig), 2.0, dtype=torch.complex128, device="cuda")
+        rpa.rpa_chi_subspace_freq(ctx, M, dev(inp.e_v[:nv]), dev(inp.e_c[:nc]), Cm, n_eig, dev(inp.omega), False, chis)
+        assert float(chis.abs().max()) == 0.0
+        e, t = rpa.rpa_correlation_energy(ctx, chis, n_eig, dev(inp.weight))
+        assert e == 0.0 and np.all(t == 0.0)
+    finally:
+        rpa.rpa_destroy(ctx)
+
+
 def test_two_contexts_in_one_process_interleaved():
     """Kernel attributes, tuning switches and plans are per context: two contexts with different grids (24^3 and 48 x 48 x 12),
     created one after the other and used alternately, must both give the oracle's M and chi~0(0)."""
