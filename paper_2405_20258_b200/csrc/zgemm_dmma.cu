@@ -380,6 +380,29 @@ __global__ void __launch_bounds__(NTHREADS, 2) zherk_tma_kernel(KArgs p, const _
   if (tid == 0)
     for (int s = 0; s < TMA_STAGES - 1 && s < nkt; s++) issue(s, kt0 + s);
 
+  // Full off-diagonal tiles (the great majority) run a loop of their own with the one 4 x 4 warp shape and no shape
+  // dispatch inside (a CTA-uniform choice, made once): its body holds exactly one DMMA schedule, and the kernel is 2-3 %
+  // faster for it (CHI_SUM(0) 2.738 -> 2.679 s, chi_s 4.264 -> 4.149 s per step at configs[2]).  Diagonal and ragged
+  // tiles take the general loop below; hoisting their shapes out as well was no further gain (more registers).
+  const bool plain_tile = !diag && p.M - m0 >= BM - 8;
+  if (plain_tile) {
+    for (int it = 0; it < nkt; it++) {
+      const int st = it % TMA_STAGES;
+      if (tid == 0) {
+        const int nx = it + TMA_STAGES - 1;
+        if (nx < nkt) {
+          const int sx = nx % TMA_STAGES;
+          if (nx >= TMA_STAGES) tma_mbar_wait(empty + sx, (unsigned)(((nx / TMA_STAGES) - 1) & 1));
+          issue(sx, kt0 + nx);
+        }
+      }
+      __syncwarp();
+      tma_mbar_wait(full + st, (unsigned)((it / TMA_STAGES) & 1));
+      mma_ktile<true, true, true, 4, 4, false, 1>(sA + st * TMA_TILE, sB + st * TMA_TILE, sW + st * BK, g, q, mb, nb, cre, cim);
+      __syncwarp();
+      if (lane == 0) tma_mbar_arrive(empty + st);
+    }
+  } else
   for (int it = 0; it < nkt; it++) {
     const int st = it % TMA_STAGES;
     if (tid == 0) {   // refill the stage all warps left one iteration ago
