@@ -20,6 +20,17 @@ int rpa_fail(rpa_ctx* ctx, int code, const char* fmt, ...) {
 
 namespace {
 
+// Cs[i][G] = C[i][G] v^1/2(G): the Coulomb factor of the projection (eq. 7) folded into the basis once per call,
+// so that the projection GEMM multiplies no weights in its main loop
+__global__ void scale_basis_kernel(const cplx* __restrict__ C, const double* __restrict__ vsqrt, int n_g, long long total,
+                                   cplx* __restrict__ out) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+    const double s = vsqrt[i % n_g];
+    const cplx c = C[i];
+    out[i] = make_double2(c.x * s, c.y * s);
+  }
+}
+
 __global__ void sqrt_kernel(const double* __restrict__ v, int n, double* __restrict__ out) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) out[i] = sqrt(v[i]);
@@ -33,7 +44,8 @@ size_t chi_freq_vchunk(const rpa_ctx* ctx, int nvb, int nc, int n_eig) {
   return std::min<size_t>(vc, (size_t)nvb);
 }
 size_t chi_freq_workspace(const rpa_ctx* ctx, int nvb, int nc, int n_eig, int n_w) {
-  return ws_round(chi_freq_vchunk(ctx, nvb, nc, n_eig) * nc * n_eig * sizeof(cplx)) + ws_round((size_t)n_w * nvb * nc * sizeof(double));
+  return ws_round(chi_freq_vchunk(ctx, nvb, nc, n_eig) * nc * n_eig * sizeof(cplx)) + ws_round((size_t)n_w * nvb * nc * sizeof(double)) +
+         ws_round((size_t)n_eig * ctx->n_g * sizeof(cplx));
 }
 size_t chi0_static_workspace(int nvb, int nc) { return ws_round((size_t)nvb * nc * sizeof(double)); }
 
@@ -75,16 +87,21 @@ int do_chi_freq(rpa_ctx* ctx, WsAlloc& ws, const cplx* M, int nvb, int nc, const
   }
   const int vchunk = (int)chi_freq_vchunk(ctx, nvb, nc, n_eig);
   cplx* Bp = ws.get<cplx>((size_t)vchunk * nc * n_eig);
+  cplx* Cs = ws.get<cplx>((size_t)n_eig * n_g);
   if (!ws.ok) return rpa_fail(ctx, RPA_ERR_WORKSPACE, "rpa_chi_subspace_freq: workspace too small (need %zu bytes)", ws.off);
+  {
+    const long long total = (long long)n_eig * n_g;
+    scale_basis_kernel<<<(unsigned)std::min<long long>((total + 255) / 256, 8192), 256, 0, ctx->stream>>>(C, ctx->d_vsqrt, n_g, total, Cs);
+    RPA_LAUNCH_CHECK(ctx);
+  }
   for (int v0 = 0; v0 < nvb; v0 += vchunk) {
     const int nv = std::min(vchunk, nvb - v0);
     const int P = nv * nc;
     // projection  Bp[p][i] = sum_G M[p][G] v^1/2(G) conj(C[i][G])        (eq. 7)
     ZgemmParams g;
     g.A = M + (long long)v0 * nc * n_g; g.lda = n_g; g.a_km = false;
-    g.B = C; g.ldb = n_g; g.b_kn = false;
+    g.B = Cs; g.ldb = n_g; g.b_kn = false;                                // v^1/2 sits in Cs: no k weights
     g.C = Bp; g.ldc = n_eig; g.M = P; g.N = n_eig; g.K = n_g; g.conj_b = true;
-    g.wk = ctx->d_vsqrt;
     { ProfScope ps(ctx, RPA_PROF_PROJ); rc = zgemm_dmma(ctx, g); }
     if (rc) return rc;
     // chi_s[k] (+)= - sum_p Bp[p][:] D_p(w_k) Bp[p][:]^H                   (eq. 8)

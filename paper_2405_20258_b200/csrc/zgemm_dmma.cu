@@ -82,7 +82,7 @@ __device__ __forceinline__ void load_tile(cplx* s, const cplx* g, long long ld, 
 // Hermitian tile.  TRI = true: three 2 x 2 lower fragment triangles on the diagonal at 0, 24, 48 (slot [t][0] =
 // (24t, 24t), [t][1] = (24t+8, 24t), [t][2] = (24t+8, 24t+8)).  3 x 3 x 3 + TRI tile the 36 fragments on or below the
 // diagonal of a diagonal Hermitian tile, 9 per warp (see the kernel).
-template <bool A_KM, bool B_KN, bool CONJ_B, int NI, int NJ, bool TRI, int BOX = 0>
+template <bool A_KM, bool B_KN, bool CONJ_B, int NI, int NJ, bool TRI, int BOX = 0, bool HASW = true>
 __device__ __forceinline__ void mma_ktile(const cplx* __restrict__ a_s, const cplx* __restrict__ b_s,
                                           const double* __restrict__ w_s, int g, int q, int mb, int nb,
                                           double (&cre)[4][4][2], double (&cim)[4][4][2], bool skip_upper = false) {
@@ -90,7 +90,7 @@ __device__ __forceinline__ void mma_ktile(const cplx* __restrict__ a_s, const cp
 #pragma unroll
   for (int k4 = 0; k4 < BK / 4; k4++) {
     const int k = k4 * 4 + q;
-    const double w = w_s[k];
+    const double w = HASW ? w_s[k] : 1.0;
     double ar[NA], ai[NA], br[NB], bi[NB];
 #pragma unroll
     for (int i = 0; i < NA; i++) {
@@ -101,7 +101,7 @@ __device__ __forceinline__ void mma_ktile(const cplx* __restrict__ a_s, const cp
       cplx a = BOX == 1 ? a_s[((m >> 3) << 7) + k * 8 + ((m & 7) ^ (k & 7))]
              : BOX == 2 ? a_s[((k >> 3) << 9) + m * 8 + ((k & 7) ^ (m & 7))]
              : A_KM ? a_s[k * LD_KM + m] : a_s[m * LD_MK + k];
-      ar[i] = a.x * w; ai[i] = a.y * w;
+      ar[i] = HASW ? a.x * w : a.x; ai[i] = HASW ? a.y * w : a.y;
     }
 #pragma unroll
     for (int j = 0; j < NB; j++) {
@@ -465,6 +465,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) zherk_tma_kernel(KArgs p, const _
 // stores (the projection has tens of thousands of tiles), rows / columns / k beyond the matrix are zero-filled by TMA.
 struct TmaMapsMK { CUtensorMap a; CUtensorMap b; CUtensorMap w; };
 
+template <bool HASW>
 __global__ void __launch_bounds__(NTHREADS, 2) zgemm_tma_mk_kernel(KArgs p, const __grid_constant__ TmaMapsMK maps) {
   extern __shared__ __align__(1024) unsigned char smem_tma[];
   cplx* sA = reinterpret_cast<cplx*>(smem_tma);
@@ -484,7 +485,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_tma_mk_kernel(KArgs p, cons
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
   __syncthreads();
-  constexpr unsigned stage_bytes = (unsigned)(2 * TMA_TILE * sizeof(cplx) + BK * sizeof(double));
+  constexpr unsigned stage_bytes = (unsigned)(2 * TMA_TILE * sizeof(cplx) + (HASW ? BK * sizeof(double) : 0));
   auto issue = [&](int stage, int kt) {   // one thread
     const int k0 = kt * BK;
     tma_mbar_expect(full + stage, stage_bytes);
@@ -493,7 +494,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_tma_mk_kernel(KArgs p, cons
       tma_load_2d(sA + stage * TMA_TILE + b * 512, &maps.a, 2 * (k0 + 8 * b), m0, full + stage);
       tma_load_2d(sB + stage * TMA_TILE + b * 512, &maps.b, 2 * (k0 + 8 * b), n0, full + stage);
     }
-    tma_load_2d(sW + stage * BK, &maps.w, k0, 0, full + stage);
+    if (HASW) tma_load_2d(sW + stage * BK, &maps.w, k0, 0, full + stage);
   };
   const int mb = wm * 32, nb = wn * 32;
   double cre[4][4][2], cim[4][4][2];
@@ -516,7 +517,7 @@ __global__ void __launch_bounds__(NTHREADS, 2) zgemm_tma_mk_kernel(KArgs p, cons
     }
     __syncwarp();
     tma_mbar_wait(full + st, (unsigned)((it / TMA_STAGES) & 1));
-    mma_ktile<false, false, true, 4, 4, false, 2>(sA + st * TMA_TILE, sB + st * TMA_TILE, sW + st * BK, g, q, mb, nb, cre, cim);
+    mma_ktile<false, false, true, 4, 4, false, 2, HASW>(sA + st * TMA_TILE, sB + st * TMA_TILE, sW + st * BK, g, q, mb, nb, cre, cim);
     __syncwarp();
     if (lane == 0) tma_mbar_arrive(empty + st);
   }
@@ -614,6 +615,7 @@ int launch_tma_mk(rpa_ctx* ctx, const KArgs& ka, dim3 grid, bool* ok) {
   }
   auto encode = reinterpret_cast<PFN_cuTensorMapEncodeTiled>(ctx->tma_encode);
   if (((uintptr_t)ka.A & 15) || ((uintptr_t)ka.B & 15) || ((uintptr_t)ka.wk & 15)) return RPA_OK;
+  const bool hasw = ka.wk != nullptr;
   TmaMapsMK maps;
   auto operand = [&](CUtensorMap* m, const cplx* base, long long ld, int rows) {
     cuuint64_t dims[2] = {(cuuint64_t)2 * ka.K, (cuuint64_t)rows};
@@ -624,7 +626,8 @@ int launch_tma_mk(rpa_ctx* ctx, const KArgs& ka, dim3 grid, bool* ok) {
                   CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
   };
   if (!operand(&maps.a, ka.A, ka.lda, ka.M) || !operand(&maps.b, ka.B, ka.ldb, ka.N)) return RPA_OK;
-  {
+  maps.w = maps.a;   // unused without weights
+  if (hasw) {
     cuuint64_t dims[2] = {(cuuint64_t)ka.K, 1};
     cuuint64_t strides[1] = {(cuuint64_t)(ka.K + (ka.K & 1)) * sizeof(double)};
     cuuint32_t box[2] = {(cuuint32_t)BK, 1};
@@ -633,9 +636,12 @@ int launch_tma_mk(rpa_ctx* ctx, const KArgs& ka, dim3 grid, bool* ok) {
                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return RPA_OK;
   }
   constexpr size_t smem = (size_t)TMA_STAGES * 2 * TMA_TILE * sizeof(cplx) + TMA_STAGES * BK * sizeof(double) + 2 * TMA_STAGES * sizeof(unsigned long long) + 128;
-  if (ctx->attr_once(RPA_ATTR_ZGEMM_TMA_MK))
-    RPA_CUDA(ctx, cudaFuncSetAttribute(zgemm_tma_mk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  zgemm_tma_mk_kernel<<<grid, NTHREADS, smem, ctx->stream>>>(ka, maps);
+  if (ctx->attr_once(RPA_ATTR_ZGEMM_TMA_MK)) {
+    RPA_CUDA(ctx, cudaFuncSetAttribute(zgemm_tma_mk_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    RPA_CUDA(ctx, cudaFuncSetAttribute(zgemm_tma_mk_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  }
+  if (hasw) zgemm_tma_mk_kernel<true><<<grid, NTHREADS, smem, ctx->stream>>>(ka, maps);
+  else zgemm_tma_mk_kernel<false><<<grid, NTHREADS, smem, ctx->stream>>>(ka, maps);
   RPA_LAUNCH_CHECK(ctx);
   *ok = true;
   return RPA_OK;
@@ -738,7 +744,7 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
 #endif
   // the projection shape: [m][k] x [n][k] conj, weights along k, one split, plain store of alpha * sum
   if (RPA_PROJ_TMA && ctx->opt.zgemm_tma && !tma_done && !p.a_km && !p.b_kn && p.conj_b && !p.herm && p.batch == 1 && !ka.atomic && !p.accumulate &&
-      !p.rs && !p.cs && p.wk && (p.lda * (long long)sizeof(cplx)) % 16 == 0) {
+      !p.rs && !p.cs && (p.lda * (long long)sizeof(cplx)) % 16 == 0) {
     if ((rc = launch_tma_mk(ctx, ka, grid, &tma_done))) return rc;
   }
   if (tma_done) rc = RPA_OK;
