@@ -101,7 +101,7 @@ int do_chi_freq(rpa_ctx* ctx, WsAlloc& ws, const cplx* M, int nvb, int nc, const
     ZgemmParams g;
     g.A = M + (long long)v0 * nc * n_g; g.lda = n_g; g.a_km = false;
     g.B = Cs; g.ldb = n_g; g.b_kn = false;                                // v^1/2 sits in Cs: no k weights
-    g.C = Bp; g.ldc = n_eig; g.M = P; g.N = n_eig; g.K = n_g; g.conj_b = true;
+    g.C = Bp; g.ldc = n_eig; g.M = P; g.N = n_eig; g.K = n_g; g.conj_b = true; g.tma_mk = true;
     { ProfScope ps(ctx, RPA_PROF_PROJ); rc = zgemm_dmma(ctx, g); }
     if (rc) return rc;
     // chi_s[k] (+)= - sum_p Bp[p][:] D_p(w_k) Bp[p][:]^H                   (eq. 8)

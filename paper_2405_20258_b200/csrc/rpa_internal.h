@@ -159,6 +159,7 @@ struct ZgemmParams {
   const double* wk = nullptr; long long strideW = 0;
   int batch = 1; long long strideA = 0, strideB = 0, strideC = 0;
   int split_k = 0;            // 0 = choose automatically
+  bool tma_mk = false;        // [m][k] x [n][k] product that may take the TMA-staged kernel (the projection asks for it)
 };
 int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p);
 // out[k][v * nc + c] = 2 D/(D^2 + omega_k^2), D = e_c[c] - e_v[v]  (eq. 5 in the reading R6); omega == nullptr: one

@@ -743,7 +743,7 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
 #define RPA_PROJ_TMA 1
 #endif
   // the projection shape: [m][k] x [n][k] conj, weights along k, one split, plain store of alpha * sum
-  if (RPA_PROJ_TMA && ctx->opt.zgemm_tma && !tma_done && !p.a_km && !p.b_kn && p.conj_b && !p.herm && p.batch == 1 && !ka.atomic && !p.accumulate &&
+  if (RPA_PROJ_TMA && p.tma_mk && ctx->opt.zgemm_tma && !tma_done && !p.a_km && !p.b_kn && p.conj_b && !p.herm && p.batch == 1 && !ka.atomic && !p.accumulate &&
       !p.rs && !p.cs && (p.lda * (long long)sizeof(cplx)) % 16 == 0) {
     if ((rc = launch_tma_mk(ctx, ka, grid, &tma_done))) return rc;
   }
