@@ -676,6 +676,9 @@ int zgemm_dmma(rpa_ctx* ctx, const ZgemmParams& p) {
   const int n_kt = (p.K + BK - 1) / BK;
   ka.n_kt = n_kt;
   int split = p.split_k;
+  // the projection's TMA kernel takes one k-split and plain stores: with several waves of tiles that beats trimming the last
+  // partial wave by a split (which would send it to the cp.async kernel and its atomics)
+  if (split <= 0 && p.tma_mk && ctx->opt.zgemm_tma && !p.herm && p.batch == 1 && tiles >= 4LL * 2 * ctx->sm_count) split = 1;
   if (split <= 0) {
     // pick the split that fills whole waves of (2 CTAs per SM): maximise CTAs / (waves * slots)
     const long long slots = 2LL * ctx->sm_count;
