@@ -243,12 +243,13 @@ __device__ __forceinline__ void pair_plane_fft8_body(const cplx* __restrict__ u_
 
 // ---------------------------------------------------------------------------------------------------------------
 // Ring variant of the same kernel (used where only ONE CTA fits per SM: N = 48, 64).  There is no block barrier in the
-// band loop: the column buffer is a ring of RING_D bands guarded by mbarriers (full[b]: all warps have written their rows
+// band loop: the column buffer is a ring of D = RingDepth<N>::value bands guarded by mbarriers (full[b]: all warps have written their rows
 // of the band into cb[b]; empty[b]: the x transforms of that band are done and cb[b] may be overwritten).  The x
 // transforms of band v are dealt, in batches of RW kept columns, to ncb warps that rotate with v, and a warp takes that
 // duty one band late -- so a warp with column duty falls behind by one duty and catches up while the others carry the
 // next bands, instead of every warp idling at a barrier while ncb of them transform columns.
-constexpr int RING_D = 3;
+// ring depth: 3 bands; 4 where shared memory allows it next to two u_c planes (N = 48: -1 % time), not at N = 64 (227 KB)
+template <int N> struct RingDepth { static constexpr int value = N == 48 ? 4 : 3; };
 
 __device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
@@ -301,7 +302,7 @@ __device__ __forceinline__ void pair_plane_fft8_ring_body(const cplx* __restrict
                                                           int N3, const cplx* __restrict__ tw, const int* __restrict__ kfreq1,
                                                           const int* __restrict__ kfreq2, int nk1, int nk2, cplx* __restrict__ T) {
   using GE = Geo<N>;
-  constexpr int R2 = GE::R2, RW = GE::RW, NWARP = GE::NWARP, G = GE::G, PS = GE::PS, PW = GE::PW, PC = GE::PC, D = RING_D;
+  constexpr int R2 = GE::R2, RW = GE::RW, NWARP = GE::NWARP, G = GE::G, PS = GE::PS, PW = GE::PW, PC = GE::PC, D = RingDepth<N>::value;
   constexpr int NTHR = NWARP * 32;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx* sc = reinterpret_cast<cplx*>(smem_raw);   // [CB][N][PS]  u_c planes
@@ -511,7 +512,7 @@ size_t smem_bytes(int nk1, int nk2) {
 namespace fft8 {
 template <int N>
 size_t smem_bytes_ring(int nk2, int cb = 1) {
-  return ((size_t)cb * N * Geo<N>::PS + (size_t)N * Geo<N>::PW + (size_t)RING_D * nk2 * Geo<N>::PC) * sizeof(cplx) +
-         (16 + 2 * RING_D) * sizeof(unsigned long long);
+  return ((size_t)cb * N * Geo<N>::PS + (size_t)N * Geo<N>::PW + (size_t)RingDepth<N>::value * nk2 * Geo<N>::PC) * sizeof(cplx) +
+         (16 + 2 * RingDepth<N>::value) * sizeof(unsigned long long);
 }
 }  // namespace fft8
